@@ -1,0 +1,135 @@
+/*
+ * prs.h -- C ABI of libprs: the Press-Ryden-Spergel (PRS) domain-wall step on one NVIDIA B200.
+ *
+ * The library advances a real scalar field phi on a periodic N^dims lattice (dims = 2 or 3, dx = 1)
+ * with the damped staggered leapfrog of arxiv 1710.10420 (Eqs. 3-6, :46-55) for the quartic
+ * potential of Eq. 1 (:30), and measures the two wall diagnostics of Eqs. 7-8 (:57-66).  Every step of
+ * that path runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * State held between calls: phi^n and phidot^{n-1/2} with step counter n, eta_n = eta0 + n*deta.
+ *
+ * Memory and ownership
+ *   - The CALLER owns the device workspace (prs_workspace_bytes() bytes, 256-byte aligned DEVICE
+ *     pointer, e.g. torch.empty(nbytes, dtype=uint8, device="cuda").data_ptr()) and the CUDA stream
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream).  The library carves the
+ *     workspace into its field arrays and reduction scratch, never allocates or frees device memory,
+ *     and launches everything on that stream.
+ *   - Fields are dense T[N^dims], linear index s = x + N*(y + N*z), x fastest; T = float
+ *     (PRS_F32) or double (PRS_F64).
+ *   - prs_destroy frees only host-side bookkeeping (and a few bytes of pinned host memory).
+ *
+ * Errors: every function returns PRS_OK (0) or a PRS_ERR_* code; nothing throws, aborts or prints.
+ * On error out-parameters are untouched.  prs_last_error(h) gives a text for the last failure on h
+ * (handle-owned, valid until the next call on h).  Asynchronous CUDA faults surface at the next
+ * synchronising call (prs_diagnostics, prs_copy_out, prs_copy_in, prs_sync).
+ * A handle is not thread-safe; distinct handles are independent.
+ */
+#ifndef PRS_H
+#define PRS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct prs_ctx* prs_handle;
+
+enum { PRS_OK = 0, PRS_ERR_INVALID_ARG = 1, PRS_ERR_UNSUPPORTED = 2, PRS_ERR_WORKSPACE = 3,
+       PRS_ERR_STATE = 4, PRS_ERR_CUDA = 5 };
+
+enum { PRS_F32 = 0, PRS_F64 = 1 };
+
+/* Diagnostics of the state in memory (phi^n, phidot^{n-1/2}); Eqs. 7-8 with the readings
+ * of DESIGN.md section 3. */
+typedef struct {
+    int64_t  step;        /* n                                                                    */
+    double   eta;         /* eta_n                                                                */
+    uint64_t link_count;  /* C: forward nearest-neighbour links (d per site, periodic) whose two   *
+                           * ends differ in IEEE sign bit (Eq. 7's sum of delta_pm) -- bit-exact   */
+    uint64_t wall_sites;  /* N_w: sites touching at least one crossing link (Eq. 8's N)            */
+    double   sum_ratio;   /* sum over wall sites of phidot^2 / V(phi), in double (0 where V == 0)  */
+    double   rho;         /* C / N^dims   (Eq. 7 with Delta A = 1, unweighted)                     */
+    double   gv2;         /* sum_ratio / (2 N_w), 0 if N_w == 0   (Eq. 8)                          */
+} prs_diag;
+
+/* Options for prs_set_option (all have defaults; tests use them to force one kernel). */
+enum {
+    PRS_OPT_STEP_KERNEL = 1,   /* PRS_KERNEL_*                                   default AUTO     */
+    PRS_OPT_ARITH       = 2,   /* PRS_ARITH_*                                    default COEF     */
+    PRS_OPT_DIAG_KERNEL = 3,   /* PRS_KERNEL_AUTO / GENERIC / TILED              default AUTO     */
+    PRS_OPT_CHUNK       = 4,   /* tuning: planes (3D) / rows (2D) one CTA marches; 0 = auto        */
+    PRS_OPT_TILE_Y      = 5    /* tuning: rows per CTA of the 3D tiled kernels, 4 / 8 / 16         */
+};
+enum {
+    PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */
+    PRS_KERNEL_GENERIC = 1,    /* one thread per site, any N >= 1                                  */
+    PRS_KERNEL_TILED   = 2,    /* shared-memory tiled, one step per pass over HBM                  */
+    PRS_KERNEL_TB2     = 3     /* temporally blocked: two steps per pass over HBM (same per-site   *
+                                * arithmetic, bit-identical to two single steps)                   */
+};
+/* Velocity update, Eq. 4 (:49): LITERAL divides per site, ((1-d)*v + deta*f)/(1+d); COEF uses
+ * A = (1-d)/(1+d) and B = deta/(1+d) formed in double on the host once per step, v' = A*v + B*f.
+ * Neither ever contracts a multiply and an add into an FMA, so each matches the oracle's
+ * arithmetic of the same name bit for bit. */
+enum { PRS_ARITH_LITERAL = 0, PRS_ARITH_COEF = 1 };
+
+/* Read-only counters for prs_get_info. */
+enum {
+    PRS_INFO_KERNEL_LAUNCHES = 1,  /* kernels launched on behalf of this handle since creation     */
+    PRS_INFO_STEP_KERNEL     = 2,  /* PRS_KERNEL_* actually used by the last prs_step              */
+    PRS_INFO_STEP            = 3,  /* n                                                            */
+    PRS_INFO_DIAG_KERNEL     = 4   /* PRS_KERNEL_* actually used by the last prs_diagnostics       */
+};
+
+/* Bytes of device workspace needed; 0 if the arguments are invalid. */
+size_t prs_workspace_bytes(int dims, int64_t N, int precision);
+
+/* Creates a simulation.  dims in {2,3}; N >= 1 sites per side; precision PRS_F32/PRS_F64;
+ * alpha >= 0 (PRS: 3) multiplies the friction term of Eq. 2 (:34); era_m = dln a/dln eta >= 0
+ * (1 radiation, 2 matter, 0 = no expansion); deta > 0 the conformal time step; W0 > 0 the wall
+ * thickness, which sets V0 = pi^2 phi0^2 / (2 W0^2); phi0 > 0 the vacuum value; seed keys the
+ * initial-condition generator.  workspace: DEVICE pointer (see above); cuda_stream: cudaStream_t. */
+int prs_create(prs_handle* out, int dims, int64_t N, int precision,
+               double alpha, double era_m, double deta, double W0, double phi0, uint64_t seed,
+               void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+int prs_destroy(prs_handle h);
+
+/* Seeded initial condition: phi_s = phi0 * u_s, u_s an odd multiple of 2^-24
+ * in (-1,1) drawn from Philox4x32-10(counter = s>>2, key = seed), word s&3; phidot = +0; n = 0,
+ * eta = eta0 > 0.  Asynchronous on the stream. */
+int prs_init(prs_handle h, double eta0);
+
+/* Advances nsteps >= 0 steps of Eqs. 3-6.  Asynchronous on the stream; no host sync, no transfer. */
+int prs_step(prs_handle h, int64_t nsteps);
+
+/* Measures Eqs. 7-8 on the current state; synchronises the stream; fills *out (HOST pointer). */
+int prs_diagnostics(prs_handle h, prs_diag* out);
+
+/* Snapshot: copies phi^n and/or phidot^{n-1/2} (T[N^dims]) to HOST or DEVICE memory (either pointer
+ * may be NULL); synchronises the stream. */
+int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst);
+
+/* Restores a state from HOST or DEVICE memory (both required) and sets eta0 > 0, n = step >= 0, so
+ * that eta_n = eta0 + n*deta; synchronises the stream. */
+int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, double eta0, int64_t step);
+
+/* Blocks until everything queued for h has finished; reports a pending asynchronous CUDA fault. */
+int prs_sync(prs_handle h);
+
+int prs_set_option(prs_handle h, int option, int64_t value);   /* PRS_ERR_UNSUPPORTED if the kernel  *
+                                                                * cannot take this (dims, N, T)      */
+int prs_get_info(prs_handle h, int info, int64_t* value);
+
+/* DEVICE pointers to the current phi^n and phidot^{n-1/2} arrays (valid until the next prs_step /
+ * prs_copy_in / prs_init): lets a caller (e.g. a torch tensor view) read the state without a copy. */
+int prs_device_pointers(prs_handle h, void** phi, void** phidot);
+
+const char* prs_last_error(prs_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

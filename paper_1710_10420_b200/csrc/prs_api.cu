@@ -1,0 +1,429 @@
+// prs_api.cu -- host side of libprs: context, workspace carving, per-step scalars, kernel selection
+// and launch, and the C ABI declared in include/prs.h.  No device memory is allocated here: the
+// caller's workspace holds everything (see prs.h, "Memory and ownership").
+#include "../../include/prs.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include <cuda_runtime.h>
+
+#include "prs_arith.cuh"
+#include "prs_kernels_generic.cuh"
+#include "prs_kernels_tiled.cuh"
+
+using namespace prs;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+constexpr int MAX_PARTIALS = 4096;           // upper bound on diagnostics blocks
+
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+inline bool args_ok(int dims, int64_t N, int precision) {
+    if (dims != 2 && dims != 3) return false;
+    if (N < 1 || N > (int64_t)1 << 20) return false;
+    if (precision != PRS_F32 && precision != PRS_F64) return false;
+    if (dims == 3 && N > 8192) return false;   // 8192^3 * 4 arrays would not fit anyway
+    return true;
+}
+
+inline size_t sites_of(int dims, int64_t N) { return dims == 3 ? (size_t)N * N * N : (size_t)N * N; }
+
+struct Layout {
+    size_t field_bytes, off_phi[2], off_pd[2], off_partials, off_result, total;
+};
+
+Layout layout_of(int dims, int64_t N, int precision) {
+    Layout L;
+    L.field_bytes = align_up(sites_of(dims, N) * (precision == PRS_F32 ? 4 : 8));
+    size_t o = 0;
+    L.off_phi[0] = o; o += L.field_bytes;
+    L.off_phi[1] = o; o += L.field_bytes;
+    L.off_pd[0] = o; o += L.field_bytes;
+    L.off_pd[1] = o; o += L.field_bytes;
+    L.off_partials = o; o += align_up(sizeof(DiagPartial) * MAX_PARTIALS);
+    L.off_result = o; o += align_up(sizeof(DiagPartial));
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+struct prs_ctx {
+    int dims, precision;
+    int64_t N;
+    size_t S;
+    double alpha, era_m, deta, W0, phi0;
+    uint64_t seed;
+    cudaStream_t stream;
+    char* ws;
+    void* phi[2];
+    void* pd[2];
+    int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
+    DiagPartial* partials;
+    DiagPartial* d_result;
+    DiagPartial* h_result;                    // pinned host, 24 bytes
+    double eta0;
+    int64_t step;
+    bool inited;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y;
+    int last_step_kernel, last_diag_kernel;
+    int64_t launches;
+    int sm_count;
+    std::string err;
+};
+
+namespace {
+
+int fail(prs_ctx* h, int code, const std::string& msg) {
+    if (h) h->err = msg;
+    return code;
+}
+
+int cuda_fail(prs_ctx* h, cudaError_t e, const char* where) {
+    return fail(h, PRS_ERR_CUDA, std::string(where) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")");
+}
+
+#define PRS_CUDA(h, call)                                        \
+    do {                                                         \
+        cudaError_t e_ = (call);                                 \
+        if (e_ != cudaSuccess) return cuda_fail((h), e_, #call); \
+    } while (0)
+
+// Per-step scalars, Eq. 6 (:55) and the constants of Eq. 1 (:30); all in double, rounded to
+// the field type once.  eta_n = eta0 + n*deta is formed from n each time, never accumulated.
+template <typename T>
+StepCoef<T> coef_at(const prs_ctx* h, int64_t n) {
+    const double pi = 3.14159265358979323846;
+    const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0);
+    const double K = 4.0 * V0 / (h->phi0 * h->phi0);
+    const double I = 1.0 / (h->phi0 * h->phi0);
+    const double eta = h->eta0 + (double)n * h->deta;
+    const double delta = ((0.5 * h->alpha) * (h->deta / eta)) * h->era_m;
+    StepCoef<T> k;
+    k.K = (T)K;
+    k.I = (T)I;
+    k.deta = (T)h->deta;
+    const T dT = (T)delta;
+    k.omd = T(1) - dT;
+    k.opd = T(1) + dT;
+    k.A = (T)((1.0 - delta) / (1.0 + delta));
+    k.B = (T)(h->deta / (1.0 + delta));
+    return k;
+}
+
+inline int vec_width(int precision) { return precision == PRS_F32 ? 4 : 2; }
+
+bool tiled_supported(const prs_ctx* h) {
+    const int W = vec_width(h->precision);
+    return h->N % W == 0 && h->N >= W && h->N <= (1 << 30);
+}
+
+int resolve_step_kernel(const prs_ctx* h) {
+    int want = h->opt_step_kernel;
+    if (want == PRS_KERNEL_AUTO) want = tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
+    return want;
+}
+
+// ---- launches -----------------------------------------------------------------------------------
+
+template <typename T, int DIMS, bool LITERAL>
+cudaError_t launch_generic(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
+    const unsigned blocks = (unsigned)((h->S + 255) / 256);
+    step_generic_kernel<T, DIMS, LITERAL><<<blocks, 256, 0, h->stream>>>(p, v, pn, vn, (long long)h->N,
+                                                                         (long long)h->S, k);
+    return cudaGetLastError();
+}
+
+int pick_chunk(const prs_ctx* h, long long tiles_per_slab, int threads_per_cta) {
+    if (h->opt_chunk > 0) return (int)std::min<int64_t>(h->opt_chunk, h->N);
+    // Short chunks win (measured, 1024^3: 8 planes 2.71 ms, 128 planes 2.74 ms, 1024 planes 2.87 ms):
+    // the grid sweeps the march axis chunk by chunk in launch order, so the two halo planes of a
+    // chunk are still in L2 from its predecessor, and many small CTAs balance the tail.  Keep at
+    // least ~16 waves of CTAs and chunks between 8 and 32 long.
+    const long long resident = (long long)h->sm_count * (1024 / threads_per_cta);
+    const long long want_ctas = 16 * resident;
+    long long chunks = (want_ctas + tiles_per_slab - 1) / tiles_per_slab;
+    if (chunks < 1) chunks = 1;
+    long long len = h->N / chunks;
+    if (len > 32) len = 32;
+    if (len < 8) len = 8;
+    if (len > h->N) len = h->N;
+    return (int)len;
+}
+
+template <typename T, bool LITERAL>
+cudaError_t launch_tiled3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N;
+    const int ty = h->opt_tile_y;
+    const unsigned gx = (unsigned)((N + 32 * W - 1) / (32 * W)), gy = (unsigned)((N + ty - 1) / ty);
+    const int ZC = pick_chunk(h, (long long)gx * gy, 32 * ty);
+    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const dim3 block(32, ty, 1);
+    if (ty == 4) step3d_tiled_kernel<T, LITERAL, 4><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    else if (ty == 16) step3d_tiled_kernel<T, LITERAL, 16><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    else step3d_tiled_kernel<T, LITERAL, 8><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    return cudaGetLastError();
+}
+
+template <typename T, bool LITERAL>
+cudaError_t launch_tiled2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N;
+    const int BX = 128;
+    const unsigned gx = (unsigned)((N + BX * W - 1) / (BX * W));
+    const int YC = pick_chunk(h, gx, BX);
+    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
+    step2d_tiled_kernel<T, LITERAL><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k);
+    return cudaGetLastError();
+}
+
+template <typename T>
+int step_once(prs_ctx* h, int kernel) {
+    const StepCoef<T> k = coef_at<T>(h, h->step);
+    const T* p = (const T*)h->phi[h->cur];
+    const T* v = (const T*)h->pd[h->cur];
+    T* pn = (T*)h->phi[h->cur ^ 1];
+    T* vn = (T*)h->pd[h->cur ^ 1];
+    const bool lit = (h->opt_arith == PRS_ARITH_LITERAL);
+    cudaError_t e;
+    if (kernel == PRS_KERNEL_TILED) {
+        if (h->dims == 3) e = lit ? launch_tiled3d<T, true>(h, p, v, pn, vn, k) : launch_tiled3d<T, false>(h, p, v, pn, vn, k);
+        else e = lit ? launch_tiled2d<T, true>(h, p, v, pn, vn, k) : launch_tiled2d<T, false>(h, p, v, pn, vn, k);
+    } else {
+        if (h->dims == 3) e = lit ? launch_generic<T, 3, true>(h, p, v, pn, vn, k) : launch_generic<T, 3, false>(h, p, v, pn, vn, k);
+        else e = lit ? launch_generic<T, 2, true>(h, p, v, pn, vn, k) : launch_generic<T, 2, false>(h, p, v, pn, vn, k);
+    }
+    if (e != cudaSuccess) return cuda_fail(h, e, "step kernel launch");
+    h->launches += 1;
+    h->cur ^= 1;
+    h->step += 1;
+    return PRS_OK;
+}
+
+template <typename T>
+int diag_launch(prs_ctx* h) {
+    const double pi = 3.14159265358979323846;
+    const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0);
+    const double I = 1.0 / (h->phi0 * h->phi0);
+    const T* p = (const T*)h->phi[h->cur];
+    const T* v = (const T*)h->pd[h->cur];
+    long long blocks = (long long)((h->S + 255) / 256);
+    const long long cap = std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 8);
+    if (blocks > cap) blocks = cap;
+    if (h->dims == 3)
+        diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+    else
+        diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics kernel launch");
+    diag_finalize_kernel<<<1, 1024, 0, h->stream>>>(h->partials, (int)blocks, h->d_result);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics finalize launch");
+    h->launches += 2;
+    h->last_diag_kernel = PRS_KERNEL_GENERIC;
+    return PRS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t prs_workspace_bytes(int dims, int64_t N, int precision) {
+    if (!args_ok(dims, N, precision)) return 0;
+    return layout_of(dims, N, precision).total;
+}
+
+int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha, double era_m, double deta,
+               double W0, double phi0, uint64_t seed, void* workspace, size_t workspace_bytes,
+               void* cuda_stream) {
+    if (!out) return PRS_ERR_INVALID_ARG;
+    if (!args_ok(dims, N, precision)) return PRS_ERR_INVALID_ARG;
+    if (!(deta > 0.0) || !(W0 > 0.0) || !(phi0 > 0.0) || !(alpha >= 0.0) || !(era_m >= 0.0))
+        return PRS_ERR_INVALID_ARG;
+    if (!std::isfinite(deta) || !std::isfinite(W0) || !std::isfinite(phi0) || !std::isfinite(alpha) ||
+        !std::isfinite(era_m))
+        return PRS_ERR_INVALID_ARG;
+    const Layout L = layout_of(dims, N, precision);
+    if (!workspace || workspace_bytes < L.total || ((uintptr_t)workspace % ALIGN) != 0) return PRS_ERR_WORKSPACE;
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return PRS_ERR_WORKSPACE;
+    }
+    prs_ctx* h = new (std::nothrow) prs_ctx();
+    if (!h) return PRS_ERR_INVALID_ARG;
+    h->dims = dims; h->precision = precision; h->N = N; h->S = sites_of(dims, N);
+    h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0; h->seed = seed;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->ws = (char*)workspace;
+    h->phi[0] = h->ws + L.off_phi[0]; h->phi[1] = h->ws + L.off_phi[1];
+    h->pd[0] = h->ws + L.off_pd[0]; h->pd[1] = h->ws + L.off_pd[1];
+    h->partials = (DiagPartial*)(h->ws + L.off_partials);
+    h->d_result = (DiagPartial*)(h->ws + L.off_result);
+    h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
+    h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_COEF; h->opt_diag_kernel = PRS_KERNEL_AUTO;
+    h->opt_chunk = 0; h->opt_tile_y = 4;
+    h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
+    h->h_result = nullptr;
+    int dev = attr.device;
+    if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) h->sm_count = 148;
+    if (cudaHostAlloc((void**)&h->h_result, sizeof(DiagPartial), cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        delete h;
+        return PRS_ERR_CUDA;
+    }
+    *out = h;
+    return PRS_OK;
+}
+
+int prs_destroy(prs_handle h) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (h->h_result) cudaFreeHost(h->h_result);
+    delete h;
+    return PRS_OK;
+}
+
+int prs_init(prs_handle h, double eta0) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!(eta0 > 0.0) || !std::isfinite(eta0)) return fail(h, PRS_ERR_INVALID_ARG, "prs_init: eta0 must be > 0");
+    const long long nquads = (long long)((h->S + 3) / 4);
+    long long blocks = (nquads + 255) / 256;
+    const long long cap = (long long)h->sm_count * 32;
+    if (blocks > cap) blocks = cap;
+    h->cur = 0;
+    if (h->precision == PRS_F32)
+        init_kernel<float><<<(unsigned)blocks, 256, 0, h->stream>>>((float*)h->phi[0], (float*)h->pd[0], (long long)h->S, h->seed, h->phi0);
+    else
+        init_kernel<double><<<(unsigned)blocks, 256, 0, h->stream>>>((double*)h->phi[0], (double*)h->pd[0], (long long)h->S, h->seed, h->phi0);
+    PRS_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    h->eta0 = eta0; h->step = 0; h->inited = true;
+    return PRS_OK;
+}
+
+int prs_step(prs_handle h, int64_t nsteps) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (nsteps < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_step: nsteps must be >= 0");
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
+    const int kernel = resolve_step_kernel(h);
+    for (int64_t i = 0; i < nsteps; ++i) {
+        const int rc = (h->precision == PRS_F32) ? step_once<float>(h, kernel) : step_once<double>(h, kernel);
+        if (rc != PRS_OK) return rc;
+    }
+    if (nsteps > 0) h->last_step_kernel = kernel;
+    return PRS_OK;
+}
+
+int prs_diagnostics(prs_handle h, prs_diag* out) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!out) return fail(h, PRS_ERR_INVALID_ARG, "prs_diagnostics: out is NULL");
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_diagnostics: call prs_init or prs_copy_in first");
+    const int rc = (h->precision == PRS_F32) ? diag_launch<float>(h) : diag_launch<double>(h);
+    if (rc != PRS_OK) return rc;
+    PRS_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, h->stream));
+    PRS_CUDA(h, cudaStreamSynchronize(h->stream));
+    prs_diag d;
+    d.step = h->step;
+    d.eta = h->eta0 + (double)h->step * h->deta;
+    d.link_count = h->h_result->links;
+    d.wall_sites = h->h_result->walls;
+    d.sum_ratio = h->h_result->sum;
+    d.rho = (double)d.link_count / (double)h->S;
+    d.gv2 = d.wall_sites ? d.sum_ratio / (2.0 * (double)d.wall_sites) : 0.0;
+    *out = d;
+    return PRS_OK;
+}
+
+int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_copy_out: no state yet");
+    const size_t bytes = h->S * (h->precision == PRS_F32 ? 4 : 8);
+    if (phi_dst) PRS_CUDA(h, cudaMemcpyAsync(phi_dst, h->phi[h->cur], bytes, cudaMemcpyDefault, h->stream));
+    if (phidot_dst) PRS_CUDA(h, cudaMemcpyAsync(phidot_dst, h->pd[h->cur], bytes, cudaMemcpyDefault, h->stream));
+    PRS_CUDA(h, cudaStreamSynchronize(h->stream));
+    return PRS_OK;
+}
+
+int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, double eta0, int64_t step) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!phi_src || !phidot_src) return fail(h, PRS_ERR_INVALID_ARG, "prs_copy_in: both fields are required");
+    if (!(eta0 > 0.0) || !std::isfinite(eta0) || step < 0)
+        return fail(h, PRS_ERR_INVALID_ARG, "prs_copy_in: eta0 must be > 0 and step >= 0");
+    const size_t bytes = h->S * (h->precision == PRS_F32 ? 4 : 8);
+    PRS_CUDA(h, cudaMemcpyAsync(h->phi[h->cur], phi_src, bytes, cudaMemcpyDefault, h->stream));
+    PRS_CUDA(h, cudaMemcpyAsync(h->pd[h->cur], phidot_src, bytes, cudaMemcpyDefault, h->stream));
+    PRS_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->eta0 = eta0; h->step = step; h->inited = true;
+    return PRS_OK;
+}
+
+int prs_sync(prs_handle h) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_CUDA(h, cudaStreamSynchronize(h->stream));
+    return PRS_OK;
+}
+
+int prs_set_option(prs_handle h, int option, int64_t value) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    switch (option) {
+        case PRS_OPT_STEP_KERNEL:
+            if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
+            if (value == PRS_KERNEL_TILED) {
+                if (!tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled step kernel needs N to be a multiple of 16 bytes of T");
+                h->opt_step_kernel = (int)value;
+                return PRS_OK;
+            }
+            if (value == PRS_KERNEL_TB2) return fail(h, PRS_ERR_UNSUPPORTED, "temporally blocked kernel is not available for this lattice");
+            return fail(h, PRS_ERR_INVALID_ARG, "unknown step kernel");
+        case PRS_OPT_ARITH:
+            if (value != PRS_ARITH_LITERAL && value != PRS_ARITH_COEF) return fail(h, PRS_ERR_INVALID_ARG, "unknown arithmetic");
+            h->opt_arith = (int)value;
+            return PRS_OK;
+        case PRS_OPT_DIAG_KERNEL:
+            if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_diag_kernel = (int)value; return PRS_OK; }
+            return fail(h, PRS_ERR_UNSUPPORTED, "only the generic diagnostics kernel exists");
+        case PRS_OPT_CHUNK:
+            if (value < 0 || value > (1 << 20)) return fail(h, PRS_ERR_INVALID_ARG, "chunk must be >= 0");
+            h->opt_chunk = (int)value;
+            return PRS_OK;
+        case PRS_OPT_TILE_Y:
+            if (value != 4 && value != 8 && value != 16) return fail(h, PRS_ERR_INVALID_ARG, "tile_y must be 4, 8 or 16");
+            h->opt_tile_y = (int)value;
+            return PRS_OK;
+        default:
+            return fail(h, PRS_ERR_INVALID_ARG, "unknown option");
+    }
+}
+
+int prs_get_info(prs_handle h, int info, int64_t* value) {
+    if (!h || !value) return PRS_ERR_INVALID_ARG;
+    switch (info) {
+        case PRS_INFO_KERNEL_LAUNCHES: *value = h->launches; return PRS_OK;
+        case PRS_INFO_STEP_KERNEL: *value = h->last_step_kernel; return PRS_OK;
+        case PRS_INFO_STEP: *value = h->step; return PRS_OK;
+        case PRS_INFO_DIAG_KERNEL: *value = h->last_diag_kernel; return PRS_OK;
+        default: return fail(h, PRS_ERR_INVALID_ARG, "unknown info key");
+    }
+}
+
+int prs_device_pointers(prs_handle h, void** phi, void** phidot) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_device_pointers: no state yet");
+    if (phi) *phi = h->phi[h->cur];
+    if (phidot) *phidot = h->pd[h->cur];
+    return PRS_OK;
+}
+
+const char* prs_last_error(prs_handle h) {
+    if (!h) return "null handle";
+    return h->err.c_str();
+}
+
+}  // extern "C"

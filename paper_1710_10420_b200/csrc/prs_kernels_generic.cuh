@@ -1,0 +1,180 @@
+// prs_kernels_generic.cuh -- kernels that take any lattice size N >= 1: the seeded initial condition,
+// a one-thread-per-site step, a grid-stride diagnostics pass and the final reduction.
+#pragma once
+
+#include "prs_arith.cuh"
+
+namespace prs {
+
+// ------------------------------------------------------------------------------------------------
+// Initial condition.  Philox4x32-10 (Salmon et al., SC'11): ten rounds of
+// two 32x32->64 multiplies and xors on a 128-bit counter, the 64-bit key bumped by Weyl constants
+// between rounds.  One block of four words serves four consecutive sites.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 ctr, uint2 key) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned int hi0 = __umulhi(0xD2511F53u, ctr.x), lo0 = 0xD2511F53u * ctr.x;
+        const unsigned int hi1 = __umulhi(0xCD9E8D57u, ctr.z), lo1 = 0xCD9E8D57u * ctr.z;
+        ctr = make_uint4(hi1 ^ ctr.y ^ key.x, lo1, hi0 ^ ctr.w ^ key.y, lo0);
+        key.x += 0x9E3779B9u;
+        key.y += 0xBB67AE85u;
+    }
+    return ctr;
+}
+
+template <typename T>
+__device__ __forceinline__ T init_value_from_word(unsigned int w, double phi0) {
+    const int k = (int)(w >> 8);                                   // 24 random bits
+    const double u = (double)(2 * k + 1 - 16777216) * (1.0 / 16777216.0);   // odd multiple of 2^-24
+    return (T)__dmul_rn(phi0, u);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+init_kernel(T* __restrict__ phi, T* __restrict__ phidot, long long S, unsigned long long seed,
+            double phi0) {
+    const long long nquads = (S + 3) >> 2;
+    const uint2 key = make_uint2((unsigned int)(seed & 0xffffffffull), (unsigned int)(seed >> 32));
+    for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < nquads;
+         q += (long long)gridDim.x * blockDim.x) {
+        const uint4 w = philox4x32_10(
+            make_uint4((unsigned int)(q & 0xffffffffll), (unsigned int)((unsigned long long)q >> 32), 0u, 0u), key);
+        const long long s = q << 2;
+        const T v0 = init_value_from_word<T>(w.x, phi0), v1 = init_value_from_word<T>(w.y, phi0);
+        const T v2 = init_value_from_word<T>(w.z, phi0), v3 = init_value_from_word<T>(w.w, phi0);
+        if (s + 3 < S) {           // S is a multiple of 4 whenever N is even: full, aligned quads
+            if (sizeof(T) == 4) {
+                reinterpret_cast<float4*>(phi)[q] = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
+                reinterpret_cast<float4*>(phidot)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+            } else {
+                reinterpret_cast<double2*>(phi)[2 * q] = make_double2((double)v0, (double)v1);
+                reinterpret_cast<double2*>(phi)[2 * q + 1] = make_double2((double)v2, (double)v3);
+                reinterpret_cast<double2*>(phidot)[2 * q] = make_double2(0.0, 0.0);
+                reinterpret_cast<double2*>(phidot)[2 * q + 1] = make_double2(0.0, 0.0);
+            }
+        } else {
+            const T v[4] = {v0, v1, v2, v3};
+            for (int j = 0; j < 4 && s + j < S; ++j) {
+                phi[s + j] = v[j];
+                phidot[s + j] = T(0);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Generic step: one thread per site, neighbours by modulo wrap (Eqs. 3-5).
+// ------------------------------------------------------------------------------------------------
+template <typename T, int DIMS, bool LITERAL>
+__global__ void __launch_bounds__(256)
+step_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
+                    T* __restrict__ phidot_next, long long N, long long S, StepCoef<T> k) {
+    const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const long long x = s % N;
+    const long long yz = s / N;
+    const long long y = (DIMS == 3) ? yz % N : yz;
+    const long long z = (DIMS == 3) ? yz / N : 0;
+    const long long row = s - x;
+    const long long xm = row + (x == 0 ? N - 1 : x - 1), xp = row + (x == N - 1 ? 0 : x + 1);
+    const long long col = s - y * N;
+    const long long ym = col + (y == 0 ? N - 1 : y - 1) * N, yp = col + (y == N - 1 ? 0 : y + 1) * N;
+    T zmv = T(0), zpv = T(0);
+    if (DIMS == 3) {
+        const long long NN = N * N;
+        const long long pil = s - z * NN;
+        zmv = phi[pil + (z == 0 ? N - 1 : z - 1) * NN];
+        zpv = phi[pil + (z == N - 1 ? 0 : z + 1) * NN];
+    }
+    T pn, vn;
+    site_update<T, DIMS, LITERAL>(k, phi[s], phi[xm], phi[xp], phi[ym], phi[yp], zmv, zpv, phidot[s], pn, vn);
+    phi_next[s] = pn;
+    phidot_next[s] = vn;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Block reduction of a DiagPartial: warp shuffles, then one value per warp through shared memory.
+// The order of the double additions is fixed by the launch configuration, so a given (grid, block)
+// gives the same bits every run.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ DiagPartial warp_reduce(DiagPartial p) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        p.links += __shfl_down_sync(0xffffffffu, p.links, off);
+        p.walls += __shfl_down_sync(0xffffffffu, p.walls, off);
+        p.sum = __dadd_rn(p.sum, __shfl_down_sync(0xffffffffu, p.sum, off));
+    }
+    return p;
+}
+
+// All threads of the block must call; the result is valid in thread 0.
+__device__ __forceinline__ DiagPartial block_reduce(DiagPartial p) {
+    __shared__ DiagPartial warp_part[32];
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const int lane = tid & 31, warp = tid >> 5, nwarps = (nthreads + 31) >> 5;
+    p = warp_reduce(p);
+    __syncthreads();                       // protects warp_part when called twice in one kernel
+    if (lane == 0) warp_part[warp] = p;
+    __syncthreads();
+    if (warp == 0) {
+        DiagPartial q = {0ull, 0ull, 0.0};
+        if (lane < nwarps) q = warp_part[lane];
+        p = warp_reduce(q);
+    }
+    return p;
+}
+
+// Generic diagnostics: grid-stride over sites; each site owns its d forward links (Eq. 7) and tests
+// all 2d links for the wall-site predicate (Eq. 8's N).
+template <typename T, int DIMS>
+__global__ void __launch_bounds__(256)
+diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, long long N, long long S,
+                    double V0, double I, DiagPartial* __restrict__ partials) {
+    using A = Ar<T>;
+    DiagPartial acc = {0ull, 0ull, 0.0};
+    for (long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x; s < S;
+         s += (long long)gridDim.x * blockDim.x) {
+        const long long x = s % N;
+        const long long yz = s / N;
+        const long long y = (DIMS == 3) ? yz % N : yz;
+        const long long z = (DIMS == 3) ? yz / N : 0;
+        const long long row = s - x, col = s - y * N;
+        const T c = phi[s];
+        const bool me = A::neg(c);
+        const bool xp = A::neg(phi[row + (x == N - 1 ? 0 : x + 1)]) != me;
+        const bool xm = A::neg(phi[row + (x == 0 ? N - 1 : x - 1)]) != me;
+        const bool yp = A::neg(phi[col + (y == N - 1 ? 0 : y + 1) * N]) != me;
+        const bool ym = A::neg(phi[col + (y == 0 ? N - 1 : y - 1) * N]) != me;
+        bool zp = false, zm = false;
+        if (DIMS == 3) {
+            const long long NN = N * N, pil = s - z * NN;
+            zp = A::neg(phi[pil + (z == N - 1 ? 0 : z + 1) * NN]) != me;
+            zm = A::neg(phi[pil + (z == 0 ? N - 1 : z - 1) * NN]) != me;
+        }
+        acc.links += (unsigned)xp + (unsigned)yp + (unsigned)zp;
+        if (xp | xm | yp | ym | zp | zm) {
+            acc.walls += 1;
+            acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(c, phidot[s], V0, I));
+        }
+    }
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
+// Final reduction of the per-block partials by one block, in a fixed order.
+__global__ void __launch_bounds__(1024)
+diag_finalize_kernel(const DiagPartial* __restrict__ partials, int npartials, DiagPartial* __restrict__ out) {
+    DiagPartial acc = {0ull, 0ull, 0.0};
+    for (int i = threadIdx.x; i < npartials; i += blockDim.x) {
+        const DiagPartial p = partials[i];
+        acc.links += p.links;
+        acc.walls += p.walls;
+        acc.sum = __dadd_rn(acc.sum, p.sum);
+    }
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0) *out = acc;
+}
+
+}  // namespace prs

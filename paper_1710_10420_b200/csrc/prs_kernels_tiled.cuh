@@ -1,0 +1,197 @@
+// prs_kernels_tiled.cuh -- single-step kernels for HBM-bound lattices (N a multiple of the 16-byte
+// vector width): one pass reads phi^n and phidot^{n-1/2} once and writes phidot^{n+1/2} and
+// phi^{n+1} once (Eqs. 3-5 fused, ":101 concatenation of kernels").
+//
+// Layout of the work.  A thread owns one 16-byte vector of consecutive x (4 floats / 2 doubles) and
+// marches along the slowest axis (z in 3D, y in 2D) keeping a three-deep register window of its own
+// column, so the neighbours along the march axis cost no memory traffic at all.  In-row neighbours
+// x-1 / x+VEC come from the adjacent lanes by warp shuffle; only the two edge lanes of a warp issue a
+// scalar load (an L1/L2 hit: the line belongs to the neighbouring warp's tile).  In 3D the y-1 / y+1
+// rows are 16-byte loads of lines that a neighbouring warp of the same CTA (or, at the tile edge, a
+// neighbouring CTA marching the same planes) has just pulled in, i.e. L1 / L2 hits.  All loads of
+// iteration z+1 are issued before the arithmetic of iteration z (one-deep software pipeline), so each
+// thread keeps two 16-byte DRAM requests in flight.
+#pragma once
+
+#include "prs_arith.cuh"
+
+namespace prs {
+
+template <typename T> struct VecOps;
+
+template <> struct VecOps<float> {
+    typedef float4 V;
+    static constexpr int W = 4;
+    static __device__ __forceinline__ V ld(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+    static __device__ __forceinline__ void st(float* p, V v) { *reinterpret_cast<float4*>(p) = v; }
+    static __device__ __forceinline__ float first(V v) { return v.x; }
+    static __device__ __forceinline__ float last(V v) { return v.w; }
+    static __device__ __forceinline__ float get(V v, int i) { return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w; }
+    static __device__ __forceinline__ void set(V& v, int i, float a) {
+        if (i == 0) v.x = a; else if (i == 1) v.y = a; else if (i == 2) v.z = a; else v.w = a;
+    }
+};
+
+template <> struct VecOps<double> {
+    typedef double2 V;
+    static constexpr int W = 2;
+    static __device__ __forceinline__ V ld(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+    static __device__ __forceinline__ void st(double* p, V v) { *reinterpret_cast<double2*>(p) = v; }
+    static __device__ __forceinline__ double first(V v) { return v.x; }
+    static __device__ __forceinline__ double last(V v) { return v.y; }
+    static __device__ __forceinline__ double get(V v, int i) { return i == 0 ? v.x : v.y; }
+    static __device__ __forceinline__ void set(V& v, int i, double a) {
+        if (i == 0) v.x = a; else v.y = a;
+    }
+};
+
+// One vector of sites: c = centre vector, left/right = the scalars beside it in x, (ym, yp) and
+// (zm, zp) the vectors beside it along the other axes.
+template <typename T, int DIMS, bool LITERAL>
+__device__ __forceinline__ void vector_update(const StepCoef<T>& k, typename VecOps<T>::V c, T left, T right,
+                                              typename VecOps<T>::V ym, typename VecOps<T>::V yp,
+                                              typename VecOps<T>::V zm, typename VecOps<T>::V zp,
+                                              typename VecOps<T>::V pd, typename VecOps<T>::V& phi_new,
+                                              typename VecOps<T>::V& pd_new) {
+    using O = VecOps<T>;
+#pragma unroll
+    for (int i = 0; i < O::W; ++i) {
+        const T xm = (i == 0) ? left : O::get(c, i - 1);
+        const T xp = (i == O::W - 1) ? right : O::get(c, i + 1);
+        T pn, vn;
+        site_update<T, DIMS, LITERAL>(k, O::get(c, i), xm, xp, O::get(ym, i), O::get(yp, i), O::get(zm, i),
+                                      O::get(zp, i), O::get(pd, i), pn, vn);
+        O::set(phi_new, i, pn);
+        O::set(pd_new, i, vn);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// 3D: block = 32 lanes in x  x  TYB rows in y; grid = (x tiles, y tiles, z chunks of ZC planes).
+// ------------------------------------------------------------------------------------------------
+template <typename T, bool LITERAL, int TYB>
+__global__ void __launch_bounds__(32 * TYB)
+step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
+                    T* __restrict__ phidot_next, int N, int ZC, StepCoef<T> k) {
+    using O = VecOps<T>;
+    using V = typename O::V;
+    constexpr int W = O::W;
+    const int lane = threadIdx.x;
+    const int y = blockIdx.y * TYB + threadIdx.y;
+    if (y >= N) return;                                   // whole warp leaves together
+    const int xraw = (blockIdx.x * 32 + lane) * W;
+    const bool live = xraw < N;
+    const int x = live ? xraw : N - W;                    // dead lanes shadow a valid address
+    const int z0 = blockIdx.z * ZC;
+    const int z1 = min(z0 + ZC, N);
+    const size_t NN = (size_t)N * N;
+    const int ym = (y == 0) ? N - 1 : y - 1, yp = (y == N - 1) ? 0 : y + 1;
+    const size_t rc = (size_t)y * N + x, rm = (size_t)ym * N + x, rp = (size_t)yp * N + x;
+    const bool edge_l = (lane == 0), edge_r = (lane == 31) || (x + W >= N);
+    const size_t rl = (size_t)y * N + (x == 0 ? N - 1 : x - 1);
+    const size_t rr = (size_t)y * N + (x + W >= N ? 0 : x + W);
+
+    const int zprev = (z0 == 0) ? N - 1 : z0 - 1;
+    const int znext0 = (z0 + 1 == N) ? 0 : z0 + 1;
+    V prev = O::ld(phi + (size_t)zprev * NN + rc);
+    V cur = O::ld(phi + (size_t)z0 * NN + rc);
+    V nxt = O::ld(phi + (size_t)znext0 * NN + rc);
+    V up = O::ld(phi + (size_t)z0 * NN + rp);
+    V dn = O::ld(phi + (size_t)z0 * NN + rm);
+    V pd = O::ld(phidot + (size_t)z0 * NN + rc);
+    T el = T(0), er = T(0);
+    if (edge_l) el = __ldg(phi + (size_t)z0 * NN + rl);
+    if (edge_r) er = __ldg(phi + (size_t)z0 * NN + rr);
+
+    for (int z = z0; z < z1; ++z) {
+        // ---- issue the loads of iteration z+1 first
+        V nn = nxt, up_n = up, dn_n = dn, pd_n = pd;
+        T el_n = el, er_n = er;
+        const int zn = (z + 1 == N) ? 0 : z + 1;
+        if (z + 1 < z1) {
+            const int znn = (zn + 1 == N) ? 0 : zn + 1;
+            const size_t pn = (size_t)zn * NN;
+            nn = O::ld(phi + (size_t)znn * NN + rc);
+            pd_n = O::ld(phidot + pn + rc);
+            up_n = O::ld(phi + pn + rp);
+            dn_n = O::ld(phi + pn + rm);
+            if (edge_l) el_n = __ldg(phi + pn + rl);
+            if (edge_r) er_n = __ldg(phi + pn + rr);
+        }
+        // ---- arithmetic of plane z
+        T left = __shfl_up_sync(0xffffffffu, O::last(cur), 1);
+        T right = __shfl_down_sync(0xffffffffu, O::first(cur), 1);
+        if (edge_l) left = el;
+        if (edge_r) right = er;
+        V pnew, vnew;
+        vector_update<T, 3, LITERAL>(k, cur, left, right, dn, up, prev, nxt, pd, pnew, vnew);
+        if (live) {
+            const size_t o = (size_t)z * NN + rc;
+            O::st(phidot_next + o, vnew);
+            O::st(phi_next + o, pnew);
+        }
+        prev = cur; cur = nxt; nxt = nn;
+        up = up_n; dn = dn_n; pd = pd_n; el = el_n; er = er_n;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// 2D: block = BX lanes in x; grid = (x tiles, y chunks of YC rows).  The march axis is y, so the
+// register window supplies both y neighbours and nothing but the two edge scalars is re-read.
+// ------------------------------------------------------------------------------------------------
+template <typename T, bool LITERAL>
+__global__ void __launch_bounds__(128)
+step2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
+                    T* __restrict__ phidot_next, int N, int YC, StepCoef<T> k) {
+    using O = VecOps<T>;
+    using V = typename O::V;
+    constexpr int W = O::W;
+    const int lane = threadIdx.x & 31;
+    const long long xraw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * W;
+    if (xraw - (long long)lane * W >= N) return;          // whole warp beyond the row
+    const bool live = xraw < N;
+    const int x = live ? (int)xraw : N - W;
+    const int y0 = blockIdx.y * YC;
+    const int y1 = min(y0 + YC, N);
+    const bool edge_l = (lane == 0), edge_r = (lane == 31) || (x + W >= N);
+    const int xl = (x == 0) ? N - 1 : x - 1, xr = (x + W >= N) ? 0 : x + W;
+
+    const int yprev = (y0 == 0) ? N - 1 : y0 - 1;
+    const int ynext0 = (y0 + 1 == N) ? 0 : y0 + 1;
+    V prev = O::ld(phi + (size_t)yprev * N + x);
+    V cur = O::ld(phi + (size_t)y0 * N + x);
+    V nxt = O::ld(phi + (size_t)ynext0 * N + x);
+    V pd = O::ld(phidot + (size_t)y0 * N + x);
+    T el = T(0), er = T(0);
+    if (edge_l) el = __ldg(phi + (size_t)y0 * N + xl);
+    if (edge_r) er = __ldg(phi + (size_t)y0 * N + xr);
+    const V zero = {};
+
+    for (int y = y0; y < y1; ++y) {
+        V nn = nxt, pd_n = pd;
+        T el_n = el, er_n = er;
+        const int yn = (y + 1 == N) ? 0 : y + 1;
+        if (y + 1 < y1) {
+            const int ynn = (yn + 1 == N) ? 0 : yn + 1;
+            nn = O::ld(phi + (size_t)ynn * N + x);
+            pd_n = O::ld(phidot + (size_t)yn * N + x);
+            if (edge_l) el_n = __ldg(phi + (size_t)yn * N + xl);
+            if (edge_r) er_n = __ldg(phi + (size_t)yn * N + xr);
+        }
+        T left = __shfl_up_sync(0xffffffffu, O::last(cur), 1);
+        T right = __shfl_down_sync(0xffffffffu, O::first(cur), 1);
+        if (edge_l) left = el;
+        if (edge_r) right = er;
+        V pnew, vnew;
+        vector_update<T, 2, LITERAL>(k, cur, left, right, prev, nxt, zero, zero, pd, pnew, vnew);
+        if (live) {
+            const size_t o = (size_t)y * N + x;
+            O::st(phidot_next + o, vnew);
+            O::st(phi_next + o, pnew);
+        }
+        prev = cur; cur = nxt; nxt = nn;
+        pd = pd_n; el = el_n; er = er_n;
+    }
+}
+
+}  // namespace prs

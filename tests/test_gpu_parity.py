@@ -1,0 +1,290 @@
+"""GPU parity: libprs (through its C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): link count bit-exact on any snapshot; fields after 20 steps within
+1e-12 (FP64) / 2e-5 (FP32) of the oracle as the paper prints the update (LITERAL arithmetic).  On top
+of that, with the same arithmetic form on both sides (COEF or LITERAL) the fields must be IDENTICAL
+bit for bit, because neither side ever fuses a multiply with an add.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import paper_1710_10420_b200 as prs  # noqa: E402
+from oracle import binding as ref  # noqa: E402
+from paper_1710_10420_b200 import prs as binding  # noqa: E402
+from tests import fieldgen as fg  # noqa: E402
+
+NP = {prs.F32: np.float32, prs.F64: np.float64}
+TOL = {prs.F32: 2e-5, prs.F64: 1e-12}
+THREADS = max(1, min(16, os.cpu_count() or 1))
+KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED]
+
+
+def make_pair(dims, N, prec, arith_gpu=prs.ARITH_COEF, arith_ref=ref.ARITH_LITERAL, kernel=prs.KERNEL_AUTO, **kw):
+    g = prs.Simulation(dims, N, prec, **kw)
+    g.set_arith(arith_gpu)
+    g.set_step_kernel(kernel)
+    r = ref.RefSim(dims, N, prec, arith=arith_ref, threads=THREADS, **kw)
+    return g, r
+
+
+def maxdiff(a, b):
+    return float(np.max(np.abs(a.astype(np.float64) - b.astype(np.float64))))
+
+
+# ------------------------------------------------------------------ T1: initial condition
+
+@pytest.mark.parametrize("dims,N", [(2, 1), (2, 5), (2, 256), (2, 1000), (3, 3), (3, 64), (3, 101)])
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("seed", [0, 1, (1 << 32) + 7])
+def test_init_is_byte_identical(dims, N, prec, seed):
+    g, r = make_pair(dims, N, prec, seed=seed, phi0=1.0 if seed != 1 else 1.75)
+    g.init(1.0)
+    r.init(1.0)
+    gp, gv = g.copy_out()
+    rp, rv = r.copy_out()
+    assert gp.tobytes() == rp.tobytes() and gv.tobytes() == rv.tobytes()
+    assert not np.any(np.signbit(gv))
+
+
+# ------------------------------------------------------------------ T2: 20 steps from the seeded state
+
+CASES_2D = [4, 36, 132, 256, 520]
+CASES_3D = [4, 20, 36, 64, 132]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, n) for n in CASES_2D] + [(3, n) for n in CASES_3D])
+@pytest.mark.parametrize("era_m", [1.0, 2.0])
+def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
+    # (a) tolerance bar against the paper's literal form, GPU in its default COEF form
+    g, r = make_pair(dims, N, prec, kernel=kernel, era_m=era_m, seed=3)
+    g.init(1.0)
+    r.init(1.0)
+    g.step(20)
+    r.step(20)
+    gp, gv = g.copy_out()
+    rp, rv = r.copy_out()
+    assert maxdiff(gp, rp) <= TOL[prec] and maxdiff(gv, rv) <= TOL[prec]
+    assert g.get_info(binding.INFO_STEP_KERNEL) == kernel
+    # (b) same arithmetic form on both sides -> identical bits
+    for ag, ar in ((prs.ARITH_COEF, ref.ARITH_COEF), (prs.ARITH_LITERAL, ref.ARITH_LITERAL)):
+        g2, r2 = make_pair(dims, N, prec, arith_gpu=ag, arith_ref=ar, kernel=kernel, era_m=era_m, seed=3)
+        g2.init(1.0)
+        r2.init(1.0)
+        g2.step(20)
+        r2.step(20)
+        a, b = g2.copy_out(), r2.copy_out()
+        assert a[0].tobytes() == b[0].tobytes() and a[1].tobytes() == b[1].tobytes()
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 7), (2, 130), (3, 5), (3, 33)])
+def test_sizes_only_the_generic_kernel_takes(prec, dims, N):
+    g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_COEF, seed=9)
+    g.init(1.0)
+    r.init(1.0)
+    g.step(20)
+    r.step(20)
+    a, b = g.copy_out(), r.copy_out()
+    assert a[0].tobytes() == b[0].tobytes() and a[1].tobytes() == b[1].tobytes()
+    W = 4 if prec == prs.F32 else 2
+    if N % W:
+        assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_GENERIC
+        with pytest.raises(prs.PrsError):
+            g.set_step_kernel(prs.KERNEL_TILED)
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 260), (3, 68)])
+@pytest.mark.parametrize("chunk,tile_y", [(1, 4), (3, 8), (7, 16), (1000, 8)])
+def test_tiling_parameters_do_not_change_a_bit(prec, dims, N, chunk, tile_y):
+    phi, pd = fg.random_state(dims, N, 77, NP[prec])
+    outs = []
+    for kernel, ch, ty in ((prs.KERNEL_GENERIC, 0, 8), (prs.KERNEL_TILED, chunk, tile_y)):
+        g = prs.Simulation(dims, N, prec)
+        g.set_step_kernel(kernel)
+        g.set_option(binding.OPT_CHUNK, ch)
+        g.set_option(binding.OPT_TILE_Y, ty)
+        g.copy_in(phi, pd, eta0=2.0, step=5)
+        g.step(6)
+        outs.append(g.copy_out())
+    assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
+
+
+# ------------------------------------------------------------------ T3: diagnostics on snapshots
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 1), (2, 2), (2, 5), (2, 256), (2, 1000), (3, 2), (3, 7), (3, 64), (3, 100)])
+def test_diagnostics_match_on_snapshots(prec, dims, N):
+    g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_COEF, seed=4)
+    g.init(1.0)
+    r.init(1.0)
+    for nsteps in (0, 20, 60):
+        g.step(nsteps)
+        r.step(nsteps)
+        dg, dr = g.diagnostics(), r.diagnostics()
+        gp, gv = g.copy_out()
+        dsnap = ref.diagnostics_of(gp, gv)                       # oracle on the GPU's exact bytes
+        for d in (dr, dsnap):
+            assert dg["link_count"] == d["link_count"] and dg["wall_sites"] == d["wall_sites"]
+            assert abs(dg["sum_ratio"] - d["sum_ratio"]) <= 1e-10 * max(d["sum_ratio"], 1e-300)
+            assert abs(dg["gv2"] - d["gv2"]) <= 1e-10 * max(d["gv2"], 1e-300)
+        assert dg["step"] == dr["step"] and dg["eta"] == dr["eta"] and dg["rho"] == dr["rho"]
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+def test_diagnostics_of_special_fields(prec):
+    dt = NP[prec]
+    N = 64
+    g = prs.Simulation(3, N, prec)
+    # vacuum: nothing
+    g.copy_in(np.full((N,) * 3, -1.0, dt), np.zeros((N,) * 3, dt))
+    d = g.diagnostics()
+    assert d["link_count"] == 0 and d["wall_sites"] == 0 and d["gv2"] == 0.0
+    # planar kink pair: exact area
+    phi = fg.kink_pair(3, N, np.pi / 10.0, dtype=dt)
+    g.copy_in(phi, np.zeros_like(phi))
+    d = g.diagnostics()
+    assert d["link_count"] == 2 * N * N and d["wall_sites"] == 4 * N * N and d["rho"] == 2.0 / N
+    # signed zeros: +0 positive, -0 negative
+    z = np.ones((N,) * 3, dt)
+    z[3, 4, 5] = -0.0
+    g.copy_in(z, np.ones_like(z))
+    d = g.diagnostics()
+    assert d["link_count"] == 6 and d["wall_sites"] == 7
+    dr = ref.diagnostics_of(z, np.ones_like(z))
+    assert abs(d["sum_ratio"] - dr["sum_ratio"]) <= 1e-12 * dr["sum_ratio"]
+
+
+# ------------------------------------------------------------------ symmetries on the GPU (P2-P5 re-run)
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 136), (3, 36)])
+def test_gpu_symmetries_are_bit_exact(kernel, prec, dims, N):
+    dt = NP[prec]
+    phi, pd = fg.random_state(dims, N, 13, dt)
+
+    def run(p, v):
+        g = prs.Simulation(dims, N, prec, era_m=2.0)
+        g.set_step_kernel(kernel)
+        g.copy_in(p, v, eta0=1.0, step=0)
+        g.step(5)
+        return g.copy_out()
+
+    p0, v0 = run(phi, pd)
+    p1, v1 = run(-phi, -pd)
+    assert np.array_equal(p0, -p1) and np.array_equal(v0, -v1)
+    sh = (5, 3, 1)[:dims]
+    p2, v2 = run(fg.roll_state(phi, sh), fg.roll_state(pd, sh))
+    assert np.array_equal(fg.roll_state(p0, sh), p2) and np.array_equal(fg.roll_state(v0, sh), v2)
+    for ax in range(dims):
+        p3, v3 = run(fg.flip_axis(phi, ax), fg.flip_axis(pd, ax))
+        assert np.array_equal(fg.flip_axis(p0, ax), p3) and np.array_equal(fg.flip_axis(v0, ax), v3)
+    vac = np.full((N,) * dims, 1.0, dt)
+    pv, vv = run(vac, np.zeros_like(vac))
+    assert np.array_equal(pv, vac) and np.all(vv == 0)
+
+
+# ------------------------------------------------------------------ T4: restart parity at late times
+
+@pytest.mark.parametrize("dims,N,prec,adv", [(2, 512, prs.F32, 600), (3, 96, prs.F32, 200), (3, 64, prs.F64, 150)])
+def test_restart_parity(dims, N, prec, adv):
+    g = prs.Simulation(dims, N, prec, seed=5)
+    g.init(1.0)
+    g.step(adv)
+    gp, gv = g.copy_out()
+    r = ref.RefSim(dims, N, prec, arith=ref.ARITH_COEF, threads=THREADS)
+    r.copy_in(gp, gv, eta0=1.0, step=adv)
+    g.step(20)
+    r.step(20)
+    a, b = g.copy_out(), r.copy_out()
+    assert a[0].tobytes() == b[0].tobytes() and a[1].tobytes() == b[1].tobytes()
+    dg, dr = g.diagnostics(), r.diagnostics()
+    assert dg["link_count"] == dr["link_count"] and dg["wall_sites"] == dr["wall_sites"]
+    assert dg["eta"] == dr["eta"]
+    # and within tolerance of the literal form
+    r2 = ref.RefSim(dims, N, prec, arith=ref.ARITH_LITERAL, threads=THREADS)
+    r2.copy_in(gp, gv, eta0=1.0, step=adv)
+    r2.step(20)
+    c = r2.copy_out()
+    assert maxdiff(a[0], c[0]) <= TOL[prec] and maxdiff(a[1], c[1]) <= TOL[prec]
+
+
+# ------------------------------------------------------------------ T5: long-run curve, config 0 (256^2)
+
+def fit_mu(etas, rhos, eta_fit):
+    sel = (etas >= eta_fit) & (rhos > 0)
+    return float(np.polyfit(np.log(etas[sel]), np.log(rhos[sel]), 1)[0])
+
+
+def test_config0_256sq_full_run_curve():
+    # BASELINE.json configs[0]: 2D 256^2 FP32, radiation era, eta 1 -> 128, link count every 10 steps;
+    # the FP64 oracle is run as well.
+    N, nsamp = 256, 127
+    g = prs.Simulation(2, N, prs.F32, seed=1)
+    r32 = ref.RefSim(2, N, ref.F32, seed=1, threads=THREADS)           # literal, FP32
+    r64 = ref.RefSim(2, N, ref.F64, seed=1, threads=THREADS)           # literal, FP64
+    for s in (g, r32, r64):
+        s.init(1.0)
+    eta, cg, c32, c64 = [], [], [], []
+    for _ in range(nsamp):
+        for s in (g, r32, r64):
+            s.step(10)
+        dg, d32, d64 = g.diagnostics(), r32.diagnostics(), r64.diagnostics()
+        eta.append(dg["eta"]); cg.append(dg["rho"]); c32.append(d32["rho"]); c64.append(d64["rho"])
+        assert dg["eta"] == d32["eta"]
+    eta, cg, c32, c64 = map(np.array, (eta, cg, c32, c64))
+    assert np.max(np.abs(cg - c32) / c32) <= 0.02
+    assert np.max(np.abs(cg - c64) / c64) <= 0.02
+    mu_g, mu_32, mu_64 = (fit_mu(eta, c, 13.2) for c in (cg, c32, c64))
+    assert abs(mu_g - mu_32) <= 0.02 and abs(mu_g - mu_64) <= 0.02
+
+
+# ------------------------------------------------------------------ state handling
+
+def test_copy_in_out_roundtrip_device_and_host_and_step_split():
+    import torch
+    N = 128
+    phi, pd = fg.random_state(2, N, 3, np.float32)
+    g = prs.Simulation(2, N, prs.F32)
+    tp, tv = torch.from_numpy(phi).cuda(), torch.from_numpy(pd).cuda()
+    g.copy_in(tp, tv, eta0=1.5, step=2)                    # device pointers
+    op, ov = torch.empty_like(tp), torch.empty_like(tv)
+    g.copy_out_to(op, ov)
+    assert torch.equal(op, tp) and torch.equal(ov, tv)
+    g.step(3); g.step(0); g.step(4)
+    a = g.copy_out()
+    g2 = prs.Simulation(2, N, prs.F32)
+    g2.copy_in(phi, pd, eta0=1.5, step=2)                  # host pointers
+    g2.step(7)
+    b = g2.copy_out()
+    assert a[0].tobytes() == b[0].tobytes() and a[1].tobytes() == b[1].tobytes()
+    assert g.get_info(binding.INFO_STEP) == 9 and g.diagnostics()["eta"] == 1.5 + 9 * 0.1
+    # device_pointers view equals copy_out
+    pp, pv = g.device_pointers()
+    assert pp and pv and pp != pv
+    assert g.kernel_launches >= 7
+
+
+def test_error_paths_on_device():
+    g = prs.Simulation(2, 16, prs.F32)
+    with pytest.raises(prs.PrsError) as e:
+        g.step(1)
+    assert e.value.code == 4
+    with pytest.raises(prs.PrsError):
+        g.diagnostics()
+    with pytest.raises(prs.PrsError):
+        g.init(-1.0)
+    g.init(1.0)
+    with pytest.raises(prs.PrsError):
+        g.step(-1)
+    with pytest.raises(prs.PrsError):
+        g.set_option(99, 0)
+    with pytest.raises(prs.PrsError):
+        g.set_option(binding.OPT_TILE_Y, 5)
