@@ -60,7 +60,8 @@ enum {
     PRS_OPT_ARITH       = 2,   /* PRS_ARITH_*                                    default COEF     */
     PRS_OPT_DIAG_KERNEL = 3,   /* PRS_KERNEL_AUTO / GENERIC / TILED              default AUTO     */
     PRS_OPT_CHUNK       = 4,   /* tuning: planes (3D) / rows (2D) one CTA marches; 0 = auto        */
-    PRS_OPT_TILE_Y      = 5    /* tuning: rows per CTA of the 3D tiled kernels, 4 / 8 / 16         */
+    PRS_OPT_TILE_Y      = 5,   /* tuning: rows per CTA of the 3D tiled kernel, 4 / 8 / 16          */
+    PRS_OPT_TB2_TILE_Y  = 6    /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 */
 };
 enum {
     PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */

@@ -14,6 +14,7 @@
 #include "prs_arith.cuh"
 #include "prs_kernels_generic.cuh"
 #include "prs_kernels_tiled.cuh"
+#include "prs_kernels_tb2.cuh"
 
 using namespace prs;
 
@@ -71,7 +72,7 @@ struct prs_ctx {
     double eta0;
     int64_t step;
     bool inited;
-    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y;
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;
@@ -184,6 +185,70 @@ cudaError_t launch_tiled2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     return cudaGetLastError();
 }
 
+template <typename T, bool LITERAL, int TY>
+cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
+                             const StepCoef<T>& k2) {
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    const size_t smem = tb2_smem_bytes<T, TY>();
+    static bool configured = false;            // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(step3d_tb2_kernel<T, LITERAL, TY>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const unsigned gx = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT), gy = (unsigned)((N + TY - 1) / TY);
+    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
+    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const dim3 block(32, TY + 4, 1);
+    step3d_tb2_kernel<T, LITERAL, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, k1, k2);
+    return cudaGetLastError();
+}
+
+template <typename T, bool LITERAL>
+cudaError_t launch_tb2_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
+                          const StepCoef<T>& k2) {
+    switch (h->opt_tb2_tile_y) {
+        case 4: return launch_tb2_3d_ty<T, LITERAL, 4>(h, p, v, pn, vn, k1, k2);
+        case 8: return launch_tb2_3d_ty<T, LITERAL, 8>(h, p, v, pn, vn, k1, k2);
+        default: return launch_tb2_3d_ty<T, LITERAL, 12>(h, p, v, pn, vn, k1, k2);
+    }
+}
+
+template <typename T, bool LITERAL>
+cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
+                          const StepCoef<T>& k2) {
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    const int BX = 128, warps = BX / 32;
+    const unsigned nwarps = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT);
+    const unsigned gx = (nwarps + warps - 1) / warps;
+    int YC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
+    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
+    step2d_tb2_kernel<T, LITERAL><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k1, k2);
+    return cudaGetLastError();
+}
+
+// Two steps in one pass (n -> n+2); the caller guarantees the lattice is supported.
+template <typename T>
+int step_twice(prs_ctx* h) {
+    const StepCoef<T> k1 = coef_at<T>(h, h->step), k2 = coef_at<T>(h, h->step + 1);
+    const T* p = (const T*)h->phi[h->cur];
+    const T* v = (const T*)h->pd[h->cur];
+    T* pn = (T*)h->phi[h->cur ^ 1];
+    T* vn = (T*)h->pd[h->cur ^ 1];
+    const bool lit = (h->opt_arith == PRS_ARITH_LITERAL);
+    cudaError_t e;
+    if (h->dims == 3) e = lit ? launch_tb2_3d<T, true>(h, p, v, pn, vn, k1, k2) : launch_tb2_3d<T, false>(h, p, v, pn, vn, k1, k2);
+    else e = lit ? launch_tb2_2d<T, true>(h, p, v, pn, vn, k1, k2) : launch_tb2_2d<T, false>(h, p, v, pn, vn, k1, k2);
+    if (e != cudaSuccess) return cuda_fail(h, e, "two-step kernel launch");
+    h->launches += 1;
+    h->cur ^= 1;
+    h->step += 2;
+    return PRS_OK;
+}
+
 template <typename T>
 int step_once(prs_ctx* h, int kernel) {
     const StepCoef<T> k = coef_at<T>(h, h->step);
@@ -269,7 +334,7 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     h->d_result = (DiagPartial*)(h->ws + L.off_result);
     h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
     h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_COEF; h->opt_diag_kernel = PRS_KERNEL_AUTO;
-    h->opt_chunk = 0; h->opt_tile_y = 4;
+    h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     h->h_result = nullptr;
     int dev = attr.device;
@@ -313,8 +378,16 @@ int prs_step(prs_handle h, int64_t nsteps) {
     if (nsteps < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_step: nsteps must be >= 0");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
     const int kernel = resolve_step_kernel(h);
-    for (int64_t i = 0; i < nsteps; ++i) {
-        const int rc = (h->precision == PRS_F32) ? step_once<float>(h, kernel) : step_once<double>(h, kernel);
+    int64_t left = nsteps;
+    if (kernel == PRS_KERNEL_TB2) {
+        for (; left >= 2; left -= 2) {
+            const int rc = (h->precision == PRS_F32) ? step_twice<float>(h) : step_twice<double>(h);
+            if (rc != PRS_OK) return rc;
+        }
+    }
+    const int single = (kernel == PRS_KERNEL_TB2) ? PRS_KERNEL_TILED : kernel;   // odd remainder
+    for (; left > 0; --left) {
+        const int rc = (h->precision == PRS_F32) ? step_once<float>(h, single) : step_once<double>(h, single);
         if (rc != PRS_OK) return rc;
     }
     if (nsteps > 0) h->last_step_kernel = kernel;
@@ -375,12 +448,11 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
     switch (option) {
         case PRS_OPT_STEP_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
-            if (value == PRS_KERNEL_TILED) {
-                if (!tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled step kernel needs N to be a multiple of 16 bytes of T");
+            if (value == PRS_KERNEL_TILED || value == PRS_KERNEL_TB2) {
+                if (!tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled / two-step kernels need N to be a multiple of 16 bytes of T");
                 h->opt_step_kernel = (int)value;
                 return PRS_OK;
             }
-            if (value == PRS_KERNEL_TB2) return fail(h, PRS_ERR_UNSUPPORTED, "temporally blocked kernel is not available for this lattice");
             return fail(h, PRS_ERR_INVALID_ARG, "unknown step kernel");
         case PRS_OPT_ARITH:
             if (value != PRS_ARITH_LITERAL && value != PRS_ARITH_COEF) return fail(h, PRS_ERR_INVALID_ARG, "unknown arithmetic");
@@ -396,6 +468,10 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
         case PRS_OPT_TILE_Y:
             if (value != 4 && value != 8 && value != 16) return fail(h, PRS_ERR_INVALID_ARG, "tile_y must be 4, 8 or 16");
             h->opt_tile_y = (int)value;
+            return PRS_OK;
+        case PRS_OPT_TB2_TILE_Y:
+            if (value != 4 && value != 8 && value != 12) return fail(h, PRS_ERR_INVALID_ARG, "tb2_tile_y must be 4, 8 or 12");
+            h->opt_tb2_tile_y = (int)value;
             return PRS_OK;
         default:
             return fail(h, PRS_ERR_INVALID_ARG, "unknown option");

@@ -195,3 +195,178 @@ step2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
 }
 
 }  // namespace prs
+
+namespace prs {
+
+// ------------------------------------------------------------------------------------------------
+// Diagnostics (Eq. 7 link count, Eq. 8 wall velocity) with the same marching layout: one
+// read of phi, phidot fetched only for vectors that contain a wall site (a few per cent of the
+// lattice once the network has formed), the 16-byte phidot load of plane z issued as soon as its
+// wall mask is known and consumed one iteration later.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ unsigned sign_mask(typename VecOps<T>::V v) {
+    using O = VecOps<T>;
+    unsigned m = 0;
+#pragma unroll
+    for (int i = 0; i < O::W; ++i) m |= (Ar<T>::neg(O::get(v, i)) ? 1u : 0u) << i;
+    return m;
+}
+
+// Link / wall bookkeeping of one vector from sign masks.  c: this vector; l / r: sign of the scalar
+// to the left / right (0 or 1); ym, yp, zm, zp: masks of the neighbouring vectors (zm = zp = c in 2D).
+template <int W, int DIMS>
+__device__ __forceinline__ void mask_links(unsigned c, unsigned l, unsigned r, unsigned ym, unsigned yp,
+                                           unsigned zm, unsigned zp, unsigned& nlinks, unsigned& wallmask) {
+    constexpr unsigned ALL = (1u << W) - 1u;
+    const unsigned right_of = ((c >> 1) | (r << (W - 1))) & ALL;   // sign of x+1 for each site
+    const unsigned left_of = ((c << 1) | l) & ALL;                 // sign of x-1 for each site
+    const unsigned fx = c ^ right_of, bx = c ^ left_of;
+    const unsigned fy = c ^ yp, by = c ^ ym;
+    unsigned fz = 0, bz = 0;
+    if (DIMS == 3) { fz = c ^ zp; bz = c ^ zm; }
+    nlinks = __popc(fx) + __popc(fy) + __popc(fz);                 // forward links owned by these sites
+    wallmask = (fx | bx | fy | by | fz | bz) & ALL;
+}
+
+template <typename T>
+__device__ __forceinline__ void accumulate_walls(unsigned wallmask, typename VecOps<T>::V c, typename VecOps<T>::V pd,
+                                                 double V0, double I, DiagPartial& acc) {
+    using O = VecOps<T>;
+#pragma unroll
+    for (int i = 0; i < O::W; ++i)
+        if (wallmask & (1u << i)) {
+            acc.walls += 1;
+            acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(O::get(c, i), O::get(pd, i), V0, I));
+        }
+}
+
+template <typename T, int TYB>
+__global__ void __launch_bounds__(32 * TYB)
+diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int N, int ZC, double V0, double I,
+                    DiagPartial* __restrict__ partials) {
+    using O = VecOps<T>;
+    using V = typename O::V;
+    constexpr int W = O::W;
+    DiagPartial acc = {0ull, 0ull, 0.0};
+    const int lane = threadIdx.x;
+    const int y = blockIdx.y * TYB + threadIdx.y;
+    const int xraw = (blockIdx.x * 32 + lane) * W;
+    if (y < N) {                                           // warp-uniform
+        const bool live = xraw < N;
+        const int x = live ? xraw : N - W;
+        const int z0 = blockIdx.z * ZC;
+        const int z1 = min(z0 + ZC, N);
+        const size_t NN = (size_t)N * N;
+        const int ym = (y == 0) ? N - 1 : y - 1, yp = (y == N - 1) ? 0 : y + 1;
+        const size_t rc = (size_t)y * N + x, rm = (size_t)ym * N + x, rp = (size_t)yp * N + x;
+        const bool edge_l = (lane == 0), edge_r = (lane == 31) || (x + W >= N);
+        const size_t rl = (size_t)y * N + (x == 0 ? N - 1 : x - 1);
+        const size_t rr = (size_t)y * N + (x + W >= N ? 0 : x + W);
+        const int zprev = (z0 == 0) ? N - 1 : z0 - 1;
+        unsigned m_prev = sign_mask<T>(O::ld(phi + (size_t)zprev * NN + rc));
+        V cur = O::ld(phi + (size_t)z0 * NN + rc);
+        V nxt = O::ld(phi + (size_t)((z0 + 1 == N) ? 0 : z0 + 1) * NN + rc);
+        unsigned m_up = sign_mask<T>(O::ld(phi + (size_t)z0 * NN + rp));
+        unsigned m_dn = sign_mask<T>(O::ld(phi + (size_t)z0 * NN + rm));
+        unsigned s_l = 0, s_r = 0;
+        if (edge_l) s_l = Ar<T>::neg(__ldg(phi + (size_t)z0 * NN + rl));
+        if (edge_r) s_r = Ar<T>::neg(__ldg(phi + (size_t)z0 * NN + rr));
+        // deferred wall work of the previous plane
+        unsigned d_mask = 0;
+        V d_c = cur, d_pd = cur;
+        for (int z = z0; z < z1; ++z) {
+            V nn = nxt;
+            unsigned m_up_n = m_up, m_dn_n = m_dn, s_l_n = s_l, s_r_n = s_r;
+            const int zn = (z + 1 == N) ? 0 : z + 1;
+            if (z + 1 < z1) {
+                const int znn = (zn + 1 == N) ? 0 : zn + 1;
+                const size_t pn = (size_t)zn * NN;
+                nn = O::ld(phi + (size_t)znn * NN + rc);
+                m_up_n = sign_mask<T>(O::ld(phi + pn + rp));
+                m_dn_n = sign_mask<T>(O::ld(phi + pn + rm));
+                if (edge_l) s_l_n = Ar<T>::neg(__ldg(phi + pn + rl));
+                if (edge_r) s_r_n = Ar<T>::neg(__ldg(phi + pn + rr));
+            }
+            const unsigned m_cur = sign_mask<T>(cur), m_nxt = sign_mask<T>(nxt);
+            unsigned l = __shfl_up_sync(0xffffffffu, (m_cur >> (W - 1)) & 1u, 1);
+            unsigned r = __shfl_down_sync(0xffffffffu, m_cur & 1u, 1);
+            if (edge_l) l = s_l;
+            if (edge_r) r = s_r;
+            unsigned nlinks, wallmask;
+            mask_links<W, 3>(m_cur, l, r, m_dn, m_up, m_prev, m_nxt, nlinks, wallmask);
+            if (!live) { nlinks = 0; wallmask = 0; }
+            acc.links += nlinks;
+            V pd_now = cur;
+            if (wallmask) pd_now = O::ld(phidot + (size_t)z * NN + rc);   // consumed next iteration
+            if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+            d_mask = wallmask; d_c = cur; d_pd = pd_now;
+            m_prev = m_cur; cur = nxt; nxt = nn;
+            m_up = m_up_n; m_dn = m_dn_n; s_l = s_l_n; s_r = s_r_n;
+        }
+        if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+    }
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0 && threadIdx.y == 0)
+        partials[blockIdx.x + gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z)] = acc;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128)
+diag2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int N, int YC, double V0, double I,
+                    DiagPartial* __restrict__ partials) {
+    using O = VecOps<T>;
+    using V = typename O::V;
+    constexpr int W = O::W;
+    DiagPartial acc = {0ull, 0ull, 0.0};
+    const int lane = threadIdx.x & 31;
+    const long long xraw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * W;
+    if (xraw - (long long)lane * W < N) {                  // warp-uniform
+        const bool live = xraw < N;
+        const int x = live ? (int)xraw : N - W;
+        const int y0 = blockIdx.y * YC;
+        const int y1 = min(y0 + YC, N);
+        const bool edge_l = (lane == 0), edge_r = (lane == 31) || (x + W >= N);
+        const int xl = (x == 0) ? N - 1 : x - 1, xr = (x + W >= N) ? 0 : x + W;
+        const int yprev = (y0 == 0) ? N - 1 : y0 - 1;
+        unsigned m_prev = sign_mask<T>(O::ld(phi + (size_t)yprev * N + x));
+        V cur = O::ld(phi + (size_t)y0 * N + x);
+        V nxt = O::ld(phi + (size_t)((y0 + 1 == N) ? 0 : y0 + 1) * N + x);
+        unsigned s_l = 0, s_r = 0;
+        if (edge_l) s_l = Ar<T>::neg(__ldg(phi + (size_t)y0 * N + xl));
+        if (edge_r) s_r = Ar<T>::neg(__ldg(phi + (size_t)y0 * N + xr));
+        unsigned d_mask = 0;
+        V d_c = cur, d_pd = cur;
+        for (int y = y0; y < y1; ++y) {
+            V nn = nxt;
+            unsigned s_l_n = s_l, s_r_n = s_r;
+            const int yn = (y + 1 == N) ? 0 : y + 1;
+            if (y + 1 < y1) {
+                const int ynn = (yn + 1 == N) ? 0 : yn + 1;
+                nn = O::ld(phi + (size_t)ynn * N + x);
+                if (edge_l) s_l_n = Ar<T>::neg(__ldg(phi + (size_t)yn * N + xl));
+                if (edge_r) s_r_n = Ar<T>::neg(__ldg(phi + (size_t)yn * N + xr));
+            }
+            const unsigned m_cur = sign_mask<T>(cur), m_nxt = sign_mask<T>(nxt);
+            unsigned l = __shfl_up_sync(0xffffffffu, (m_cur >> (W - 1)) & 1u, 1);
+            unsigned r = __shfl_down_sync(0xffffffffu, m_cur & 1u, 1);
+            if (edge_l) l = s_l;
+            if (edge_r) r = s_r;
+            unsigned nlinks, wallmask;
+            mask_links<W, 2>(m_cur, l, r, m_prev, m_nxt, m_cur, m_cur, nlinks, wallmask);
+            if (!live) { nlinks = 0; wallmask = 0; }
+            acc.links += nlinks;
+            V pd_now = cur;
+            if (wallmask) pd_now = O::ld(phidot + (size_t)y * N + x);
+            if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+            d_mask = wallmask; d_c = cur; d_pd = pd_now;
+            m_prev = m_cur; cur = nxt; nxt = nn;
+            s_l = s_l_n; s_r = s_r_n;
+        }
+        if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+    }
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x + (size_t)gridDim.x * blockIdx.y] = acc;
+}
+
+}  // namespace prs

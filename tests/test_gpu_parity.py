@@ -20,7 +20,7 @@ from tests import fieldgen as fg  # noqa: E402
 NP = {prs.F32: np.float32, prs.F64: np.float64}
 TOL = {prs.F32: 2e-5, prs.F64: 1e-12}
 THREADS = max(1, min(16, os.cpu_count() or 1))
-KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED]
+KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED, prs.KERNEL_TB2]
 
 
 def make_pair(dims, N, prec, arith_gpu=prs.ARITH_COEF, arith_ref=ref.ARITH_LITERAL, kernel=prs.KERNEL_AUTO, **kw):
@@ -71,6 +71,7 @@ def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
     rp, rv = r.copy_out()
     assert maxdiff(gp, rp) <= TOL[prec] and maxdiff(gv, rv) <= TOL[prec]
     assert g.get_info(binding.INFO_STEP_KERNEL) == kernel
+    assert g.get_info(binding.INFO_STEP) == 20
     # (b) same arithmetic form on both sides -> identical bits
     for ag, ar in ((prs.ARITH_COEF, ref.ARITH_COEF), (prs.ARITH_LITERAL, ref.ARITH_LITERAL)):
         g2, r2 = make_pair(dims, N, prec, arith_gpu=ag, arith_ref=ar, kernel=kernel, era_m=era_m, seed=3)
@@ -101,18 +102,41 @@ def test_sizes_only_the_generic_kernel_takes(prec, dims, N):
 
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("dims,N", [(2, 260), (3, 68)])
-@pytest.mark.parametrize("chunk,tile_y", [(1, 4), (3, 8), (7, 16), (1000, 8)])
-def test_tiling_parameters_do_not_change_a_bit(prec, dims, N, chunk, tile_y):
+@pytest.mark.parametrize("chunk,tile_y,tb2_tile_y", [(1, 4, 4), (3, 8, 8), (7, 16, 12), (1000, 8, 12)])
+def test_tiling_parameters_do_not_change_a_bit(prec, dims, N, chunk, tile_y, tb2_tile_y):
     phi, pd = fg.random_state(dims, N, 77, NP[prec])
     outs = []
-    for kernel, ch, ty in ((prs.KERNEL_GENERIC, 0, 8), (prs.KERNEL_TILED, chunk, tile_y)):
+    for kernel, ch in ((prs.KERNEL_GENERIC, 0), (prs.KERNEL_TILED, chunk), (prs.KERNEL_TB2, chunk)):
         g = prs.Simulation(dims, N, prec)
         g.set_step_kernel(kernel)
         g.set_option(binding.OPT_CHUNK, ch)
-        g.set_option(binding.OPT_TILE_Y, ty)
+        g.set_option(binding.OPT_TILE_Y, tile_y)
+        g.set_option(binding.OPT_TB2_TILE_Y, tb2_tile_y)
         g.copy_in(phi, pd, eta0=2.0, step=5)
         g.step(6)
         outs.append(g.copy_out())
+    for o in outs[1:]:
+        assert outs[0][0].tobytes() == o[0].tobytes() and outs[0][1].tobytes() == o[1].tobytes()
+
+
+# ------------------------------------------------------------------ T6: temporal blocking == single steps
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 4), (2, 8), (2, 120), (2, 124), (2, 1024), (3, 4), (3, 8), (3, 60), (3, 124), (3, 200)])
+@pytest.mark.parametrize("nsteps", [1, 2, 7])
+def test_two_step_kernel_equals_single_steps_bitwise(prec, dims, N, nsteps):
+    phi, pd = fg.random_state(dims, N, 5, NP[prec])
+    outs = []
+    for kernel in (prs.KERNEL_TILED, prs.KERNEL_TB2):
+        g = prs.Simulation(dims, N, prec, era_m=2.0)
+        g.set_step_kernel(kernel)
+        g.copy_in(phi, pd, eta0=1.0, step=3)
+        g.step(nsteps)
+        outs.append(g.copy_out())
+        assert g.get_info(binding.INFO_STEP) == 3 + nsteps
+        # launches: two steps per launch, plus one single step for an odd remainder
+        want = nsteps if kernel == prs.KERNEL_TILED else nsteps // 2 + nsteps % 2
+        assert g.kernel_launches == want
     assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
 
 
