@@ -55,7 +55,12 @@ BYTES_PER_SITE_UPDATE = {0: 16, 1: 32}        # read phi, phidot; write phidot, 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed
 # `ncu --set full` capture of the headline config (profiles/): filled in once measured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {
+    # profiles/r01a_ncu_step3d_tb2_f32_1024.md: 9.186 GB read + 8.551 GB written per two-step launch
+    ("3d_1024_f32_rad", "tb2"): 17_737_048_000,
+    # profiles/r01a_ncu_step3d_tiled_f32_1024.md: 8.867 GB read + 8.549 GB written per single-step launch
+    ("3d_1024_f32_rad", "tiled"): 17_415_889_000,
+}
 
 
 def measured_peak_gbs():
@@ -246,6 +251,7 @@ def run_gpu(args):
     launch_ms = ms_kernels / (step_kernel_launches / steps_per_launch)
     achieved = S * steps_per_launch * bpu / (launch_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak_gbs()
+    kernel_name = {1: "generic", 2: "tiled", 3: "tb2"}.get(step_kernel, str(step_kernel))
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
     e2e = None
@@ -305,9 +311,9 @@ def run_gpu(args):
                        "W0": 10.0, "substeps_per_step": SUBSTEPS, "diagnostics_per_step": 1,
                        "parallelism": "replicas x%d (no sharding, no collective)" % world,
                        "l2": "state (%.1f GiB) exceeds L2; no flush needed" % (4 * fbytes / 2 ** 30),
-                       "step_kernel": {1: "generic", 2: "tiled", 3: "tb2"}.get(step_kernel, str(step_kernel))},
+                       "step_kernel": kernel_name},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
+                         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((args.config, kernel_name)),
                          "kernel": "step kernel", "launch_ms": launch_ms, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": S * steps_per_launch * bpu,
                          "step_kernel_share_of_step": ms_kernels / ms_total},

@@ -21,7 +21,7 @@ using namespace prs;
 namespace {
 
 constexpr size_t ALIGN = 256;
-constexpr int MAX_PARTIALS = 4096;           // upper bound on diagnostics blocks
+constexpr int MAX_PARTIALS = 1 << 16;        // upper bound on diagnostics blocks (1.5 MiB of scratch)
 
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
@@ -127,7 +127,13 @@ bool tiled_supported(const prs_ctx* h) {
 
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
-    if (want == PRS_KERNEL_AUTO) want = tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
+    if (want == PRS_KERNEL_AUTO) {
+        // Measured on B200 (profiles/): the two-step kernel wins once the lattice fills the chip
+        // (4096^2, 512^3 and up); below that a launch is latency-bound and the shorter single-step
+        // march is quicker.
+        if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
+        else want = (h->S >= ((size_t)1 << 22)) ? PRS_KERNEL_TB2 : PRS_KERNEL_TILED;
+    }
     return want;
 }
 
@@ -272,6 +278,31 @@ int step_once(prs_ctx* h, int kernel) {
     return PRS_OK;
 }
 
+bool diag_tiled_supported(const prs_ctx* h) {
+    if (!tiled_supported(h)) return false;
+    const int W = vec_width(h->precision);
+    const long long gx = (h->N + 32LL * W - 1) / (32LL * W);
+    const long long tiles = (h->dims == 3) ? gx * ((h->N + 3) / 4) : (h->N + 128LL * W - 1) / (128LL * W);
+    return tiles <= MAX_PARTIALS;
+}
+
+int resolve_diag_kernel(const prs_ctx* h) {
+    int want = h->opt_diag_kernel;
+    if (want == PRS_KERNEL_AUTO) want = diag_tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
+    return want;
+}
+
+// Chunk length of the diagnostics march: as short as the partials scratch allows, but no shorter
+// than 16 (the first plane / row of a chunk costs three loads instead of one).
+int diag_chunk(const prs_ctx* h, long long tiles_per_slab) {
+    long long max_chunks = MAX_PARTIALS / tiles_per_slab;
+    if (max_chunks < 1) max_chunks = 1;
+    long long len = (h->N + max_chunks - 1) / max_chunks;
+    if (len < 16) len = 16;
+    if (len > h->N) len = h->N;
+    return (int)len;
+}
+
 template <typename T>
 int diag_launch(prs_ctx* h) {
     const double pi = 3.14159265358979323846;
@@ -279,20 +310,41 @@ int diag_launch(prs_ctx* h) {
     const double I = 1.0 / (h->phi0 * h->phi0);
     const T* p = (const T*)h->phi[h->cur];
     const T* v = (const T*)h->pd[h->cur];
-    long long blocks = (long long)((h->S + 255) / 256);
-    const long long cap = std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 8);
-    if (blocks > cap) blocks = cap;
-    if (h->dims == 3)
-        diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
-    else
-        diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+    const int kernel = resolve_diag_kernel(h);
+    long long blocks;
+    if (kernel == PRS_KERNEL_TILED) {
+        constexpr int W = VecOps<T>::W;
+        const int N = (int)h->N;
+        if (h->dims == 3) {
+            constexpr int TY = 4;
+            const unsigned gx = (unsigned)((N + 32 * W - 1) / (32 * W)), gy = (unsigned)((N + TY - 1) / TY);
+            const int ZC = diag_chunk(h, (long long)gx * gy);
+            const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+            blocks = (long long)grid.x * grid.y * grid.z;
+            diag3d_tiled_kernel<T, TY><<<grid, dim3(32, TY, 1), 0, h->stream>>>(p, v, N, ZC, V0, I, h->partials);
+        } else {
+            const unsigned gx = (unsigned)((N + 128 * W - 1) / (128 * W));
+            const int YC = diag_chunk(h, gx);
+            const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
+            blocks = (long long)grid.x * grid.y;
+            diag2d_tiled_kernel<T><<<grid, 128, 0, h->stream>>>(p, v, N, YC, V0, I, h->partials);
+        }
+    } else {
+        blocks = (long long)((h->S + 255) / 256);
+        const long long cap = std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 8);
+        if (blocks > cap) blocks = cap;
+        if (h->dims == 3)
+            diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+        else
+            diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics kernel launch");
     diag_finalize_kernel<<<1, 1024, 0, h->stream>>>(h->partials, (int)blocks, h->d_result);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics finalize launch");
     h->launches += 2;
-    h->last_diag_kernel = PRS_KERNEL_GENERIC;
+    h->last_diag_kernel = kernel;
     return PRS_OK;
 }
 
@@ -460,7 +512,12 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             return PRS_OK;
         case PRS_OPT_DIAG_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_diag_kernel = (int)value; return PRS_OK; }
-            return fail(h, PRS_ERR_UNSUPPORTED, "only the generic diagnostics kernel exists");
+            if (value == PRS_KERNEL_TILED) {
+                if (!diag_tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled diagnostics kernel cannot take this lattice");
+                h->opt_diag_kernel = (int)value;
+                return PRS_OK;
+            }
+            return fail(h, PRS_ERR_INVALID_ARG, "unknown diagnostics kernel");
         case PRS_OPT_CHUNK:
             if (value < 0 || value > (1 << 20)) return fail(h, PRS_ERR_INVALID_ARG, "chunk must be >= 0");
             h->opt_chunk = (int)value;

@@ -142,10 +142,18 @@ def test_two_step_kernel_equals_single_steps_bitwise(prec, dims, N, nsteps):
 
 # ------------------------------------------------------------------ T3: diagnostics on snapshots
 
+@pytest.mark.parametrize("diag_kernel", [prs.KERNEL_GENERIC, prs.KERNEL_TILED])
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
-@pytest.mark.parametrize("dims,N", [(2, 1), (2, 2), (2, 5), (2, 256), (2, 1000), (3, 2), (3, 7), (3, 64), (3, 100)])
-def test_diagnostics_match_on_snapshots(prec, dims, N):
+@pytest.mark.parametrize("dims,N", [(2, 1), (2, 2), (2, 4), (2, 5), (2, 256), (2, 520), (2, 1000), (3, 2), (3, 4), (3, 7),
+                                    (3, 64), (3, 100), (3, 132)])
+def test_diagnostics_match_on_snapshots(diag_kernel, prec, dims, N):
     g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_COEF, seed=4)
+    W = 4 if prec == prs.F32 else 2
+    if diag_kernel == prs.KERNEL_TILED and N % W:
+        with pytest.raises(prs.PrsError):
+            g.set_option(binding.OPT_DIAG_KERNEL, diag_kernel)
+        return
+    g.set_option(binding.OPT_DIAG_KERNEL, diag_kernel)
     g.init(1.0)
     r.init(1.0)
     for nsteps in (0, 20, 60):
@@ -159,6 +167,7 @@ def test_diagnostics_match_on_snapshots(prec, dims, N):
             assert abs(dg["sum_ratio"] - d["sum_ratio"]) <= 1e-10 * max(d["sum_ratio"], 1e-300)
             assert abs(dg["gv2"] - d["gv2"]) <= 1e-10 * max(d["gv2"], 1e-300)
         assert dg["step"] == dr["step"] and dg["eta"] == dr["eta"] and dg["rho"] == dr["rho"]
+        assert g.get_info(binding.INFO_DIAG_KERNEL) == diag_kernel
 
 
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
