@@ -3,27 +3,35 @@
 // site-update halves to 8 B (FP32) / 16 B (FP64); the per-site arithmetic is the same sequence of
 // individually rounded operations as two single steps, so the result is bit-identical to them.
 //
+// With half the HBM traffic the kernel is bound by instruction issue, not by memory, so the design
+// goal is instructions per site-update: packed FP32 arithmetic (prs_pack.cuh: FADD2 / FMUL2 round two
+// sites per instruction), each thread's own column kept in a register window (only neighbour rows go
+// through shared memory), no integer division and no 64-bit address arithmetic inside the march.
+//
 // 3D scheme.  A CTA owns TY rows x 30 vectors of x (120 floats / 60 doubles) of output and marches a
 // chunk of z planes.  It is 32 lanes wide and TY+4 warps tall: lane 0 / lane 31 and the two outer
-// rows on each side are halo.  Per iteration j it
-//   (0) has every thread issue one 16-byte cp.async for its own column of the phi^n plane two
-//       ahead and of the phidot^{n-1/2} plane one ahead, straight into shared-memory rings (no
-//       register staging, PF planes of prefetch);
-//   (1) stage 1: rows 1..TY+2 compute phi^{n+1}, phidot^{n+1/2} on plane zi = z0-1+j from the
-//       phi^n ring (z+-1 from the ring, y+-1 from the neighbouring rows of the ring, x+-1 by warp
-//       shuffle) and publish phi^{n+1} to a two-slot shared plane;
-//   (2) stage 2: rows 2..TY+1 compute phi^{n+2}, phidot^{n+3/2} on plane zi-1 from their own register
-//       window of phi^{n+1} (three planes deep), the neighbouring rows of the published plane and
-//       shuffles, and store lanes 1..30 to HBM.
-// Values at the halo rim that lack a neighbour are computed from finite stand-ins and never used.
-// Periodic wrap is plain index arithmetic on the cp.async source addresses.
+// rows on each side are halo.  Plane index a = 0, 1, ... stands for z = z0-2+a (periodic).  In
+// iteration j every thread
+//   (0) waits for its cp.async group j (phi^n plane a = j+2, phidot^{n-1/2} plane z0-1+j), then the
+//       CTA barrier makes every thread's group j visible and retires all reads of iteration j-1;
+//   (1) issues one 16-byte cp.async for its own column of phi^n plane a = j+2+PF and of the phidot
+//       plane PF ahead, straight into shared-memory rings (no register staging);
+//   (2) stage 1 (rows 1..TY+2): phi^{n+1}, phidot^{n+1/2} on plane a = j+1 from its register window
+//       (z-1, z), its own column of the ring (z+1), the neighbouring rows of the ring (y+-1) and warp
+//       shuffles (x+-1); publishes phi^{n+1} to a two-slot shared plane;
+//   (3) stage 2 (rows 2..TY+1, j >= 2): phi^{n+2}, phidot^{n+3/2} on plane a = j from its register
+//       window of phi^{n+1} (three planes deep), the neighbouring rows of the plane published one
+//       iteration ago and shuffles; lanes 1..30 store to HBM.
+// Values at the halo rim that lack a neighbour are computed from stand-ins and never used.
 //
 // 2D scheme.  Same idea with the march along y and no shared memory at all: both register windows
 // supply the y neighbours and shuffles supply the x neighbours; a warp outputs 30 vectors of x.
 #pragma once
 
+#include <type_traits>
+
 #include "prs_arith.cuh"
-#include "prs_kernels_tiled.cuh"
+#include "prs_pack.cuh"
 
 namespace prs {
 
@@ -42,8 +50,8 @@ __host__ __device__ __forceinline__ int wrap_mod(int i, int n) {
 
 constexpr int TB2_XOUT = 30;       // output vectors per warp row (lanes 1..30)
 constexpr int TB2_PF = 2;          // planes of prefetch
-constexpr int TB2_RA = 3 + TB2_PF; // phi^n ring slots
-constexpr int TB2_RP = 1 + TB2_PF; // phidot^{n-1/2} ring slots
+constexpr int TB2_RA = 4;          // phi^n ring slots: planes a = j+1, j+2 being read, PF in flight
+constexpr int TB2_RP = 4;          // phidot^{n-1/2} ring slots: 1 being read, PF in flight (power of two)
 
 template <typename T, int TY>
 constexpr size_t tb2_smem_bytes() {
@@ -51,19 +59,22 @@ constexpr size_t tb2_smem_bytes() {
 }
 
 template <typename T, bool LITERAL, int TY>
-__global__ void __launch_bounds__(32 * (TY + 4))
+__global__ void __launch_bounds__(32 * (TY + 4), 2)
 step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int ZC, StepCoef<T> k1, StepCoef<T> k2) {
-    using O = VecOps<T>;
-    using V = typename O::V;
-    constexpr int W = O::W;
+    using K = Pk<T>;
+    using V = typename K::V;
+    constexpr int W = K::W;
     constexpr int ROWS = TY + 4;
+    constexpr int PLANE = ROWS * 32;                                 // vectors per shared plane
+    static_assert(TB2_RA == 4 && TB2_RP == 4 && TB2_PF == 2, "the slot arithmetic below assumes these");
     extern __shared__ __align__(16) unsigned char tb2_smem[];
-    V* const ringA = reinterpret_cast<V*>(tb2_smem);                 // [RA][ROWS][32]
-    V* const ringP = ringA + TB2_RA * ROWS * 32;                     // [RP][ROWS][32]
-    V* const planeB = ringP + TB2_RP * ROWS * 32;                    // [2][ROWS][32]
-
     const int lane = threadIdx.x, row = threadIdx.y;
+    const int me = row * 32 + lane;
+    V* const sA = reinterpret_cast<V*>(tb2_smem) + me;               // ring A [4][PLANE], this thread's slot
+    V* const sP = sA + TB2_RA * PLANE;                               // ring P [4][PLANE]
+    V* const sB = sP + TB2_RP * PLANE;                               // plane B [2][PLANE]
+
     const int NQ = N / W;
     const int qraw = TB2_XOUT * (int)blockIdx.x - 1 + lane;
     const int q = wrap_mod(qraw, NQ);
@@ -77,71 +88,89 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const bool stage1_row = (row >= 1) && (row <= TY + 2);
     const bool stage2_row = (row >= 2) && (row <= TY + 1);
     const bool store_ok = stage2_row && (yraw < N) && (lane >= 1) && (lane <= TB2_XOUT) && (qraw < NQ);
-    const int me = row * 32 + lane;
 
-    // ---- prologue: planes a = 0, 1 (z0-2, z0-1), then plane a = 2 with phidot plane p = 0, then PF-1 more
-    cp_async16(&ringA[(0 * ROWS) * 32 + me], phi + (size_t)wrap_mod(z0 - 2, N) * NN + col);
-    cp_async16(&ringA[(1 * ROWS) * 32 + me], phi + (size_t)wrap_mod(z0 - 1, N) * NN + col);
+    PackCoef<T> c1, c2;
+    c1.template set<3>(k1);
+    c2.template set<3>(k2);
+
+    // One load cursor serves both fields: issue i fetches phi^n plane a = i (z = z0-2+i, periodic)
+    // and the phidot plane of the same z, which stage 1 needs one iteration later than phi^n.
+    const ptrdiff_t d_in = phidot - phi, d_out = phidot_out - phi_out;
+    int zl = wrap_mod(z0 - 2, N);
+    const T* la = phi + (size_t)zl * NN + col;
+    const size_t wrap_back = (size_t)N * NN;
+    int ni = 0;                                                      // issues so far
+    auto issue = [&](int slot_a, int slot_p) {
+        if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, la);
+        if (stage1_row && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, la + d_in);
+        ++ni; la += NN;
+        if (++zl == N) { zl = 0; la -= wrap_back; }
+    };
+
+    // ---- prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
+    issue(0, 3); issue(1, 0); issue(2, 1);
     cp_async_commit();
-#pragma unroll
-    for (int g = 0; g < TB2_PF; ++g) {          // group g carries A plane 2+g and P plane g
-        if (g < niter) {
-            cp_async16(&ringA[(((2 + g) % TB2_RA) * ROWS) * 32 + me], phi + (size_t)wrap_mod(z0 + g, N) * NN + col);
-            if (stage1_row)
-                cp_async16(&ringP[((g % TB2_RP) * ROWS) * 32 + me], phidot + (size_t)wrap_mod(z0 - 1 + g, N) * NN + col);
-        }
-        cp_async_commit();
-    }
+    issue(3, 2);
+    cp_async_commit();
 
-    V b_prev = {}, b_cur = {}, q_cur = {};
-    for (int j = 0; j < niter; ++j) {
-        // (0) prefetch group j+PF: A plane j+2+PF (z = z0+j+PF), P plane j+PF (z = z0-1+j+PF)
-        if (j + TB2_PF < niter) {
-            cp_async16(&ringA[(((j + 2 + TB2_PF) % TB2_RA) * ROWS) * 32 + me],
-                       phi + (size_t)wrap_mod(z0 + j + TB2_PF, N) * NN + col);
-            if (stage1_row)
-                cp_async16(&ringP[(((j + TB2_PF) % TB2_RP) * ROWS) * 32 + me],
-                           phidot + (size_t)wrap_mod(z0 - 1 + j + TB2_PF, N) * NN + col);
-        }
-        cp_async_commit();
-        cp_async_wait<TB2_PF>();                // group j (A plane j+2, P plane j) has landed for this thread
-        __syncthreads();                        // ... and for every thread; also fences last iteration's reads
+    // Register window of the thread's own column: phi^n at planes a = j, j+1.  Plane 0 is needed for
+    // nothing else, so it is read here, before its ring slot is reused (a thread's own cp.async data
+    // is visible to it after wait_group; no barrier needed).
+    cp_async_wait<TB2_PF - 1>();
+    V a_zm = sA[0 * PLANE], a_c = sA[1 * PLANE];
+    V b_prev = {}, b_cur = {}, q_cur = {};      // phi^{n+1} at planes a = j-1, j; phidot^{n+1/2} at plane j
+    T* po = phi_out + (size_t)z0 * NN + col;    // store cursor (plane a = j, first used at j = 2)
 
-        // (1) stage 1 on plane zi = z0-1+j
+    // One iteration; U = j mod 4 is a compile-time constant so that every ring slot is an immediate.
+    auto iteration = [&](auto u_tag, int j) {
+        constexpr int U = decltype(u_tag)::value;
+        cp_async_wait<TB2_PF - 1>();            // group j has landed for this thread
+        __syncthreads();                        // ... and for every thread; retires iteration j-1's reads
+        issue(U, (U + 3) & 3);                  // issue j+4: phi^n plane j+4 takes the slot of plane j
+        cp_async_commit();
+
+        // stage 1 on plane a = j+1
         V b_new = {}, q_new = {};
         if (stage1_row) {
-            const V* A0 = ringA + ((j % TB2_RA) * ROWS) * 32;
-            const V* A1 = ringA + (((j + 1) % TB2_RA) * ROWS) * 32;
-            const V* A2 = ringA + (((j + 2) % TB2_RA) * ROWS) * 32;
-            const V c = A1[me];
-            const V zm = A0[me], zp = A2[me];
-            const V ym = A1[me - 32], yp = A1[me + 32];
-            const V pd = ringP[((j % TB2_RP) * ROWS) * 32 + me];
-            const T left = __shfl_up_sync(0xffffffffu, O::last(c), 1);
-            const T right = __shfl_down_sync(0xffffffffu, O::first(c), 1);
-            vector_update<T, 3, LITERAL>(k1, c, left, right, ym, yp, zm, zp, pd, b_new, q_new);
-            planeB[((j & 1) * ROWS) * 32 + me] = b_new;
+            const V zp = sA[((U + 2) & 3) * PLANE];
+            const V ym = sA[((U + 1) & 3) * PLANE - 32], yp = sA[((U + 1) & 3) * PLANE + 32];
+            const V pd = sP[U * PLANE];
+            const T left = __shfl_up_sync(0xffffffffu, K::last(a_c), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(a_c), 1);
+            packed_vector_update<T, 3, LITERAL>(c1, a_c, left, right, ym, yp, a_zm, zp, pd, b_new, q_new);
+            sB[(U & 1) * PLANE] = b_new;
+            a_zm = a_c; a_c = zp;
         }
-        // No barrier here: stage 2 below reads the plane published one iteration ago (slot (j-1)&1),
-        // which the barrier at the top of this iteration already ordered; the slot written above is
-        // read only after the next top-of-iteration barrier.
+        // No barrier here: stage 2 reads the plane published one iteration ago (slot (j-1)&1), which
+        // the barrier at the top of this iteration already ordered; the slot written above is read
+        // only after the next top-of-iteration barrier.
 
-        // (2) stage 2 on plane zo = zi-1 = z0+j-2
+        // stage 2 on plane a = j  (z = z0+j-2)
         if (j >= 2 && stage2_row) {
-            const V* B = planeB + (((j - 1) & 1) * ROWS) * 32;
-            const V ym = B[me - 32], yp = B[me + 32];
-            const T left = __shfl_up_sync(0xffffffffu, O::last(b_cur), 1);
-            const T right = __shfl_down_sync(0xffffffffu, O::first(b_cur), 1);
+            const V ym = sB[((U + 1) & 1) * PLANE - 32], yp = sB[((U + 1) & 1) * PLANE + 32];
+            const T left = __shfl_up_sync(0xffffffffu, K::last(b_cur), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(b_cur), 1);
             V pout, vout;
-            vector_update<T, 3, LITERAL>(k2, b_cur, left, right, ym, yp, b_prev, b_new, q_cur, pout, vout);
+            packed_vector_update<T, 3, LITERAL>(c2, b_cur, left, right, ym, yp, b_prev, b_new, q_cur, pout, vout);
             if (store_ok) {
-                const size_t o = (size_t)(z0 + j - 2) * NN + col;
-                O::st(phidot_out + o, vout);
-                O::st(phi_out + o, pout);
+                K::stg(po + d_out, vout);
+                K::stg(po, pout);
             }
+            po += NN;
         }
         b_prev = b_cur; b_cur = b_new; q_cur = q_new;
+    };
+
+    for (int j = 0; j < niter; j += 4) {
+        iteration(std::integral_constant<int, 0>{}, j);
+        if (j + 1 >= niter) break;
+        iteration(std::integral_constant<int, 1>{}, j + 1);
+        if (j + 2 >= niter) break;
+        iteration(std::integral_constant<int, 2>{}, j + 2);
+        if (j + 3 >= niter) break;
+        iteration(std::integral_constant<int, 3>{}, j + 3);
     }
+    cp_async_wait<0>();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -151,9 +180,9 @@ template <typename T, bool LITERAL>
 __global__ void __launch_bounds__(128)
 step2d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int YC, StepCoef<T> k1, StepCoef<T> k2) {
-    using O = VecOps<T>;
-    using V = typename O::V;
-    constexpr int W = O::W;
+    using K = Pk<T>;
+    using V = typename K::V;
+    constexpr int W = K::W;
     const int lane = threadIdx.x & 31;
     const int warp_global = (int)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int NQ = N / W;
@@ -167,41 +196,60 @@ step2d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const bool store_ok = (lane >= 1) && (lane <= TB2_XOUT) && (qraw < NQ);
     const V zero = {};
 
+    PackCoef<T> c1, c2;
+    c1.template set<2>(k1);
+    c2.template set<2>(k2);
+
+    // load cursors (periodic rows): la = phi row two ahead of stage 1, lp = phidot row one ahead
+    int yla = wrap_mod(y0 - 2, N), ylp = wrap_mod(y0 - 1, N);
+    const T* la = phi + (size_t)yla * N + colx;
+    const T* lp = phidot + (size_t)ylp * N + colx;
+    const size_t wrap_back = (size_t)N * N;
+#define TB2_NEXT_A(dst)                                         \
+    do {                                                        \
+        dst = K::ldg(la); la += N;                              \
+        if (++yla == N) { yla = 0; la -= wrap_back; }           \
+    } while (0)
+#define TB2_NEXT_P(dst)                                         \
+    do {                                                        \
+        dst = K::ldg(lp); lp += N;                              \
+        if (++ylp == N) { ylp = 0; lp -= wrap_back; }           \
+    } while (0)
+
     // register windows: a* = phi^n rows, b* = phi^{n+1} rows
-    V a_prev = O::ld(phi + (size_t)wrap_mod(y0 - 2, N) * N + colx);
-    V a_cur = O::ld(phi + (size_t)wrap_mod(y0 - 1, N) * N + colx);
-    V a_next = O::ld(phi + (size_t)wrap_mod(y0, N) * N + colx);
-    V pd = O::ld(phidot + (size_t)wrap_mod(y0 - 1, N) * N + colx);
+    V a_prev, a_cur, a_next, pd;
+    TB2_NEXT_A(a_prev); TB2_NEXT_A(a_cur); TB2_NEXT_A(a_next); TB2_NEXT_P(pd);
     V b_prev = zero, b_cur = zero, q_cur = zero;
+    T* po = phi_out + (size_t)y0 * N + colx;
+    T* vo = phidot_out + (size_t)y0 * N + colx;
     for (int j = 0; j < niter; ++j) {
-        // loads of the next iteration first: phi^n row y0+j+1, phidot row y0+j
-        V a_nn = a_next, pd_n = pd;
-        if (j + 1 < niter) {
-            a_nn = O::ld(phi + (size_t)wrap_mod(y0 + j + 1, N) * N + colx);
-            pd_n = O::ld(phidot + (size_t)wrap_mod(y0 + j, N) * N + colx);
-        }
+        // loads of the next iteration first: phi^n row y0+j+1, phidot row y0+j (unused past the end)
+        V a_nn, pd_n;
+        TB2_NEXT_A(a_nn); TB2_NEXT_P(pd_n);
         // stage 1 on row yi = y0-1+j
         V b_new, q_new;
         {
-            const T left = __shfl_up_sync(0xffffffffu, O::last(a_cur), 1);
-            const T right = __shfl_down_sync(0xffffffffu, O::first(a_cur), 1);
-            vector_update<T, 2, LITERAL>(k1, a_cur, left, right, a_prev, a_next, zero, zero, pd, b_new, q_new);
+            const T left = __shfl_up_sync(0xffffffffu, K::last(a_cur), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(a_cur), 1);
+            packed_vector_update<T, 2, LITERAL>(c1, a_cur, left, right, a_prev, a_next, zero, zero, pd, b_new, q_new);
         }
         // stage 2 on row yo = y0+j-2
         if (j >= 2) {
-            const T left = __shfl_up_sync(0xffffffffu, O::last(b_cur), 1);
-            const T right = __shfl_down_sync(0xffffffffu, O::first(b_cur), 1);
+            const T left = __shfl_up_sync(0xffffffffu, K::last(b_cur), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(b_cur), 1);
             V pout, vout;
-            vector_update<T, 2, LITERAL>(k2, b_cur, left, right, b_prev, b_new, zero, zero, q_cur, pout, vout);
+            packed_vector_update<T, 2, LITERAL>(c2, b_cur, left, right, b_prev, b_new, zero, zero, q_cur, pout, vout);
             if (store_ok) {
-                const size_t o = (size_t)(y0 + j - 2) * N + colx;
-                O::st(phidot_out + o, vout);
-                O::st(phi_out + o, pout);
+                K::stg(vo, vout);
+                K::stg(po, pout);
             }
+            po += N; vo += N;
         }
         a_prev = a_cur; a_cur = a_next; a_next = a_nn; pd = pd_n;
         b_prev = b_cur; b_cur = b_new; q_cur = q_new;
     }
+#undef TB2_NEXT_A
+#undef TB2_NEXT_P
 }
 
 }  // namespace prs

@@ -73,3 +73,33 @@ def test_product_never_imports_the_oracle():
                 for ln in text.splitlines():
                     if "import" in ln or "#include" in ln or "dlopen" in ln or "CDLL" in ln:
                         assert "oracle" not in ln.lower(), (f, ln)
+
+
+def test_no_fused_multiply_add_in_the_step_kernels():
+    """Bit-for-bit parity with the oracle rests on every multiply and add being rounded on its own.
+    ptxas contracts packed mul.rn.f32x2 + add.rn.f32x2 into FFMA2 whatever --fmad says (prs_pack.cuh
+    works around it), so look at the machine code: no FFMA / FFMA2 / DFMA in any step kernel of the
+    default (COEF, template argument LITERAL = false) arithmetic.  The LITERAL kernels legitimately
+    contain FMAs inside the correctly rounded division routine."""
+    import re
+    import shutil
+    import subprocess
+
+    from paper_1710_10420_b200 import build as prs_build
+
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", prs_build.build()], stdout=subprocess.PIPE, text=True, check=True).stdout
+    cur, seen, bad = None, set(), []
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            continue
+        if cur and "step" in cur and "Lb0E" in cur:
+            seen.add(cur)
+            if re.search(r"\b(FFMA2?|DFMA)\b", line):
+                bad.append((cur, line.strip()))
+    assert len(seen) >= 12, "expected the generic, tiled and two-step kernels in the library"
+    assert not bad, bad[:5]
