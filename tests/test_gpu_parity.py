@@ -19,7 +19,7 @@ from tests import fieldgen as fg  # noqa: E402
 
 NP = {prs.F32: np.float32, prs.F64: np.float64}
 TOL = {prs.F32: 2e-5, prs.F64: 1e-12}
-THREADS = max(1, min(16, os.cpu_count() or 1))
+THREADS = max(1, min(32, len(os.sched_getaffinity(0))))
 KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED, prs.KERNEL_TB2]
 
 
@@ -321,3 +321,55 @@ def test_error_paths_on_device():
         g.set_option(99, 0)
     with pytest.raises(prs.PrsError):
         g.set_option(binding.OPT_TILE_Y, 5)
+
+
+# ------------------------------------------------------------------ full sizes of BASELINE.json, bench.py's launch configuration
+
+def chunked_maxdiff(a, b, chunk=1 << 26):
+    fa, fb = a.reshape(-1), b.reshape(-1)
+    m = 0.0
+    for i in range(0, fa.size, chunk):
+        m = max(m, float(np.max(np.abs(fa[i:i + chunk].astype(np.float64) - fb[i:i + chunk].astype(np.float64)))))
+    return m
+
+
+FULL_SIZE_CASES = [
+    # dims, N, precision, era_m      (configs[1] .. configs[4] of BASELINE.json; both eras and both
+    #                                 precisions appear at the headline size)
+    (2, 4096, prs.F32, 1.0), (2, 4096, prs.F32, 2.0),
+    (2, 16384, prs.F32, 1.0), (2, 16384, prs.F64, 1.0),
+    (3, 512, prs.F32, 1.0),
+    (3, 1024, prs.F32, 1.0), (3, 1024, prs.F64, 2.0),
+]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("dims,N,prec,era_m", FULL_SIZE_CASES)
+def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m):
+    """T2 at full size: default options (the kernel selection and tiling bench.py times), seeded
+    initial state, 20 steps, every site compared with the oracle run on the host cores: identical
+    bits against the oracle in the same arithmetic form, within the north_star tolerance against the
+    paper's literal form (checked on phidot and phi), and the diagnostics of the final state."""
+    g = prs.Simulation(dims, N, prec, era_m=era_m, seed=2)
+    g.init(1.0)
+    g.step(20)
+    assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_TB2
+    dg = g.diagnostics()
+    gp, gv = g.copy_out()
+    g.close()
+    r = ref.RefSim(dims, N, prec, era_m=era_m, seed=2, arith=ref.ARITH_COEF, threads=THREADS)
+    r.init(1.0)
+    r.step(20)
+    dr = r.diagnostics()
+    rp, rv = r.copy_out()
+    r.close()
+    assert np.array_equal(gp, rp) and np.array_equal(gv, rv)
+    assert dg["link_count"] == dr["link_count"] and dg["wall_sites"] == dr["wall_sites"]
+    assert abs(dg["sum_ratio"] - dr["sum_ratio"]) <= 1e-10 * dr["sum_ratio"]
+    del rp, rv
+    r = ref.RefSim(dims, N, prec, era_m=era_m, seed=2, arith=ref.ARITH_LITERAL, threads=THREADS)
+    r.init(1.0)
+    r.step(20)
+    lp, lv = r.copy_out()
+    r.close()
+    assert chunked_maxdiff(gp, lp) <= TOL[prec] and chunked_maxdiff(gv, lv) <= TOL[prec]
