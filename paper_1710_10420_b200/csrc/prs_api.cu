@@ -125,6 +125,12 @@ bool tiled_supported(const prs_ctx* h) {
     return h->N % W == 0 && h->N >= W && h->N <= (1 << 30);
 }
 
+// The 3D two-step kernel addresses 16-byte vectors with 32-bit indices (cursor overshoot included).
+bool tb2_supported(const prs_ctx* h) {
+    if (!tiled_supported(h)) return false;
+    return h->dims == 2 || h->S / (size_t)vec_width(h->precision) < ((size_t)1 << 30);
+}
+
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
     if (want == PRS_KERNEL_AUTO) {
@@ -132,7 +138,7 @@ int resolve_step_kernel(const prs_ctx* h) {
         // (4096^2, 512^3 and up); below that a launch is latency-bound and the shorter single-step
         // march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        else want = (h->S >= ((size_t)1 << 22)) ? PRS_KERNEL_TB2 : PRS_KERNEL_TILED;
+        else want = (h->S >= ((size_t)1 << 22) && tb2_supported(h)) ? PRS_KERNEL_TB2 : PRS_KERNEL_TILED;
     }
     return want;
 }
@@ -218,6 +224,9 @@ cudaError_t launch_tb2_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, cons
     switch (h->opt_tb2_tile_y) {
         case 4: return launch_tb2_3d_ty<T, LITERAL, 4>(h, p, v, pn, vn, k1, k2);
         case 8: return launch_tb2_3d_ty<T, LITERAL, 8>(h, p, v, pn, vn, k1, k2);
+        case 10: return launch_tb2_3d_ty<T, LITERAL, 10>(h, p, v, pn, vn, k1, k2);
+        case 20: return launch_tb2_3d_ty<T, LITERAL, 20>(h, p, v, pn, vn, k1, k2);
+        case 28: return launch_tb2_3d_ty<T, LITERAL, 28>(h, p, v, pn, vn, k1, k2);
         default: return launch_tb2_3d_ty<T, LITERAL, 12>(h, p, v, pn, vn, k1, k2);
     }
 }
@@ -501,6 +510,7 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
         case PRS_OPT_STEP_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
             if (value == PRS_KERNEL_TILED || value == PRS_KERNEL_TB2) {
+                if (value == PRS_KERNEL_TB2 && !tb2_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the two-step kernel cannot take this lattice");
                 if (!tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled / two-step kernels need N to be a multiple of 16 bytes of T");
                 h->opt_step_kernel = (int)value;
                 return PRS_OK;
@@ -527,7 +537,8 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             h->opt_tile_y = (int)value;
             return PRS_OK;
         case PRS_OPT_TB2_TILE_Y:
-            if (value != 4 && value != 8 && value != 12) return fail(h, PRS_ERR_INVALID_ARG, "tb2_tile_y must be 4, 8 or 12");
+            if (value != 4 && value != 8 && value != 10 && value != 12 && value != 20 && value != 28)
+                return fail(h, PRS_ERR_INVALID_ARG, "tb2_tile_y must be 4, 8, 10, 12, 20 or 28");
             h->opt_tb2_tile_y = (int)value;
             return PRS_OK;
         default:

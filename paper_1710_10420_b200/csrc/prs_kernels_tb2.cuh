@@ -59,7 +59,7 @@ constexpr size_t tb2_smem_bytes() {
 }
 
 template <typename T, bool LITERAL, int TY>
-__global__ void __launch_bounds__(32 * (TY + 4), 2)
+__global__ void __launch_bounds__(32 * (TY + 4), (32 * (TY + 4) > 512) ? 1 : 2)
 step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int ZC, StepCoef<T> k1, StepCoef<T> k2) {
     using K = Pk<T>;
@@ -82,95 +82,111 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const int y = wrap_mod(yraw, N);
     const int z0 = (int)blockIdx.z * ZC;
     const int zend = min(z0 + ZC, N);
-    const int niter = (zend - z0) + 2;
-    const size_t NN = (size_t)N * N;
-    const size_t col = (size_t)y * N + (size_t)q * W;              // offset of this thread's column in a plane
-    const bool stage1_row = (row >= 1) && (row <= TY + 2);
-    const bool stage2_row = (row >= 2) && (row <= TY + 1);
-    const bool store_ok = stage2_row && (yraw < N) && (lane >= 1) && (lane <= TB2_XOUT) && (qraw < NQ);
+    const int niter = (zend - z0) + 2;                               // >= 3
+    const bool store_ok = (yraw < N) && (lane >= 1) && (lane <= TB2_XOUT) && (qraw < NQ);
 
     PackCoef<T> c1, c2;
     c1.template set<3>(k1);
     c2.template set<3>(k2);
 
+    // All global addresses are 32-bit indices of 16-byte vectors (the host checks N^3 / W < 2^31):
+    // one IMAD.WIDE forms an address, one IADD advances a cursor.
+    const V* const gA = reinterpret_cast<const V*>(phi);
+    const V* const gP = reinterpret_cast<const V*>(phidot);
+    V* const oA = reinterpret_cast<V*>(phi_out);
+    V* const oP = reinterpret_cast<V*>(phidot_out);
+    const int NNv = N * NQ;                                          // vectors per plane
+    const int colv = y * NQ + q;                                     // this thread's column within a plane
     // One load cursor serves both fields: issue i fetches phi^n plane a = i (z = z0-2+i, periodic)
     // and the phidot plane of the same z, which stage 1 needs one iteration later than phi^n.
-    const ptrdiff_t d_in = phidot - phi, d_out = phidot_out - phi_out;
     int zl = wrap_mod(z0 - 2, N);
-    const T* la = phi + (size_t)zl * NN + col;
-    const size_t wrap_back = (size_t)N * NN;
-    int ni = 0;                                                      // issues so far
-    auto issue = [&](int slot_a, int slot_p) {
-        if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, la);
-        if (stage1_row && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, la + d_in);
-        ++ni; la += NN;
-        if (++zl == N) { zl = 0; la -= wrap_back; }
-    };
+    int il = zl * NNv + colv;
+    int left_to_wrap = N - zl;                                       // issues until z wraps to 0
+    int io = z0 * NNv + colv;                                        // store cursor (plane a = j, from j = 2)
 
-    // ---- prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
-    issue(0, 3); issue(1, 0); issue(2, 1);
-    cp_async_commit();
-    issue(3, 2);
-    cp_async_commit();
-
-    // Register window of the thread's own column: phi^n at planes a = j, j+1.  Plane 0 is needed for
-    // nothing else, so it is read here, before its ring slot is reused (a thread's own cp.async data
-    // is visible to it after wait_group; no barrier needed).
-    cp_async_wait<TB2_PF - 1>();
-    V a_zm = sA[0 * PLANE], a_c = sA[1 * PLANE];
-    V b_prev = {}, b_cur = {}, q_cur = {};      // phi^{n+1} at planes a = j-1, j; phidot^{n+1/2} at plane j
-    T* po = phi_out + (size_t)z0 * NN + col;    // store cursor (plane a = j, first used at j = 2)
-
-    // One iteration; U = j mod 4 is a compile-time constant so that every ring slot is an immediate.
-    auto iteration = [&](auto u_tag, int j) {
-        constexpr int U = decltype(u_tag)::value;
-        cp_async_wait<TB2_PF - 1>();            // group j has landed for this thread
-        __syncthreads();                        // ... and for every thread; retires iteration j-1's reads
-        issue(U, (U + 3) & 3);                  // issue j+4: phi^n plane j+4 takes the slot of plane j
+    // The three kinds of row run their own march, so that no per-iteration test of the row survives
+    // and the register windows rotate by renaming in the unrolled code:
+    //   role 0  rows 0, TY+3      load phi^n only (they are the y halo of stage 1)
+    //   role 1  rows 1, TY+2      stage 1 only (they are the y halo of stage 2)
+    //   role 2  rows 2 .. TY+1    stage 1 and stage 2, store
+    auto march = [&](auto role_tag) {
+        constexpr int ROLE = decltype(role_tag)::value;
+        int ni = 0;                                                  // issues so far
+        auto issue = [&](int slot_a, int slot_p) {
+            if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
+            if (ROLE >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
+            ++ni; il += NNv;
+            if (--left_to_wrap == 0) { il -= N * NNv; left_to_wrap = N; }
+        };
+        // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
+        issue(0, 3); issue(1, 0); issue(2, 1);
+        cp_async_commit();
+        issue(3, 2);
         cp_async_commit();
 
-        // stage 1 on plane a = j+1
-        V b_new = {}, q_new = {};
-        if (stage1_row) {
+        // Register window of the thread's own column: phi^n at planes a = j, j+1.  Plane 0 is needed
+        // for nothing else, so it is read here, before its ring slot is reused (a thread's own
+        // cp.async data is visible to it after wait_group; no barrier needed).
+        cp_async_wait<TB2_PF - 1>();
+        V a_zm = sA[0 * PLANE], a_c = sA[1 * PLANE];
+        V b_prev = {}, b_cur = {}, q_cur = {};  // phi^{n+1} at planes a = j-1, j; phidot^{n+1/2} at plane j
+
+        // One iteration; U = j mod 4 is a compile-time constant so that every ring slot is an immediate.
+        auto iteration = [&](auto u_tag, auto s2_tag) {
+            constexpr int U = decltype(u_tag)::value;
+            constexpr bool STAGE2 = decltype(s2_tag)::value && ROLE == 2;
+            cp_async_wait<TB2_PF - 1>();        // group j has landed for this thread
+            __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
+            issue(U, (U + 3) & 3);              // issue j+4: phi^n plane j+4 takes the slot of plane j
+            cp_async_commit();
+            if (ROLE == 0) return;
+
+            // stage 1 on plane a = j+1
             const V zp = sA[((U + 2) & 3) * PLANE];
-            const V ym = sA[((U + 1) & 3) * PLANE - 32], yp = sA[((U + 1) & 3) * PLANE + 32];
+            const V ym1 = sA[((U + 1) & 3) * PLANE - 32], yp1 = sA[((U + 1) & 3) * PLANE + 32];
             const V pd = sP[U * PLANE];
-            const T left = __shfl_up_sync(0xffffffffu, K::last(a_c), 1);
-            const T right = __shfl_down_sync(0xffffffffu, K::first(a_c), 1);
-            packed_vector_update<T, 3, LITERAL>(c1, a_c, left, right, ym, yp, a_zm, zp, pd, b_new, q_new);
+            const T left1 = __shfl_up_sync(0xffffffffu, K::last(a_c), 1);
+            const T right1 = __shfl_down_sync(0xffffffffu, K::first(a_c), 1);
+            V b_new, q_new;
+            packed_vector_update<T, 3, LITERAL>(c1, a_c, left1, right1, ym1, yp1, a_zm, zp, pd, b_new, q_new);
             sB[(U & 1) * PLANE] = b_new;
             a_zm = a_c; a_c = zp;
-        }
-        // No barrier here: stage 2 reads the plane published one iteration ago (slot (j-1)&1), which
-        // the barrier at the top of this iteration already ordered; the slot written above is read
-        // only after the next top-of-iteration barrier.
+            // No barrier here: stage 2 reads the plane published one iteration ago (slot (j-1)&1),
+            // which the barrier at the top of this iteration already ordered; the slot written above
+            // is read only after the next top-of-iteration barrier.
 
-        // stage 2 on plane a = j  (z = z0+j-2)
-        if (j >= 2 && stage2_row) {
-            const V ym = sB[((U + 1) & 1) * PLANE - 32], yp = sB[((U + 1) & 1) * PLANE + 32];
-            const T left = __shfl_up_sync(0xffffffffu, K::last(b_cur), 1);
-            const T right = __shfl_down_sync(0xffffffffu, K::first(b_cur), 1);
-            V pout, vout;
-            packed_vector_update<T, 3, LITERAL>(c2, b_cur, left, right, ym, yp, b_prev, b_new, q_cur, pout, vout);
-            if (store_ok) {
-                K::stg(po + d_out, vout);
-                K::stg(po, pout);
+            // stage 2 on plane a = j  (z = z0+j-2)
+            if (STAGE2) {
+                const V ym2 = sB[((U + 1) & 1) * PLANE - 32], yp2 = sB[((U + 1) & 1) * PLANE + 32];
+                const T left2 = __shfl_up_sync(0xffffffffu, K::last(b_cur), 1);
+                const T right2 = __shfl_down_sync(0xffffffffu, K::first(b_cur), 1);
+                V pout, vout;
+                packed_vector_update<T, 3, LITERAL>(c2, b_cur, left2, right2, ym2, yp2, b_prev, b_new, q_cur, pout, vout);
+                if (store_ok) {
+                    oP[io] = vout;
+                    oA[io] = pout;
+                }
+                io += NNv;
             }
-            po += NN;
+            if (ROLE == 2) { b_prev = b_cur; b_cur = b_new; q_cur = q_new; }
+        };
+        using std::integral_constant;
+        iteration(integral_constant<int, 0>{}, integral_constant<bool, false>{});
+        iteration(integral_constant<int, 1>{}, integral_constant<bool, false>{});
+        for (int j = 2; j < niter; j += 4) {
+            iteration(integral_constant<int, 2>{}, integral_constant<bool, true>{});
+            if (j + 1 >= niter) break;
+            iteration(integral_constant<int, 3>{}, integral_constant<bool, true>{});
+            if (j + 2 >= niter) break;
+            iteration(integral_constant<int, 0>{}, integral_constant<bool, true>{});
+            if (j + 3 >= niter) break;
+            iteration(integral_constant<int, 1>{}, integral_constant<bool, true>{});
         }
-        b_prev = b_cur; b_cur = b_new; q_cur = q_new;
+        cp_async_wait<0>();
     };
-
-    for (int j = 0; j < niter; j += 4) {
-        iteration(std::integral_constant<int, 0>{}, j);
-        if (j + 1 >= niter) break;
-        iteration(std::integral_constant<int, 1>{}, j + 1);
-        if (j + 2 >= niter) break;
-        iteration(std::integral_constant<int, 2>{}, j + 2);
-        if (j + 3 >= niter) break;
-        iteration(std::integral_constant<int, 3>{}, j + 3);
-    }
-    cp_async_wait<0>();
+    if (row == 0 || row == ROWS - 1) march(std::integral_constant<int, 0>{});
+    else if (row == 1 || row == ROWS - 2) march(std::integral_constant<int, 1>{});
+    else march(std::integral_constant<int, 2>{});
 }
 
 // ------------------------------------------------------------------------------------------------
