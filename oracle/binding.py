@@ -9,7 +9,7 @@ import numpy as np
 from . import build as _build
 
 F32, F64 = 0, 1
-ARITH_LITERAL, ARITH_COEF = 0, 1
+ARITH_LITERAL, ARITH_COEF, ARITH_FMA = 0, 1, 2
 _DT = {F32: np.float32, F64: np.float64}
 
 

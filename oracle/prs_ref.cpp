@@ -141,6 +141,18 @@ inline void site_update(const StepCoef<T>& k, const T* phi, const T* phidot, int
         const T sz = phi[x + N * y + zp * N * N] + phi[x + N * y + zm * N * N];
         sum = sum + sz;
     }
+    if (k.arith == PRS_REF_ARITH_FMA) {
+        /* Contracted form (R13): the same formulas with every product that feeds a sum
+         * evaluated as one fused multiply-add (a single rounding), which is what an OpenCL / CUDA
+         * compiler emits from Eqs. 3-5 by default.  Coefficients A, B as in the COEF form. */
+        const T lapf = std::fma(-T(2 * k.dims), c, sum);  /* Eq. 3:  sum - 2d c            */
+        const T tf = std::fma(c * c, k.I, T(-1));         /* phi^2/phi0^2 - 1               */
+        const T ff = std::fma((-k.K) * c, tf, lapf);      /* lap - (K c) t = lap - dV/dphi  */
+        const T vf = std::fma(k.A, phidot[s], k.B * ff);  /* Eq. 4                          */
+        *phidot_next = vf;
+        *phi_next = std::fma(k.deta, vf, c);              /* Eq. 5                          */
+        return;
+    }
     const T lap = sum - T(2 * k.dims) * c;               /* Eq. 3 */
     const T q = c * c;
     const T r = q * k.I;
@@ -305,7 +317,7 @@ int prs_ref_destroy(prs_ref_handle h) {
 }
 
 int prs_ref_set_arith(prs_ref_handle h, int arith) {
-    if (!h || (arith != PRS_REF_ARITH_LITERAL && arith != PRS_REF_ARITH_COEF)) return 1;
+    if (!h || (arith != PRS_REF_ARITH_LITERAL && arith != PRS_REF_ARITH_COEF && arith != PRS_REF_ARITH_FMA)) return 1;
     h->arith = arith;
     return 0;
 }
@@ -400,7 +412,7 @@ int prs_ref_step_sites(int dims, int64_t N, int precision, int arith, double alp
     if (!phi || !phidot || !sites || !phi_next_out || !phidot_next_out || nsites < 0 || n < 0 ||
         !(eta0 > 0.0) || !args_ok(dims, N, precision, alpha, era_m, deta, W0, phi0))
         return 1;
-    if (arith != PRS_REF_ARITH_LITERAL && arith != PRS_REF_ARITH_COEF) return 1;
+    if (arith != PRS_REF_ARITH_LITERAL && arith != PRS_REF_ARITH_COEF && arith != PRS_REF_ARITH_FMA) return 1;
     const Scalars sc = scalars_at(alpha, era_m, deta, W0, phi0, eta0, n);
     const int64_t S = (dims == 3) ? N * N * N : N * N;
     for (int64_t i = 0; i < nsites; ++i) {

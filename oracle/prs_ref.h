@@ -29,8 +29,12 @@ enum { PRS_REF_F32 = 0, PRS_REF_F64 = 1 };
 /* Arithmetic of the velocity update (Eq. 4):
  *   LITERAL: phidot' = ((1-delta)*phidot + deta*f) / (1+delta), one division per site;
  *   COEF   : phidot' = A*phidot + B*f with A=(1-delta)/(1+delta), B=deta/(1+delta) formed in
- *            double once per step and rounded to T.  Algebraically identical; differs by rounding. */
-enum { PRS_REF_ARITH_LITERAL = 0, PRS_REF_ARITH_COEF = 1 };
+ *            double once per step and rounded to T.  Algebraically identical; differs by rounding.
+ *   FMA    : COEF with every product that feeds a sum contracted into one fused multiply-add
+ *            (std::fma, one rounding): lap = fma(-2d, c, sum); t = fma(c*c, I, -1);
+ *            f = fma((-K)*c, t, lap); phidot' = fma(A, phidot, B*f); phi' = fma(deta, phidot', c).
+ *            IEEE-754 fixes fma exactly, so a GPU evaluating the same sequence matches bit for bit. */
+enum { PRS_REF_ARITH_LITERAL = 0, PRS_REF_ARITH_COEF = 1, PRS_REF_ARITH_FMA = 2 };
 
 typedef struct {
     int64_t  step;        /* n of the state measured                                  */

@@ -26,7 +26,7 @@ def run(dims, N, prec, phi, pd, nsteps, eta0=1.0, arith=ref.ARITH_LITERAL, threa
 # ------------------------------------------------------------------ P1: hand-computed 4x4 step
 
 @pytest.mark.parametrize("prec,dt", PRECS)
-@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF])
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
 def test_hand_computed_4x4_step(prec, dt, arith):
     g = read_sections("step_4x4.txt")
     phi0, pd0 = as_array(g["phi0"], dt), as_array(g["phidot0"], dt)
@@ -61,13 +61,17 @@ def test_scalars_of_the_hand_example_and_eq6_time_level():
 
 @pytest.mark.parametrize("prec,dt", PRECS)
 @pytest.mark.parametrize("dims,N", [(2, 12), (3, 6)])
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
 @pytest.mark.parametrize("era_m", [0.0, 1.0, 2.0])
-def test_vacua_are_exact_fixed_points(prec, dt, dims, N, era_m):
+def test_vacua_are_exact_fixed_points(prec, dt, dims, N, era_m, arith):
+    # In the contracted form t = fma(phi^2, 1/phi0^2, -1) is the exact residual of the rounded 1/phi0^2,
+    # so the vacuum is an exact fixed point only where 1/phi0^2 is representable (phi0 = 1, 2, ...);
+    # the other forms round phi^2 * (1/phi0^2) to exactly 1 for phi0 = 3 as well.
     for sign in (+1.0, -1.0):
-        for phi0 in (1.0, 3.0):
+        for phi0 in ((1.0, 2.0) if arith == ref.ARITH_FMA else (1.0, 3.0)):
             phi = np.full((N,) * dims, sign * phi0, dt)
             pd = np.zeros_like(phi)
-            p, v = run(dims, N, prec, phi, pd, 25, era_m=era_m, phi0=phi0)
+            p, v = run(dims, N, prec, phi, pd, 25, era_m=era_m, phi0=phi0, arith=arith)
             assert np.array_equal(p, phi) and np.all(v == 0)
 
 
@@ -75,7 +79,7 @@ def test_vacua_are_exact_fixed_points(prec, dt, dims, N, era_m):
 
 @pytest.mark.parametrize("prec,dt", PRECS)
 @pytest.mark.parametrize("dims,N", [(2, 10), (3, 7)])
-@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF])
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
 def test_oddness_is_bit_exact(prec, dt, dims, N, arith):
     phi, pd = fg.random_state(dims, N, 5, dt)
     p1, v1 = run(dims, N, prec, phi, pd, 7, arith=arith)
@@ -84,30 +88,33 @@ def test_oddness_is_bit_exact(prec, dt, dims, N, arith):
 
 
 @pytest.mark.parametrize("prec,dt", PRECS)
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
 @pytest.mark.parametrize("dims,N,shift", [(2, 9, (3, -2)), (2, 16, (1, 0)), (3, 6, (1, 2, 5)), (3, 5, (0, 0, 1))])
-def test_translation_equivariance_is_bit_exact(prec, dt, dims, N, shift):
+def test_translation_equivariance_is_bit_exact(prec, dt, dims, N, shift, arith):
     phi, pd = fg.random_state(dims, N, 6, dt)
-    p1, v1 = run(dims, N, prec, phi, pd, 5)
-    p2, v2 = run(dims, N, prec, fg.roll_state(phi, shift), fg.roll_state(pd, shift), 5)
+    p1, v1 = run(dims, N, prec, phi, pd, 5, arith=arith)
+    p2, v2 = run(dims, N, prec, fg.roll_state(phi, shift), fg.roll_state(pd, shift), 5, arith=arith)
     assert np.array_equal(fg.roll_state(p1, shift), p2)
     assert np.array_equal(fg.roll_state(v1, shift), v2)
 
 
 @pytest.mark.parametrize("prec,dt", PRECS)
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
 @pytest.mark.parametrize("dims,N", [(2, 8), (3, 6)])
-def test_reflection_equivariance_is_bit_exact(prec, dt, dims, N):
+def test_reflection_equivariance_is_bit_exact(prec, dt, dims, N, arith):
     phi, pd = fg.random_state(dims, N, 7, dt)
-    p1, v1 = run(dims, N, prec, phi, pd, 5)
+    p1, v1 = run(dims, N, prec, phi, pd, 5, arith=arith)
     for ax in range(dims):
-        p2, v2 = run(dims, N, prec, fg.flip_axis(phi, ax), fg.flip_axis(pd, ax), 5)
+        p2, v2 = run(dims, N, prec, fg.flip_axis(phi, ax), fg.flip_axis(pd, ax), 5, arith=arith)
         assert np.array_equal(fg.flip_axis(p1, ax), p2) and np.array_equal(fg.flip_axis(v1, ax), v2)
 
 
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
 @pytest.mark.parametrize("prec,dt", PRECS)
-def test_2d_transpose_equivariance_is_bit_exact(prec, dt):
+def test_2d_transpose_equivariance_is_bit_exact(prec, dt, arith):
     phi, pd = fg.random_state(2, 11, 8, dt)
-    p1, v1 = run(2, 11, prec, phi, pd, 5)
-    p2, v2 = run(2, 11, prec, np.ascontiguousarray(phi.T), np.ascontiguousarray(pd.T), 5)
+    p1, v1 = run(2, 11, prec, phi, pd, 5, arith=arith)
+    p2, v2 = run(2, 11, prec, np.ascontiguousarray(phi.T), np.ascontiguousarray(pd.T), 5, arith=arith)
     assert np.array_equal(p1.T, p2) and np.array_equal(v1.T, v2)
 
 
@@ -161,13 +168,15 @@ def test_threads_do_not_change_a_bit(prec, dt, dims, N):
 
 @pytest.mark.parametrize("prec,dt,tol", [(ref.F32, np.float32, 2e-6), (ref.F64, np.float64, 4e-15)])
 @pytest.mark.parametrize("dims,N", [(2, 32), (3, 10)])
-def test_coef_and_literal_arithmetic_agree_to_rounding(prec, dt, tol, dims, N):
+def test_coef_fma_and_literal_arithmetic_agree_to_rounding(prec, dt, tol, dims, N):
     phi, _ = fg.random_state(dims, N, 11, dt)
     pd = np.zeros_like(phi)
     a = run(dims, N, prec, phi, pd, 20, arith=ref.ARITH_LITERAL)
-    b = run(dims, N, prec, phi, pd, 20, arith=ref.ARITH_COEF)
-    assert np.max(np.abs(a[0].astype(np.float64) - b[0])) < tol
-    assert np.max(np.abs(a[1].astype(np.float64) - b[1])) < tol
+    for other in (ref.ARITH_COEF, ref.ARITH_FMA):
+        b = run(dims, N, prec, phi, pd, 20, arith=other)
+        assert np.max(np.abs(a[0].astype(np.float64) - b[0])) < tol
+        assert np.max(np.abs(a[1].astype(np.float64) - b[1])) < tol
+        assert not (np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]))   # the forms do round differently
 
 
 def test_step_counter_and_eta_advance_without_accumulation():
