@@ -57,11 +57,11 @@ typedef struct {
 /* Options for prs_set_option (all have defaults; tests use them to force one kernel). */
 enum {
     PRS_OPT_STEP_KERNEL = 1,   /* PRS_KERNEL_*                                   default AUTO     */
-    PRS_OPT_ARITH       = 2,   /* PRS_ARITH_*                                    default COEF     */
+    PRS_OPT_ARITH       = 2,   /* PRS_ARITH_*                                    default FMA      */
     PRS_OPT_DIAG_KERNEL = 3,   /* PRS_KERNEL_AUTO / GENERIC / TILED              default AUTO     */
     PRS_OPT_CHUNK       = 4,   /* tuning: planes (3D) / rows (2D) one CTA marches; 0 = auto        */
     PRS_OPT_TILE_Y      = 5,   /* tuning: rows per CTA of the 3D tiled kernel, 4 / 8 / 16          */
-    PRS_OPT_TB2_TILE_Y  = 6    /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 */
+    PRS_OPT_TB2_TILE_Y  = 6    /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
 };
 enum {
     PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */
@@ -70,11 +70,15 @@ enum {
     PRS_KERNEL_TB2     = 3     /* temporally blocked: two steps per pass over HBM (same per-site   *
                                 * arithmetic, bit-identical to two single steps)                   */
 };
-/* Velocity update, Eq. 4 (:49): LITERAL divides per site, ((1-d)*v + deta*f)/(1+d); COEF uses
- * A = (1-d)/(1+d) and B = deta/(1+d) formed in double on the host once per step, v' = A*v + B*f.
- * Neither ever contracts a multiply and an add into an FMA, so each matches the oracle's
- * arithmetic of the same name bit for bit. */
-enum { PRS_ARITH_LITERAL = 0, PRS_ARITH_COEF = 1 };
+/* Arithmetic form of Eqs. 3-5 (R13).  LITERAL: Eq. 4 (:49) as printed, one division per
+ * site, ((1-d)*v + deta*f)/(1+d).  COEF: A = (1-d)/(1+d) and B = deta/(1+d) formed in double on the
+ * host once per step, v' = A*v + B*f.  In both, every multiply and add is rounded on its own (never
+ * contracted).  FMA (default): COEF with every product that feeds a sum contracted into one fused
+ * multiply-add -- lap = fma(-2d, c, sum); t = fma(c*c, 1/phi0^2, -1); f = fma((-K)*c, t, lap);
+ * v' = fma(A, v, B*f); phi' = fma(deta, v', c) -- what a compiler emits from the formulas by default,
+ * and the fastest form.  Each form matches the oracle's form of the same name bit for bit; all three
+ * agree within rounding (about 2e-7 FP32 / 4e-16 FP64 after 20 steps). */
+enum { PRS_ARITH_LITERAL = 0, PRS_ARITH_COEF = 1, PRS_ARITH_FMA = 2 };
 
 /* Read-only counters for prs_get_info. */
 enum {

@@ -145,10 +145,10 @@ int resolve_step_kernel(const prs_ctx* h) {
 
 // ---- launches -----------------------------------------------------------------------------------
 
-template <typename T, int DIMS, bool LITERAL>
+template <typename T, int DIMS, int ARITH>
 cudaError_t launch_generic(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
     const unsigned blocks = (unsigned)((h->S + 255) / 256);
-    step_generic_kernel<T, DIMS, LITERAL><<<blocks, 256, 0, h->stream>>>(p, v, pn, vn, (long long)h->N,
+    step_generic_kernel<T, DIMS, ARITH><<<blocks, 256, 0, h->stream>>>(p, v, pn, vn, (long long)h->N,
                                                                          (long long)h->S, k);
     return cudaGetLastError();
 }
@@ -170,7 +170,7 @@ int pick_chunk(const prs_ctx* h, long long tiles_per_slab, int threads_per_cta) 
     return (int)len;
 }
 
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 cudaError_t launch_tiled3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
     constexpr int W = VecOps<T>::W;
     const int N = (int)h->N;
@@ -179,13 +179,13 @@ cudaError_t launch_tiled3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     const int ZC = pick_chunk(h, (long long)gx * gy, 32 * ty);
     const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
     const dim3 block(32, ty, 1);
-    if (ty == 4) step3d_tiled_kernel<T, LITERAL, 4><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
-    else if (ty == 16) step3d_tiled_kernel<T, LITERAL, 16><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
-    else step3d_tiled_kernel<T, LITERAL, 8><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    if (ty == 4) step3d_tiled_kernel<T, ARITH, 4><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    else if (ty == 16) step3d_tiled_kernel<T, ARITH, 16><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    else step3d_tiled_kernel<T, ARITH, 8><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
     return cudaGetLastError();
 }
 
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 cudaError_t launch_tiled2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
     constexpr int W = VecOps<T>::W;
     const int N = (int)h->N;
@@ -193,11 +193,11 @@ cudaError_t launch_tiled2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     const unsigned gx = (unsigned)((N + BX * W - 1) / (BX * W));
     const int YC = pick_chunk(h, gx, BX);
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
-    step2d_tiled_kernel<T, LITERAL><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k);
+    step2d_tiled_kernel<T, ARITH><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k);
     return cudaGetLastError();
 }
 
-template <typename T, bool LITERAL, int TY>
+template <typename T, int ARITH, int TY>
 cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
                              const StepCoef<T>& k2) {
     constexpr int W = VecOps<T>::W;
@@ -205,7 +205,7 @@ cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, c
     const size_t smem = tb2_smem_bytes<T, TY>();
     static bool configured = false;            // per instantiation
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step3d_tb2_kernel<T, LITERAL, TY>,
+        cudaError_t e = cudaFuncSetAttribute(step3d_tb2_kernel<T, ARITH, TY>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
@@ -214,24 +214,22 @@ cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, c
     int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
     const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
     const dim3 block(32, TY + 4, 1);
-    step3d_tb2_kernel<T, LITERAL, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, k1, k2);
+    step3d_tb2_kernel<T, ARITH, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, k1, k2);
     return cudaGetLastError();
 }
 
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 cudaError_t launch_tb2_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
                           const StepCoef<T>& k2) {
     switch (h->opt_tb2_tile_y) {
-        case 4: return launch_tb2_3d_ty<T, LITERAL, 4>(h, p, v, pn, vn, k1, k2);
-        case 8: return launch_tb2_3d_ty<T, LITERAL, 8>(h, p, v, pn, vn, k1, k2);
-        case 10: return launch_tb2_3d_ty<T, LITERAL, 10>(h, p, v, pn, vn, k1, k2);
-        case 20: return launch_tb2_3d_ty<T, LITERAL, 20>(h, p, v, pn, vn, k1, k2);
-        case 28: return launch_tb2_3d_ty<T, LITERAL, 28>(h, p, v, pn, vn, k1, k2);
-        default: return launch_tb2_3d_ty<T, LITERAL, 12>(h, p, v, pn, vn, k1, k2);
+        case 4: return launch_tb2_3d_ty<T, ARITH, 4>(h, p, v, pn, vn, k1, k2);
+        case 8: return launch_tb2_3d_ty<T, ARITH, 8>(h, p, v, pn, vn, k1, k2);
+        case 28: return launch_tb2_3d_ty<T, ARITH, 28>(h, p, v, pn, vn, k1, k2);
+        default: return launch_tb2_3d_ty<T, ARITH, 12>(h, p, v, pn, vn, k1, k2);
     }
 }
 
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
                           const StepCoef<T>& k2) {
     constexpr int W = VecOps<T>::W;
@@ -241,7 +239,7 @@ cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, cons
     const unsigned gx = (nwarps + warps - 1) / warps;
     int YC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
-    step2d_tb2_kernel<T, LITERAL><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k1, k2);
+    step2d_tb2_kernel<T, ARITH><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k1, k2);
     return cudaGetLastError();
 }
 
@@ -253,10 +251,10 @@ int step_twice(prs_ctx* h) {
     const T* v = (const T*)h->pd[h->cur];
     T* pn = (T*)h->phi[h->cur ^ 1];
     T* vn = (T*)h->pd[h->cur ^ 1];
-    const bool lit = (h->opt_arith == PRS_ARITH_LITERAL);
     cudaError_t e;
-    if (h->dims == 3) e = lit ? launch_tb2_3d<T, true>(h, p, v, pn, vn, k1, k2) : launch_tb2_3d<T, false>(h, p, v, pn, vn, k1, k2);
-    else e = lit ? launch_tb2_2d<T, true>(h, p, v, pn, vn, k1, k2) : launch_tb2_2d<T, false>(h, p, v, pn, vn, k1, k2);
+#define PRS_TB2(AR) (h->dims == 3 ? launch_tb2_3d<T, AR>(h, p, v, pn, vn, k1, k2) : launch_tb2_2d<T, AR>(h, p, v, pn, vn, k1, k2))
+    e = (h->opt_arith == PRS_ARITH_LITERAL) ? PRS_TB2(ARITH_LITERAL) : (h->opt_arith == PRS_ARITH_COEF) ? PRS_TB2(ARITH_COEF) : PRS_TB2(ARITH_FMA);
+#undef PRS_TB2
     if (e != cudaSuccess) return cuda_fail(h, e, "two-step kernel launch");
     h->launches += 1;
     h->cur ^= 1;
@@ -271,15 +269,13 @@ int step_once(prs_ctx* h, int kernel) {
     const T* v = (const T*)h->pd[h->cur];
     T* pn = (T*)h->phi[h->cur ^ 1];
     T* vn = (T*)h->pd[h->cur ^ 1];
-    const bool lit = (h->opt_arith == PRS_ARITH_LITERAL);
     cudaError_t e;
-    if (kernel == PRS_KERNEL_TILED) {
-        if (h->dims == 3) e = lit ? launch_tiled3d<T, true>(h, p, v, pn, vn, k) : launch_tiled3d<T, false>(h, p, v, pn, vn, k);
-        else e = lit ? launch_tiled2d<T, true>(h, p, v, pn, vn, k) : launch_tiled2d<T, false>(h, p, v, pn, vn, k);
-    } else {
-        if (h->dims == 3) e = lit ? launch_generic<T, 3, true>(h, p, v, pn, vn, k) : launch_generic<T, 3, false>(h, p, v, pn, vn, k);
-        else e = lit ? launch_generic<T, 2, true>(h, p, v, pn, vn, k) : launch_generic<T, 2, false>(h, p, v, pn, vn, k);
-    }
+#define PRS_ONE(AR)                                                                                                      \
+    (kernel == PRS_KERNEL_TILED                                                                                           \
+         ? (h->dims == 3 ? launch_tiled3d<T, AR>(h, p, v, pn, vn, k) : launch_tiled2d<T, AR>(h, p, v, pn, vn, k))         \
+         : (h->dims == 3 ? launch_generic<T, 3, AR>(h, p, v, pn, vn, k) : launch_generic<T, 2, AR>(h, p, v, pn, vn, k)))
+    e = (h->opt_arith == PRS_ARITH_LITERAL) ? PRS_ONE(ARITH_LITERAL) : (h->opt_arith == PRS_ARITH_COEF) ? PRS_ONE(ARITH_COEF) : PRS_ONE(ARITH_FMA);
+#undef PRS_ONE
     if (e != cudaSuccess) return cuda_fail(h, e, "step kernel launch");
     h->launches += 1;
     h->cur ^= 1;
@@ -394,7 +390,7 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     h->partials = (DiagPartial*)(h->ws + L.off_partials);
     h->d_result = (DiagPartial*)(h->ws + L.off_result);
     h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
-    h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_COEF; h->opt_diag_kernel = PRS_KERNEL_AUTO;
+    h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_FMA; h->opt_diag_kernel = PRS_KERNEL_AUTO;
     h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     h->h_result = nullptr;
@@ -517,7 +513,7 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             }
             return fail(h, PRS_ERR_INVALID_ARG, "unknown step kernel");
         case PRS_OPT_ARITH:
-            if (value != PRS_ARITH_LITERAL && value != PRS_ARITH_COEF) return fail(h, PRS_ERR_INVALID_ARG, "unknown arithmetic");
+            if (value != PRS_ARITH_LITERAL && value != PRS_ARITH_COEF && value != PRS_ARITH_FMA) return fail(h, PRS_ERR_INVALID_ARG, "unknown arithmetic");
             h->opt_arith = (int)value;
             return PRS_OK;
         case PRS_OPT_DIAG_KERNEL:
@@ -537,8 +533,8 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             h->opt_tile_y = (int)value;
             return PRS_OK;
         case PRS_OPT_TB2_TILE_Y:
-            if (value != 4 && value != 8 && value != 10 && value != 12 && value != 20 && value != 28)
-                return fail(h, PRS_ERR_INVALID_ARG, "tb2_tile_y must be 4, 8, 10, 12, 20 or 28");
+            if (value != 4 && value != 8 && value != 12 && value != 28)
+                return fail(h, PRS_ERR_INVALID_ARG, "tb2_tile_y must be 4, 8, 12 or 28");
             h->opt_tb2_tile_y = (int)value;
             return PRS_OK;
         default:

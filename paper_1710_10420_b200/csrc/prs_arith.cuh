@@ -20,6 +20,7 @@ template <> struct Ar<float> {
     static __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
     static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
     static __device__ __forceinline__ float div(float a, float b) { return __fdiv_rn(a, b); }
+    static __device__ __forceinline__ float fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
     static __device__ __forceinline__ bool neg(float v) { return (__float_as_uint(v) >> 31) != 0u; }
 };
 
@@ -28,8 +29,12 @@ template <> struct Ar<double> {
     static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
     static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
     static __device__ __forceinline__ double div(double a, double b) { return __ddiv_rn(a, b); }
+    static __device__ __forceinline__ double fma(double a, double b, double c) { return __fma_rn(a, b, c); }
     static __device__ __forceinline__ bool neg(double v) { return __double2hiint(v) < 0; }
 };
+
+// Arithmetic forms (values of PRS_ARITH_* in prs.h).
+constexpr int ARITH_LITERAL = 0, ARITH_COEF = 1, ARITH_FMA = 2;
 
 // Per-step scalars in the field's precision; formed on the host in double (Eq. 6) and rounded once.
 template <typename T>
@@ -58,10 +63,10 @@ __device__ __forceinline__ T force(const StepCoef<T>& k, T c, T sxy, T sz) {
     return A::sub(lap, dV);
 }
 
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 __device__ __forceinline__ T velocity(const StepCoef<T>& k, T pd, T f) {
     using A = Ar<T>;
-    if (LITERAL) {
+    if (ARITH == ARITH_LITERAL) {
         const T num = A::add(A::mul(k.omd, pd), A::mul(k.deta, f));
         return A::div(num, k.opd);                                // Eq. 4 as printed
     }
@@ -73,14 +78,24 @@ __device__ __forceinline__ T advance(const StepCoef<T>& k, T c, T pd_new) {
     return Ar<T>::add(c, Ar<T>::mul(k.deta, pd_new));             // Eq. 5
 }
 
-template <typename T, int DIMS, bool LITERAL>
+template <typename T, int DIMS, int ARITH>
 __device__ __forceinline__ void site_update(const StepCoef<T>& k, T c, T xm, T xp, T ym, T yp, T zm,
                                             T zp, T pd, T& phi_new, T& pd_new) {
     using A = Ar<T>;
     const T sxy = A::add(A::add(xp, xm), A::add(yp, ym));
     const T sz = (DIMS == 3) ? A::add(zp, zm) : T(0);
+    if (ARITH == ARITH_FMA) {
+        // Contracted form (R13): every product that feeds a sum is one fused multiply-add.
+        const T sum = (DIMS == 3) ? A::add(sxy, sz) : sxy;
+        const T lap = A::fma(T(-2 * DIMS), c, sum);               // Eq. 3
+        const T t = A::fma(A::mul(c, c), k.I, T(-1));
+        const T f = A::fma(A::mul(-k.K, c), t, lap);              // lap - dV/dphi
+        pd_new = A::fma(k.A, pd, A::mul(k.B, f));                 // Eq. 4
+        phi_new = A::fma(k.deta, pd_new, c);                      // Eq. 5
+        return;
+    }
     const T f = force<T, DIMS>(k, c, sxy, sz);
-    pd_new = velocity<T, LITERAL>(k, pd, f);
+    pd_new = velocity<T, ARITH>(k, pd, f);
     phi_new = advance<T>(k, c, pd_new);
 }
 

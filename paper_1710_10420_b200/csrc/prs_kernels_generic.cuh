@@ -66,7 +66,7 @@ init_kernel(T* __restrict__ phi, T* __restrict__ phidot, long long S, unsigned l
 // ------------------------------------------------------------------------------------------------
 // Generic step: one thread per site, neighbours by modulo wrap (Eqs. 3-5).
 // ------------------------------------------------------------------------------------------------
-template <typename T, int DIMS, bool LITERAL>
+template <typename T, int DIMS, int ARITH>
 __global__ void __launch_bounds__(256)
 step_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
                     T* __restrict__ phidot_next, long long N, long long S, StepCoef<T> k) {
@@ -88,7 +88,7 @@ step_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
         zpv = phi[pil + (z == N - 1 ? 0 : z + 1) * NN];
     }
     T pn, vn;
-    site_update<T, DIMS, LITERAL>(k, phi[s], phi[xm], phi[xp], phi[ym], phi[yp], zmv, zpv, phidot[s], pn, vn);
+    site_update<T, DIMS, ARITH>(k, phi[s], phi[xm], phi[xp], phi[ym], phi[yp], zmv, zpv, phidot[s], pn, vn);
     phi_next[s] = pn;
     phidot_next[s] = vn;
 }

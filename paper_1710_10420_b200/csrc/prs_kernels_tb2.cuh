@@ -58,7 +58,7 @@ constexpr size_t tb2_smem_bytes() {
     return (size_t)(TB2_RA + TB2_RP + 2) * (TY + 4) * 32 * 16;
 }
 
-template <typename T, bool LITERAL, int TY>
+template <typename T, int ARITH, int TY>
 __global__ void __launch_bounds__(32 * (TY + 4), (32 * (TY + 4) > 512) ? 1 : 2)
 step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int ZC, StepCoef<T> k1, StepCoef<T> k2) {
@@ -148,7 +148,7 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             const T left1 = __shfl_up_sync(0xffffffffu, K::last(a_c), 1);
             const T right1 = __shfl_down_sync(0xffffffffu, K::first(a_c), 1);
             V b_new, q_new;
-            packed_vector_update<T, 3, LITERAL>(c1, a_c, left1, right1, ym1, yp1, a_zm, zp, pd, b_new, q_new);
+            packed_vector_update<T, 3, ARITH>(c1, a_c, left1, right1, ym1, yp1, a_zm, zp, pd, b_new, q_new);
             sB[(U & 1) * PLANE] = b_new;
             a_zm = a_c; a_c = zp;
             // No barrier here: stage 2 reads the plane published one iteration ago (slot (j-1)&1),
@@ -161,7 +161,7 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
                 const T left2 = __shfl_up_sync(0xffffffffu, K::last(b_cur), 1);
                 const T right2 = __shfl_down_sync(0xffffffffu, K::first(b_cur), 1);
                 V pout, vout;
-                packed_vector_update<T, 3, LITERAL>(c2, b_cur, left2, right2, ym2, yp2, b_prev, b_new, q_cur, pout, vout);
+                packed_vector_update<T, 3, ARITH>(c2, b_cur, left2, right2, ym2, yp2, b_prev, b_new, q_cur, pout, vout);
                 if (store_ok) {
                     oP[io] = vout;
                     oA[io] = pout;
@@ -192,7 +192,7 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 // ------------------------------------------------------------------------------------------------
 // 2D: block = BX lanes (multiple of 32); every warp outputs 30 vectors of x and marches YC rows.
 // ------------------------------------------------------------------------------------------------
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 __global__ void __launch_bounds__(128)
 step2d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int YC, StepCoef<T> k1, StepCoef<T> k2) {
@@ -247,14 +247,14 @@ step2d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
         {
             const T left = __shfl_up_sync(0xffffffffu, K::last(a_cur), 1);
             const T right = __shfl_down_sync(0xffffffffu, K::first(a_cur), 1);
-            packed_vector_update<T, 2, LITERAL>(c1, a_cur, left, right, a_prev, a_next, zero, zero, pd, b_new, q_new);
+            packed_vector_update<T, 2, ARITH>(c1, a_cur, left, right, a_prev, a_next, zero, zero, pd, b_new, q_new);
         }
         // stage 2 on row yo = y0+j-2
         if (j >= 2) {
             const T left = __shfl_up_sync(0xffffffffu, K::last(b_cur), 1);
             const T right = __shfl_down_sync(0xffffffffu, K::first(b_cur), 1);
             V pout, vout;
-            packed_vector_update<T, 2, LITERAL>(c2, b_cur, left, right, b_prev, b_new, zero, zero, q_cur, pout, vout);
+            packed_vector_update<T, 2, ARITH>(c2, b_cur, left, right, b_prev, b_new, zero, zero, q_cur, pout, vout);
             if (store_ok) {
                 K::stg(vo, vout);
                 K::stg(po, pout);

@@ -47,7 +47,7 @@ template <> struct VecOps<double> {
 
 // One vector of sites: c = centre vector, left/right = the scalars beside it in x, (ym, yp) and
 // (zm, zp) the vectors beside it along the other axes.
-template <typename T, int DIMS, bool LITERAL>
+template <typename T, int DIMS, int ARITH>
 __device__ __forceinline__ void vector_update(const StepCoef<T>& k, typename VecOps<T>::V c, T left, T right,
                                               typename VecOps<T>::V ym, typename VecOps<T>::V yp,
                                               typename VecOps<T>::V zm, typename VecOps<T>::V zp,
@@ -59,7 +59,7 @@ __device__ __forceinline__ void vector_update(const StepCoef<T>& k, typename Vec
         const T xm = (i == 0) ? left : O::get(c, i - 1);
         const T xp = (i == O::W - 1) ? right : O::get(c, i + 1);
         T pn, vn;
-        site_update<T, DIMS, LITERAL>(k, O::get(c, i), xm, xp, O::get(ym, i), O::get(yp, i), O::get(zm, i),
+        site_update<T, DIMS, ARITH>(k, O::get(c, i), xm, xp, O::get(ym, i), O::get(yp, i), O::get(zm, i),
                                       O::get(zp, i), O::get(pd, i), pn, vn);
         O::set(phi_new, i, pn);
         O::set(pd_new, i, vn);
@@ -69,7 +69,7 @@ __device__ __forceinline__ void vector_update(const StepCoef<T>& k, typename Vec
 // ------------------------------------------------------------------------------------------------
 // 3D: block = 32 lanes in x  x  TYB rows in y; grid = (x tiles, y tiles, z chunks of ZC planes).
 // ------------------------------------------------------------------------------------------------
-template <typename T, bool LITERAL, int TYB>
+template <typename T, int ARITH, int TYB>
 __global__ void __launch_bounds__(32 * TYB)
 step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
                     T* __restrict__ phidot_next, int N, int ZC, StepCoef<T> k) {
@@ -124,7 +124,7 @@ step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
         if (edge_l) left = el;
         if (edge_r) right = er;
         V pnew, vnew;
-        vector_update<T, 3, LITERAL>(k, cur, left, right, dn, up, prev, nxt, pd, pnew, vnew);
+        vector_update<T, 3, ARITH>(k, cur, left, right, dn, up, prev, nxt, pd, pnew, vnew);
         if (live) {
             const size_t o = (size_t)z * NN + rc;
             O::st(phidot_next + o, vnew);
@@ -139,7 +139,7 @@ step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
 // 2D: block = BX lanes in x; grid = (x tiles, y chunks of YC rows).  The march axis is y, so the
 // register window supplies both y neighbours and nothing but the two edge scalars is re-read.
 // ------------------------------------------------------------------------------------------------
-template <typename T, bool LITERAL>
+template <typename T, int ARITH>
 __global__ void __launch_bounds__(128)
 step2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
                     T* __restrict__ phidot_next, int N, int YC, StepCoef<T> k) {
@@ -183,7 +183,7 @@ step2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
         if (edge_l) left = el;
         if (edge_r) right = er;
         V pnew, vnew;
-        vector_update<T, 2, LITERAL>(k, cur, left, right, prev, nxt, zero, zero, pd, pnew, vnew);
+        vector_update<T, 2, ARITH>(k, cur, left, right, prev, nxt, zero, zero, pd, pnew, vnew);
         if (live) {
             const size_t o = (size_t)y * N + x;
             O::st(phidot_next + o, vnew);

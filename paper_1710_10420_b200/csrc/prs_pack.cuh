@@ -24,6 +24,7 @@ template <> struct Pk<float> {
     static constexpr int W = 4;
     static __device__ __forceinline__ P add(P a, P b) { P r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
     static __device__ __forceinline__ P mul(P a, P b) { P r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+    static __device__ __forceinline__ P fma(P a, P b, P c) { P r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
     static __device__ __forceinline__ P pack(float lo, float hi) { P r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
     static __device__ __forceinline__ void unpack(P p, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p)); }
     static __device__ __forceinline__ P dup(float s) { return pack(s, s); }
@@ -58,6 +59,7 @@ template <> struct Pk<double> {
     static constexpr int W = 2;
     static __device__ __forceinline__ P add(P a, P b) { return __dadd_rn(a, b); }
     static __device__ __forceinline__ P mul(P a, P b) { return __dmul_rn(a, b); }
+    static __device__ __forceinline__ P fma(P a, P b, P c) { return __fma_rn(a, b, c); }
     static __device__ __forceinline__ P dup(double s) { return s; }
     static __device__ __forceinline__ P addm(P a, P m) { return __dadd_rn(a, m); }
     static __device__ __forceinline__ P div(P a, P b) { return __ddiv_rn(a, b); }
@@ -87,7 +89,7 @@ struct PackCoef {
 
 // One pack of sites: c centre, sx = x+1 plus x-1 (already summed), (ym, yp), (zm, zp) neighbours,
 // pd = phidot^{n-1/2}.  Same operations, same order as site_update() in prs_arith.cuh.
-template <typename T, int DIMS, bool LITERAL>
+template <typename T, int DIMS, int ARITH>
 __device__ __forceinline__ void pack_update(const PackCoef<T>& k, typename Pk<T>::P c, typename Pk<T>::P sx,
                                             typename Pk<T>::P ym, typename Pk<T>::P yp, typename Pk<T>::P zm,
                                             typename Pk<T>::P zp, typename Pk<T>::P pd, typename Pk<T>::P& phi_new,
@@ -95,19 +97,28 @@ __device__ __forceinline__ void pack_update(const PackCoef<T>& k, typename Pk<T>
     using K = Pk<T>;
     typename K::P sum = K::add(sx, K::add(yp, ym));
     if (DIMS == 3) sum = K::add(sum, K::add(zp, zm));
+    if (ARITH == ARITH_FMA) {
+        // Contracted form (R13): FFMA2 / DFMA, one rounding per product-sum.
+        const typename K::P lapf = K::fma(k.n2d, c, sum);                // Eq. 3
+        const typename K::P tf = K::fma(K::mul(c, c), k.I, k.m1);
+        const typename K::P ff = K::fma(K::mul(k.nK, c), tf, lapf);      // lap - dV/dphi
+        pd_new = K::fma(k.A, pd, K::mul(k.B, ff));                       // Eq. 4
+        phi_new = K::fma(k.deta, pd_new, c);                             // Eq. 5
+        return;
+    }
     const typename K::P lap = K::addm(sum, K::mul(k.n2d, c));             // Eq. 3:  sum - 2d*c
     const typename K::P q = K::mul(c, c);
     const typename K::P r = K::mul(q, k.I);
     const typename K::P t = K::addm(k.m1, r);                          // r - 1
     const typename K::P ndV = K::mul(K::mul(k.nK, c), t);                // -(K*c)*t = -dV/dphi (Eq. 1)
     const typename K::P f = K::addm(lap, ndV);                          // lap - dV
-    if (LITERAL) pd_new = K::div(K::addm(K::mul(k.omd, pd), K::mul(k.deta, f)), k.opd);   // Eq. 4 as printed
+    if (ARITH == ARITH_LITERAL) pd_new = K::div(K::addm(K::mul(k.omd, pd), K::mul(k.deta, f)), k.opd);   // Eq. 4 as printed
     else pd_new = K::addm(K::mul(k.A, pd), K::mul(k.B, f));             // Eq. 4, pre-divided coefficients
     phi_new = K::addm(c, K::mul(k.deta, pd_new));                      // Eq. 5
 }
 
 // One 16-byte vector of sites (two packs).
-template <typename T, int DIMS, bool LITERAL>
+template <typename T, int DIMS, int ARITH>
 __device__ __forceinline__ void packed_vector_update(const PackCoef<T>& k, typename Pk<T>::V c, T left, T right,
                                                      typename Pk<T>::V ym, typename Pk<T>::V yp,
                                                      typename Pk<T>::V zm, typename Pk<T>::V zp,
@@ -115,8 +126,8 @@ __device__ __forceinline__ void packed_vector_update(const PackCoef<T>& k, typen
                                                      typename Pk<T>::V& pd_new) {
     using K = Pk<T>;
     const typename K::V sx = K::xsum(c, left, right);
-    pack_update<T, DIMS, LITERAL>(k, c.x, sx.x, ym.x, yp.x, zm.x, zp.x, pd.x, phi_new.x, pd_new.x);
-    pack_update<T, DIMS, LITERAL>(k, c.y, sx.y, ym.y, yp.y, zm.y, zp.y, pd.y, phi_new.y, pd_new.y);
+    pack_update<T, DIMS, ARITH>(k, c.x, sx.x, ym.x, yp.x, zm.x, zp.x, pd.x, phi_new.x, pd_new.x);
+    pack_update<T, DIMS, ARITH>(k, c.y, sx.y, ym.y, yp.y, zm.y, zp.y, pd.y, phi_new.y, pd_new.y);
 }
 
 }  // namespace prs

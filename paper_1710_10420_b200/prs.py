@@ -13,7 +13,7 @@ import ctypes as C
 from . import build as _build
 
 F32, F64 = 0, 1
-ARITH_LITERAL, ARITH_COEF = 0, 1
+ARITH_LITERAL, ARITH_COEF, ARITH_FMA = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_TB2 = 0, 1, 2, 3
 OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y = 1, 2, 3, 4, 5, 6
 INFO_KERNEL_LAUNCHES, INFO_STEP_KERNEL, INFO_STEP, INFO_DIAG_KERNEL = 1, 2, 3, 4

@@ -2,8 +2,9 @@
 
 Bars (BASELINE.json north_star): link count bit-exact on any snapshot; fields after 20 steps within
 1e-12 (FP64) / 2e-5 (FP32) of the oracle as the paper prints the update (LITERAL arithmetic).  On top
-of that, with the same arithmetic form on both sides (COEF or LITERAL) the fields must be IDENTICAL
-bit for bit, because neither side ever fuses a multiply with an add.
+of that, with the same arithmetic form on both sides (FMA, COEF or LITERAL; R13) the fields
+must be IDENTICAL bit for bit: IEEE-754 fixes every operation of each form, and neither side ever
+contracts (or splits) a multiply-add that the form does not prescribe.
 """
 import os
 
@@ -23,7 +24,7 @@ THREADS = max(1, min(32, len(os.sched_getaffinity(0))))
 KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED, prs.KERNEL_TB2]
 
 
-def make_pair(dims, N, prec, arith_gpu=prs.ARITH_COEF, arith_ref=ref.ARITH_LITERAL, kernel=prs.KERNEL_AUTO, **kw):
+def make_pair(dims, N, prec, arith_gpu=prs.ARITH_FMA, arith_ref=ref.ARITH_LITERAL, kernel=prs.KERNEL_AUTO, **kw):
     g = prs.Simulation(dims, N, prec, **kw)
     g.set_arith(arith_gpu)
     g.set_step_kernel(kernel)
@@ -61,7 +62,7 @@ CASES_3D = [4, 20, 36, 64, 132]
 @pytest.mark.parametrize("dims,N", [(2, n) for n in CASES_2D] + [(3, n) for n in CASES_3D])
 @pytest.mark.parametrize("era_m", [1.0, 2.0])
 def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
-    # (a) tolerance bar against the paper's literal form, GPU in its default COEF form
+    # (a) tolerance bar against the paper's literal form, GPU in its default (FMA) form
     g, r = make_pair(dims, N, prec, kernel=kernel, era_m=era_m, seed=3)
     g.init(1.0)
     r.init(1.0)
@@ -73,7 +74,7 @@ def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
     assert g.get_info(binding.INFO_STEP_KERNEL) == kernel
     assert g.get_info(binding.INFO_STEP) == 20
     # (b) same arithmetic form on both sides -> identical bits
-    for ag, ar in ((prs.ARITH_COEF, ref.ARITH_COEF), (prs.ARITH_LITERAL, ref.ARITH_LITERAL)):
+    for ag, ar in ((prs.ARITH_FMA, ref.ARITH_FMA), (prs.ARITH_COEF, ref.ARITH_COEF), (prs.ARITH_LITERAL, ref.ARITH_LITERAL)):
         g2, r2 = make_pair(dims, N, prec, arith_gpu=ag, arith_ref=ar, kernel=kernel, era_m=era_m, seed=3)
         g2.init(1.0)
         r2.init(1.0)
@@ -86,7 +87,7 @@ def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("dims,N", [(2, 7), (2, 130), (3, 5), (3, 33)])
 def test_sizes_only_the_generic_kernel_takes(prec, dims, N):
-    g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_COEF, seed=9)
+    g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_FMA, seed=9)
     g.init(1.0)
     r.init(1.0)
     g.step(20)
@@ -147,7 +148,7 @@ def test_two_step_kernel_equals_single_steps_bitwise(prec, dims, N, nsteps):
 @pytest.mark.parametrize("dims,N", [(2, 1), (2, 2), (2, 4), (2, 5), (2, 256), (2, 520), (2, 1000), (3, 2), (3, 4), (3, 7),
                                     (3, 64), (3, 100), (3, 132)])
 def test_diagnostics_match_on_snapshots(diag_kernel, prec, dims, N):
-    g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_COEF, seed=4)
+    g, r = make_pair(dims, N, prec, arith_ref=ref.ARITH_FMA, seed=4)
     W = 4 if prec == prs.F32 else 2
     if diag_kernel == prs.KERNEL_TILED and N % W:
         with pytest.raises(prs.PrsError):
@@ -232,7 +233,7 @@ def test_restart_parity(dims, N, prec, adv):
     g.init(1.0)
     g.step(adv)
     gp, gv = g.copy_out()
-    r = ref.RefSim(dims, N, prec, arith=ref.ARITH_COEF, threads=THREADS)
+    r = ref.RefSim(dims, N, prec, arith=ref.ARITH_FMA, threads=THREADS)
     r.copy_in(gp, gv, eta0=1.0, step=adv)
     g.step(20)
     r.step(20)
@@ -357,7 +358,7 @@ def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m):
     dg = g.diagnostics()
     gp, gv = g.copy_out()
     g.close()
-    r = ref.RefSim(dims, N, prec, era_m=era_m, seed=2, arith=ref.ARITH_COEF, threads=THREADS)
+    r = ref.RefSim(dims, N, prec, era_m=era_m, seed=2, arith=ref.ARITH_FMA, threads=THREADS)
     r.init(1.0)
     r.step(20)
     dr = r.diagnostics()

@@ -75,31 +75,37 @@ def test_product_never_imports_the_oracle():
                         assert "oracle" not in ln.lower(), (f, ln)
 
 
-def test_no_fused_multiply_add_in_the_step_kernels():
-    """Bit-for-bit parity with the oracle rests on every multiply and add being rounded on its own.
-    ptxas contracts packed mul.rn.f32x2 + add.rn.f32x2 into FFMA2 whatever --fmad says (prs_pack.cuh
-    works around it), so look at the machine code: no FFMA / FFMA2 / DFMA in any step kernel of the
-    default (COEF, template argument LITERAL = false) arithmetic.  The LITERAL kernels legitimately
-    contain FMAs inside the correctly rounded division routine."""
-    import re
+def test_multiply_adds_are_fused_exactly_where_the_arithmetic_form_says():
+    """Bit-for-bit parity with the oracle rests on the machine code doing the operations the form
+    names.  ptxas contracts packed mul.rn.f32x2 + add.rn.f32x2 into FFMA2 whatever --fmad says
+    (prs_pack.cuh works around it), so look at the SASS: no FFMA / FFMA2 / DFMA in any step kernel of
+    the COEF form (template argument ARITH = 1), and fused instructions present in every kernel of
+    the FMA form (ARITH = 2).  LITERAL kernels legitimately contain FMAs inside the correctly rounded
+    division routine."""
     import shutil
     import subprocess
 
     from paper_1710_10420_b200 import build as prs_build
 
     cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
-    if not os.path.exists(cuobjdump):
-        pytest.skip("cuobjdump not available")
+    cufilt = shutil.which("cu++filt") or "/usr/local/cuda/bin/cu++filt"
+    if not (os.path.exists(cuobjdump) and os.path.exists(cufilt)):
+        pytest.skip("cuobjdump / cu++filt not available")
     sass = subprocess.run([cuobjdump, "-sass", prs_build.build()], stdout=subprocess.PIPE, text=True, check=True).stdout
-    cur, seen, bad = None, set(), []
+    names = sorted(set(re.findall(r"Function : (\S+)", sass)))
+    plain = subprocess.run([cufilt] + names, stdout=subprocess.PIPE, text=True, check=True).stdout.splitlines()
+    arith_of = {}
+    for mangled, dem in zip(names, plain):
+        m = re.search(r"prs::step_generic_kernel<\w+, \(int\)\d+, \(int\)(\d)>|prs::step\dd_(?:tiled|tb2)_kernel<\w+, \(int\)(\d)", dem)
+        if m:
+            arith_of[mangled] = int(m.group(1) or m.group(2))
+    assert sorted(set(arith_of.values())) == [0, 1, 2] and len(arith_of) >= 36
+    cur, fused = None, {k: 0 for k in arith_of}
     for line in sass.splitlines():
         m = re.search(r"Function : (\S+)", line)
         if m:
             cur = m.group(1)
-            continue
-        if cur and "step" in cur and "Lb0E" in cur:
-            seen.add(cur)
-            if re.search(r"\b(FFMA2?|DFMA)\b", line):
-                bad.append((cur, line.strip()))
-    assert len(seen) >= 12, "expected the generic, tiled and two-step kernels in the library"
-    assert not bad, bad[:5]
+        elif cur in fused and re.search(r"\b(FFMA2?|DFMA)\b", line):
+            fused[cur] += 1
+    assert [k for k, a in arith_of.items() if a == 1 and fused[k]] == []
+    assert [k for k, a in arith_of.items() if a == 2 and not fused[k]] == []
