@@ -56,8 +56,10 @@ BYTES_PER_SITE_UPDATE = {0: 16, 1: 32}        # read phi, phidot; write phidot, 
 # dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed
 # `ncu --set full` capture of the headline config (profiles/): filled in once measured.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    # profiles/r01a_ncu_step3d_tb2_f32_1024.md: 9.186 GB read + 8.551 GB written per two-step launch
-    ("3d_1024_f32_rad", "tb2"): 17_737_048_000,
+    # profiles/r01b_ncu_step3d_tb2_f32_1024.md: 9.136 GB read + 8.552 GB written per two-step launch
+    ("3d_1024_f32_rad", "tb2"): 17_687_191_000,
+    # profiles/r01b_ncu_step3d_tb2_f64_1024.md: 18.451 GB read + 17.144 GB written per two-step launch
+    ("3d_1024_f64_rad", "tb2"): 35_594_988_000,
     # profiles/r01a_ncu_step3d_tiled_f32_1024.md: 8.867 GB read + 8.549 GB written per single-step launch
     ("3d_1024_f32_rad", "tiled"): 17_415_889_000,
 }
