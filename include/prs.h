@@ -61,14 +61,18 @@ enum {
     PRS_OPT_DIAG_KERNEL = 3,   /* PRS_KERNEL_AUTO / GENERIC / TILED              default AUTO     */
     PRS_OPT_CHUNK       = 4,   /* tuning: planes (3D) / rows (2D) one CTA marches; 0 = auto        */
     PRS_OPT_TILE_Y      = 5,   /* tuning: rows per CTA of the 3D tiled kernel, 4 / 8 / 16          */
-    PRS_OPT_TB2_TILE_Y  = 6    /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
+    PRS_OPT_TB2_TILE_Y  = 6,   /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
+    PRS_OPT_TBS_STEPS   = 7    /* steps per pass of the 3D multi-step kernel, 3 or 4            default 4 */
 };
 enum {
     PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */
     PRS_KERNEL_GENERIC = 1,    /* one thread per site, any N >= 1                                  */
     PRS_KERNEL_TILED   = 2,    /* shared-memory tiled, one step per pass over HBM                  */
-    PRS_KERNEL_TB2     = 3     /* temporally blocked: two steps per pass over HBM (same per-site   *
+    PRS_KERNEL_TB2     = 3,    /* temporally blocked: two steps per pass over HBM (same per-site   *
                                 * arithmetic, bit-identical to two single steps)                   */
+    PRS_KERNEL_TBS     = 4     /* 3D only: PRS_OPT_TBS_STEPS steps per pass over HBM, bit-identical *
+                                * to single steps; leftovers of a prs_step call go through TB2 and  *
+                                * TILED                                                             */
 };
 /* Arithmetic form of Eqs. 3-5 (R13).  LITERAL: Eq. 4 (:49) as printed, one division per
  * site, ((1-d)*v + deta*f)/(1+d).  COEF: A = (1-d)/(1+d) and B = deta/(1+d) formed in double on the

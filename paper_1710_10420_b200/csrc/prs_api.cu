@@ -15,6 +15,7 @@
 #include "prs_kernels_generic.cuh"
 #include "prs_kernels_tiled.cuh"
 #include "prs_kernels_tb2.cuh"
+#include "prs_kernels_tbs.cuh"
 
 using namespace prs;
 
@@ -72,7 +73,7 @@ struct prs_ctx {
     double eta0;
     int64_t step;
     bool inited;
-    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps;
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;
@@ -262,6 +263,48 @@ int step_twice(prs_ctx* h) {
     return PRS_OK;
 }
 
+// S steps in one pass (n -> n+S), 3D only; the caller guarantees tb2_supported(h).
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
+    constexpr int TY = 16;
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    StepCoefs<T, S> ks;
+    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
+    const size_t smem = tbs_smem_bytes<T, S, TY>();
+    static bool configured = false;            // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(step3d_tbs_kernel<T, ARITH, S, TY>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    constexpr int XOUT = tbs_xout<T, S>();
+    const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
+    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
+    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const dim3 block(32, TY + 2 * S, 1);
+    step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks);
+    return cudaGetLastError();
+}
+
+template <typename T>
+int step_many(prs_ctx* h, int S) {
+    const T* p = (const T*)h->phi[h->cur];
+    const T* v = (const T*)h->pd[h->cur];
+    T* pn = (T*)h->phi[h->cur ^ 1];
+    T* vn = (T*)h->pd[h->cur ^ 1];
+    cudaError_t e;
+#define PRS_TBS(AR) (S == 3 ? launch_tbs_3d<T, AR, 3>(h, p, v, pn, vn) : launch_tbs_3d<T, AR, 4>(h, p, v, pn, vn))
+    e = (h->opt_arith == PRS_ARITH_LITERAL) ? PRS_TBS(ARITH_LITERAL) : (h->opt_arith == PRS_ARITH_COEF) ? PRS_TBS(ARITH_COEF) : PRS_TBS(ARITH_FMA);
+#undef PRS_TBS
+    if (e != cudaSuccess) return cuda_fail(h, e, "multi-step kernel launch");
+    h->launches += 1;
+    h->cur ^= 1;
+    h->step += S;
+    return PRS_OK;
+}
+
 template <typename T>
 int step_once(prs_ctx* h, int kernel) {
     const StepCoef<T> k = coef_at<T>(h, h->step);
@@ -391,7 +434,7 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     h->d_result = (DiagPartial*)(h->ws + L.off_result);
     h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
     h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_FMA; h->opt_diag_kernel = PRS_KERNEL_AUTO;
-    h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
+    h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12; h->opt_tbs_steps = 4;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     h->h_result = nullptr;
     int dev = attr.device;
@@ -436,13 +479,20 @@ int prs_step(prs_handle h, int64_t nsteps) {
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
     const int kernel = resolve_step_kernel(h);
     int64_t left = nsteps;
-    if (kernel == PRS_KERNEL_TB2) {
+    if (kernel == PRS_KERNEL_TBS) {
+        const int S = h->opt_tbs_steps;
+        for (; left >= S; left -= S) {
+            const int rc = (h->precision == PRS_F32) ? step_many<float>(h, S) : step_many<double>(h, S);
+            if (rc != PRS_OK) return rc;
+        }
+    }
+    if (kernel == PRS_KERNEL_TB2 || kernel == PRS_KERNEL_TBS) {
         for (; left >= 2; left -= 2) {
             const int rc = (h->precision == PRS_F32) ? step_twice<float>(h) : step_twice<double>(h);
             if (rc != PRS_OK) return rc;
         }
     }
-    const int single = (kernel == PRS_KERNEL_TB2) ? PRS_KERNEL_TILED : kernel;   // odd remainder
+    const int single = (kernel == PRS_KERNEL_TB2 || kernel == PRS_KERNEL_TBS) ? PRS_KERNEL_TILED : kernel;   // odd remainder
     for (; left > 0; --left) {
         const int rc = (h->precision == PRS_F32) ? step_once<float>(h, single) : step_once<double>(h, single);
         if (rc != PRS_OK) return rc;
@@ -505,6 +555,11 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
     switch (option) {
         case PRS_OPT_STEP_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
+            if (value == PRS_KERNEL_TBS) {
+                if (h->dims != 3 || !tb2_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the multi-step kernel is 3D only and needs N a multiple of 16 bytes of T");
+                h->opt_step_kernel = (int)value;
+                return PRS_OK;
+            }
             if (value == PRS_KERNEL_TILED || value == PRS_KERNEL_TB2) {
                 if (value == PRS_KERNEL_TB2 && !tb2_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the two-step kernel cannot take this lattice");
                 if (!tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled / two-step kernels need N to be a multiple of 16 bytes of T");
@@ -531,6 +586,10 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
         case PRS_OPT_TILE_Y:
             if (value != 4 && value != 8 && value != 16) return fail(h, PRS_ERR_INVALID_ARG, "tile_y must be 4, 8 or 16");
             h->opt_tile_y = (int)value;
+            return PRS_OK;
+        case PRS_OPT_TBS_STEPS:
+            if (value != 3 && value != 4) return fail(h, PRS_ERR_INVALID_ARG, "tbs_steps must be 3 or 4");
+            h->opt_tbs_steps = (int)value;
             return PRS_OK;
         case PRS_OPT_TB2_TILE_Y:
             if (value != 4 && value != 8 && value != 12 && value != 28)

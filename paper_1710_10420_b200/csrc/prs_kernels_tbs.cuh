@@ -1,0 +1,199 @@
+// prs_kernels_tbs.cuh -- the 3D temporally blocked kernel generalised to S PRS steps per pass over
+// HBM (S = 3, 4): PAPER.md Eqs. 3-5 applied S times with the S consecutive sets of Eq. 6 scalars.
+// The compulsory traffic per site-update falls to 16/S B (FP32) / 32/S B (FP64); every site still
+// sees exactly the operations of S single steps, so the result is bit-identical to them.
+//
+// Why: the two-step kernel (prs_kernels_tb2.cuh) ended up HBM-bound at 8 B per site-update with the
+// issue slots a third busy (profiles/r01b_*); the only way further is fewer bytes per update.
+//
+// Scheme (same machinery as the two-step kernel, S pipeline stages instead of two).  A CTA owns TY
+// rows x XOUT vectors of output and marches a chunk of z planes; it is 32 lanes wide and TY+2S warps
+// tall.  Plane index a = 0, 1, ... stands for z = z0-S+a (periodic).  In iteration j, stage s
+// (0 <= s < S, active once j >= 2s) advances plane a = j+1-s from time level n+s to n+s+1:
+//   - its z-1 and z planes are a two-deep register window of its input field (own column);
+//   - its z+1 plane is what stage s-1 has just produced in this iteration (stage 0: the cp.async ring);
+//   - its y+-1 rows come from the plane stage s-1 published to shared memory one iteration earlier
+//     (stage 0: from the ring), its x+-1 sites from warp shuffles;
+//   - its phidot input is what stage s-1 produced for that plane one iteration earlier (a register;
+//     stage 0: the phidot ring);
+//   - it publishes its phi output for the y neighbours of stage s+1; the last stage stores to HBM.
+// A row that is r rows from the tile edge runs min(r, S) stages (row 0 only loads); each kind of row
+// has its own copy of the march, so the loop body tests nothing.  One CTA barrier per iteration.
+// Each stage loses one site of validity per side: S sites = ceil(S/W) halo lanes per side in x and S
+// halo rows per side in y.
+#pragma once
+
+#include <type_traits>
+
+#include "prs_arith.cuh"
+#include "prs_pack.cuh"
+#include "prs_kernels_tb2.cuh"      // cp_async16 / commit / wait, wrap_mod
+
+namespace prs {
+
+template <int I, int E, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (I < E) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, E>(f);
+    }
+}
+
+template <typename T, int S>
+struct StepCoefs {
+    StepCoef<T> k[S];
+};
+
+template <typename T, int S> __host__ __device__ constexpr int tbs_xhalo() { return (S + Pk<T>::W - 1) / Pk<T>::W; }
+template <typename T, int S> __host__ __device__ constexpr int tbs_xout() { return 32 - 2 * tbs_xhalo<T, S>(); }
+template <typename T, int S, int TY>
+constexpr size_t tbs_smem_bytes() {
+    return (size_t)(4 + 4 + 2 * (S - 1)) * (TY + 2 * S) * 32 * 16;
+}
+
+template <typename T, int ARITH, int S, int TY>
+__global__ void __launch_bounds__(32 * (TY + 2 * S), 1)
+step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
+                  T* __restrict__ phidot_out, int N, int ZC, StepCoefs<T, S> coefs) {
+    using K = Pk<T>;
+    using V = typename K::V;
+    using std::integral_constant;
+    constexpr int W = K::W;
+    constexpr int XH = tbs_xhalo<T, S>(), XOUT = tbs_xout<T, S>();
+    constexpr int ROWS = TY + 2 * S;
+    constexpr int PLANE = ROWS * 32;                                 // vectors per shared plane
+    extern __shared__ __align__(16) unsigned char tbs_smem[];
+    const int lane = threadIdx.x, row = threadIdx.y;
+    const int me = row * 32 + lane;
+    V* const sA = reinterpret_cast<V*>(tbs_smem) + me;               // ring A [4][PLANE], this thread's slot
+    V* const sP = sA + 4 * PLANE;                                    // ring P [4][PLANE]
+    V* const sB = sP + 4 * PLANE;                                    // published planes [S-1][2][PLANE]
+
+    const int NQ = N / W;
+    const int qraw = XOUT * (int)blockIdx.x - XH + lane;
+    const int q = wrap_mod(qraw, NQ);
+    const int yraw = TY * (int)blockIdx.y - S + row;
+    const int y = wrap_mod(yraw, N);
+    const int z0 = (int)blockIdx.z * ZC;
+    const int zend = min(z0 + ZC, N);
+    const int niter = (zend - z0) + 2 * S - 2;                       // >= 2S-1
+    const bool store_ok = (yraw < N) && (lane >= XH) && (lane < 32 - XH) && (qraw < NQ);
+
+    PackCoef<T> pc[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) pc[s].template set<3>(coefs.k[s]);
+
+    // 32-bit indices of 16-byte vectors (the host checks N^3 / W < 2^30).
+    const V* const gA = reinterpret_cast<const V*>(phi);
+    const V* const gP = reinterpret_cast<const V*>(phidot);
+    V* const oA = reinterpret_cast<V*>(phi_out);
+    V* const oP = reinterpret_cast<V*>(phidot_out);
+    const int NNv = N * NQ;                                          // vectors per plane
+    const int colv = y * NQ + q;                                     // this thread's column within a plane
+    int zl = wrap_mod(z0 - S, N);
+    int il = zl * NNv + colv;                                        // load cursor: issue i = plane a = i
+    int left_to_wrap = N - zl;                                       // issues until z wraps to 0
+    int io = z0 * NNv + colv;                                        // store cursor
+
+    auto march = [&](auto ns_tag) {
+        constexpr int NS = decltype(ns_tag)::value;                  // stages this row runs
+        int ni = 0;
+        auto issue = [&](int slot_a, int slot_p) {
+            if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
+            if (NS >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
+            ++ni; il += NNv;
+            if (--left_to_wrap == 0) { il -= N * NNv; left_to_wrap = N; }
+        };
+        // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
+        issue(0, 3); issue(1, 0); issue(2, 1);
+        cp_async_commit();
+        issue(3, 2);
+        cp_async_commit();
+        cp_async_wait<1>();
+        // register windows: wprev[s], wcur[s] = input field of stage s at planes a_s-1, a_s (own column);
+        // qcur[s] = phidot input of stage s at plane a_s (s >= 1)
+        V wprev[S], wcur[S], qcur[S];
+#pragma unroll
+        for (int s = 0; s < S; ++s) { wprev[s] = V{}; wcur[s] = V{}; qcur[s] = V{}; }
+        wprev[0] = sA[0 * PLANE];
+        wcur[0] = sA[1 * PLANE];
+
+        // One iteration.  U = j mod 4 (ring slots) and PAR = j mod 2 (published plane) are compile-time
+        // constants; ACTRAW = number of stages that have started (j/2 + 1, capped at S).
+        auto iteration = [&](auto u_tag, auto act_tag) {
+            constexpr int U = decltype(u_tag)::value, PAR = U & 1;
+            constexpr int ACTRAW = decltype(act_tag)::value;
+            constexpr int ACT = (NS > ACTRAW) ? ACTRAW : NS;
+            cp_async_wait<1>();                 // group j has landed for this thread
+            __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
+            issue(U, (U + 3) & 3);              // issue j+4: phi^n plane j+4 takes the slot of plane j
+            cp_async_commit();
+            if constexpr (NS >= 1) {
+                V carry, qout[S];
+                {   // stage 0 on plane a = j+1
+                    const V zp = sA[((U + 2) & 3) * PLANE];
+                    const V ym = sA[((U + 1) & 3) * PLANE - 32], yp = sA[((U + 1) & 3) * PLANE + 32];
+                    const V pd = sP[U * PLANE];
+                    const T left = __shfl_up_sync(0xffffffffu, K::last(wcur[0]), 1);
+                    const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[0]), 1);
+                    V out;
+                    packed_vector_update<T, 3, ARITH>(pc[0], wcur[0], left, right, ym, yp, wprev[0], zp, pd, out, qout[0]);
+                    if (S > 1) sB[(0 * 2 + PAR) * PLANE] = out;
+                    wprev[0] = wcur[0]; wcur[0] = zp; carry = out;
+                }
+                static_for<1, ACT>([&](auto s_tag) {                 // stage s on plane a = j+1-s
+                    constexpr int s = decltype(s_tag)::value;
+                    const V* Bs = sB + ((s - 1) * 2 + (PAR ^ 1)) * PLANE;      // published one iteration ago
+                    const V ym = Bs[-32], yp = Bs[32];
+                    const T left = __shfl_up_sync(0xffffffffu, K::last(wcur[s]), 1);
+                    const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[s]), 1);
+                    V out;
+                    packed_vector_update<T, 3, ARITH>(pc[s], wcur[s], left, right, ym, yp, wprev[s], carry, qcur[s], out, qout[s]);
+                    if constexpr (s < S - 1) {
+                        sB[(s * 2 + PAR) * PLANE] = out;
+                    } else {
+                        if (store_ok) {
+                            oP[io] = qout[s];
+                            oA[io] = out;
+                        }
+                        io += NNv;
+                    }
+                    wprev[s] = wcur[s]; wcur[s] = carry; carry = out;
+                });
+                if constexpr (ACT < NS) {       // feed the window of the stage that has not started yet
+                    wprev[ACT] = wcur[ACT]; wcur[ACT] = carry;
+                }
+                static_for<1, (ACT < NS ? ACT + 1 : NS)>([&](auto s_tag) {
+                    constexpr int s = decltype(s_tag)::value;
+                    qcur[s] = qout[s - 1];
+                });
+            }
+        };
+        // start-up: iterations 0 .. 2S-3, stage s joins at j = 2s
+        static_for<0, 2 * S - 2>([&](auto j_tag) {
+            constexpr int j = decltype(j_tag)::value;
+            iteration(integral_constant<int, j & 3>{}, integral_constant<int, j / 2 + 1>{});
+        });
+        // steady state from j = 2S-2, unrolled four times
+        constexpr int J0 = 2 * S - 2;
+        for (int j = J0; j < niter; j += 4) {
+            iteration(integral_constant<int, (J0 + 0) & 3>{}, integral_constant<int, S>{});
+            if (j + 1 >= niter) break;
+            iteration(integral_constant<int, (J0 + 1) & 3>{}, integral_constant<int, S>{});
+            if (j + 2 >= niter) break;
+            iteration(integral_constant<int, (J0 + 2) & 3>{}, integral_constant<int, S>{});
+            if (j + 3 >= niter) break;
+            iteration(integral_constant<int, (J0 + 3) & 3>{}, integral_constant<int, S>{});
+        }
+        cp_async_wait<0>();
+    };
+    // rows r from the tile edge run min(r, S) stages
+    const int edge = min(row, ROWS - 1 - row);
+    static_for<0, S>([&](auto r_tag) {
+        constexpr int r = decltype(r_tag)::value;
+        if (edge == r) march(integral_constant<int, r>{});
+    });
+    if (edge >= S) march(integral_constant<int, S>{});
+}
+
+}  // namespace prs
