@@ -206,7 +206,8 @@ def run_gpu(args):
     bpu = BYTES_PER_SITE_UPDATE[prec]
     sim = prs.Simulation(dims, N, prec, era_m=era_m, seed=rank + 1)
     if args.kernel:
-        sim.set_step_kernel({"generic": prs.KERNEL_GENERIC, "tiled": prs.KERNEL_TILED, "tb2": prs.KERNEL_TB2}[args.kernel])
+        sim.set_step_kernel({"generic": prs.KERNEL_GENERIC, "tiled": prs.KERNEL_TILED, "tb2": prs.KERNEL_TB2,
+                             "tbs": prs.KERNEL_TBS}[args.kernel])
     sim.init(1.0)
     stream = torch.cuda.current_stream()
 
@@ -249,11 +250,13 @@ def run_gpu(args):
     value = updates / (ms_total * 1e-3)
     step_kernel_launches = SUBSTEPS * args.steps
     step_kernel = sim.get_info(binding.INFO_STEP_KERNEL)
-    steps_per_launch = 2 if step_kernel == prs.KERNEL_TB2 else 1
+    # PRS steps the dominant kernel advances per launch; a prs_step(50) of the four-step kernel is 12
+    # four-step launches and one two-step launch, so launch_ms is the time per steps_per_launch steps
+    steps_per_launch = {prs.KERNEL_TB2: 2, prs.KERNEL_TBS: 4}.get(step_kernel, 1)
     launch_ms = ms_kernels / (step_kernel_launches / steps_per_launch)
     achieved = S * steps_per_launch * bpu / (launch_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak_gbs()
-    kernel_name = {1: "generic", 2: "tiled", 3: "tb2"}.get(step_kernel, str(step_kernel))
+    kernel_name = {1: "generic", 2: "tiled", 3: "tb2", 4: "tbs"}.get(step_kernel, str(step_kernel))
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
     e2e = None
@@ -336,7 +339,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default=DEFAULT_CONFIG, choices=sorted(CONFIGS))
-    ap.add_argument("--kernel", default=None, choices=["generic", "tiled", "tb2"])
+    ap.add_argument("--kernel", default=None, choices=["generic", "tiled", "tb2", "tbs"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

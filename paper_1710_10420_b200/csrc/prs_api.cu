@@ -135,11 +135,12 @@ bool tb2_supported(const prs_ctx* h) {
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
     if (want == PRS_KERNEL_AUTO) {
-        // Measured on B200 (profiles/): the two-step kernel wins once the lattice fills the chip
-        // (4096^2, 512^3 and up); below that a launch is latency-bound and the shorter single-step
-        // march is quicker.
+        // Measured on B200 (profiles/): the temporally blocked kernels (four steps per pass in 3D, two
+        // in 2D) win once the lattice fills the chip (4096^2, 512^3 and up); below that a launch is
+        // latency-bound and the shorter single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        else want = (h->S >= ((size_t)1 << 22) && tb2_supported(h)) ? PRS_KERNEL_TB2 : PRS_KERNEL_TILED;
+        else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = (h->dims == 3) ? PRS_KERNEL_TBS : PRS_KERNEL_TB2;
+        else want = PRS_KERNEL_TILED;
     }
     return want;
 }
@@ -281,7 +282,9 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     }
     constexpr int XOUT = tbs_xout<T, S>();
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
-    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
+    // Chunks of 128 planes: each chunk re-reads 2S halo planes (measured 1024^3 FP32, S = 4: 64 planes
+    // 1.25 ms/step, 128 planes 1.21, 256 planes 1.24 as the grid gets too coarse for 148 SMs).
+    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(128, N);
     const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
     const dim3 block(32, TY + 2 * S, 1);
     step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks);

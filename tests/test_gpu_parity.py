@@ -21,7 +21,7 @@ from tests import fieldgen as fg  # noqa: E402
 NP = {prs.F32: np.float32, prs.F64: np.float64}
 TOL = {prs.F32: 2e-5, prs.F64: 1e-12}
 THREADS = max(1, min(32, len(os.sched_getaffinity(0))))
-KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED, prs.KERNEL_TB2]
+KERNELS = [prs.KERNEL_GENERIC, prs.KERNEL_TILED, prs.KERNEL_TB2, prs.KERNEL_TBS]
 
 
 def make_pair(dims, N, prec, arith_gpu=prs.ARITH_FMA, arith_ref=ref.ARITH_LITERAL, kernel=prs.KERNEL_AUTO, **kw):
@@ -62,6 +62,8 @@ CASES_3D = [4, 20, 36, 64, 132]
 @pytest.mark.parametrize("dims,N", [(2, n) for n in CASES_2D] + [(3, n) for n in CASES_3D])
 @pytest.mark.parametrize("era_m", [1.0, 2.0])
 def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
+    if kernel == prs.KERNEL_TBS and dims == 2:
+        pytest.skip("the multi-step kernel is 3D only")
     # (a) tolerance bar against the paper's literal form, GPU in its default (FMA) form
     g, r = make_pair(dims, N, prec, kernel=kernel, era_m=era_m, seed=3)
     g.init(1.0)
@@ -107,9 +109,14 @@ def test_sizes_only_the_generic_kernel_takes(prec, dims, N):
 def test_tiling_parameters_do_not_change_a_bit(prec, dims, N, chunk, tile_y, tb2_tile_y):
     phi, pd = fg.random_state(dims, N, 77, NP[prec])
     outs = []
-    for kernel, ch in ((prs.KERNEL_GENERIC, 0), (prs.KERNEL_TILED, chunk), (prs.KERNEL_TB2, chunk)):
+    kernels = [(prs.KERNEL_GENERIC, 0), (prs.KERNEL_TILED, chunk), (prs.KERNEL_TB2, chunk)]
+    if dims == 3:
+        kernels.append((prs.KERNEL_TBS, chunk))
+    for kernel, ch in kernels:
         g = prs.Simulation(dims, N, prec)
         g.set_step_kernel(kernel)
+        if kernel == prs.KERNEL_TBS:
+            g.set_option(binding.OPT_TBS_STEPS, 3 if chunk % 2 else 4)
         g.set_option(binding.OPT_CHUNK, ch)
         g.set_option(binding.OPT_TILE_Y, tile_y)
         g.set_option(binding.OPT_TB2_TILE_Y, tb2_tile_y)
@@ -139,6 +146,31 @@ def test_two_step_kernel_equals_single_steps_bitwise(prec, dims, N, nsteps):
         want = nsteps if kernel == prs.KERNEL_TILED else nsteps // 2 + nsteps % 2
         assert g.kernel_launches == want
     assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("N", [4, 8, 20, 36, 60, 124, 200])
+@pytest.mark.parametrize("S", [3, 4])
+def test_multi_step_kernel_equals_single_steps_bitwise(prec, N, S):
+    phi, pd = fg.random_state(3, N, 5, NP[prec])
+    for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
+        for nsteps in (S, 2 * S + 1, 11):
+            outs = []
+            for kernel in (prs.KERNEL_TILED, prs.KERNEL_TBS):
+                g = prs.Simulation(3, N, prec, era_m=2.0)
+                g.set_step_kernel(kernel)
+                g.set_arith(arith)
+                g.set_option(binding.OPT_TBS_STEPS, S)
+                g.copy_in(phi, pd, eta0=1.0, step=3)
+                g.step(nsteps)
+                outs.append(g.copy_out())
+                assert g.get_info(binding.INFO_STEP) == 3 + nsteps
+                if kernel == prs.KERNEL_TBS:     # S-step launches, then a two-step launch, then a single step
+                    rest = nsteps % S
+                    assert g.kernel_launches == nsteps // S + rest // 2 + rest % 2
+            assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
+            if arith != prs.ARITH_FMA:
+                break                             # the other forms: one length is enough
 
 
 # ------------------------------------------------------------------ T3: diagnostics on snapshots
@@ -201,6 +233,8 @@ def test_diagnostics_of_special_fields(prec):
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("dims,N", [(2, 136), (3, 36)])
 def test_gpu_symmetries_are_bit_exact(kernel, prec, dims, N):
+    if kernel == prs.KERNEL_TBS and dims == 2:
+        pytest.skip("the multi-step kernel is 3D only")
     dt = NP[prec]
     phi, pd = fg.random_state(dims, N, 13, dt)
 
@@ -354,7 +388,7 @@ def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m):
     g = prs.Simulation(dims, N, prec, era_m=era_m, seed=2)
     g.init(1.0)
     g.step(20)
-    assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_TB2
+    assert g.get_info(binding.INFO_STEP_KERNEL) == (prs.KERNEL_TBS if dims == 3 else prs.KERNEL_TB2)
     dg = g.diagnostics()
     gp, gv = g.copy_out()
     g.close()
