@@ -56,6 +56,10 @@ BYTES_PER_SITE_UPDATE = {0: 16, 1: 32}        # read phi, phidot; write phidot, 
 # dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed
 # `ncu --set full` capture of the headline config (profiles/): filled in once measured.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
+    # profiles/r01c_ncu_step3d_tbs4_f32_1024.md: 9.485 GB read + 8.558 GB written per four-step launch
+    ("3d_1024_f32_rad", "tbs"): 18_043_506_000,
+    # profiles/r01c_ncu_step3d_tbs4_f64_1024.md: 20.726 GB read + 17.164 GB written per four-step launch
+    ("3d_1024_f64_rad", "tbs"): 37_889_208_000,
     # profiles/r01b_ncu_step3d_tb2_f32_1024.md: 9.136 GB read + 8.552 GB written per two-step launch
     ("3d_1024_f32_rad", "tb2"): 17_687_191_000,
     # profiles/r01b_ncu_step3d_tb2_f64_1024.md: 18.451 GB read + 17.144 GB written per two-step launch
