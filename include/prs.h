@@ -62,7 +62,7 @@ enum {
     PRS_OPT_CHUNK       = 4,   /* tuning: planes (3D) / rows (2D) one CTA marches; 0 = auto        */
     PRS_OPT_TILE_Y      = 5,   /* tuning: rows per CTA of the 3D tiled kernel, 4 / 8 / 16          */
     PRS_OPT_TB2_TILE_Y  = 6,   /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
-    PRS_OPT_TBS_STEPS   = 7    /* steps per pass of the 3D multi-step kernel, 3 or 4            default 4 */
+    PRS_OPT_TBS_STEPS   = 7    /* steps per pass of the multi-step kernel, 3 or 4               default 4 */
 };
 enum {
     PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */
@@ -70,7 +70,7 @@ enum {
     PRS_KERNEL_TILED   = 2,    /* shared-memory tiled, one step per pass over HBM                  */
     PRS_KERNEL_TB2     = 3,    /* temporally blocked: two steps per pass over HBM (same per-site   *
                                 * arithmetic, bit-identical to two single steps)                   */
-    PRS_KERNEL_TBS     = 4     /* 3D only: PRS_OPT_TBS_STEPS steps per pass over HBM, bit-identical *
+    PRS_KERNEL_TBS     = 4     /* PRS_OPT_TBS_STEPS steps per pass over HBM (2D and 3D), bit-identical *
                                 * to single steps; leftovers of a prs_step call go through TB2 and  *
                                 * TILED                                                             */
 };

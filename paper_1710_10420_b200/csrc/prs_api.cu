@@ -131,15 +131,19 @@ bool tb2_supported(const prs_ctx* h) {
     if (!tiled_supported(h)) return false;
     return h->dims == 2 || h->S / (size_t)vec_width(h->precision) < ((size_t)1 << 30);
 }
+// So do the multi-step kernels, in 2D as well.
+bool tbs_supported(const prs_ctx* h) {
+    return tiled_supported(h) && h->S / (size_t)vec_width(h->precision) < ((size_t)1 << 30);
+}
 
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
     if (want == PRS_KERNEL_AUTO) {
-        // Measured on B200 (profiles/): the temporally blocked kernels (four steps per pass in 3D, two
-        // in 2D) win once the lattice fills the chip (4096^2, 512^3 and up); below that a launch is
+        // Measured on B200 (profiles/): the temporally blocked kernels (four steps per pass) win once the lattice fills the chip (4096^2, 512^3 and up); below that a launch is
         // latency-bound and the shorter single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = (h->dims == 3) ? PRS_KERNEL_TBS : PRS_KERNEL_TB2;
+        else if (h->S >= ((size_t)1 << 22) && tbs_supported(h)) want = PRS_KERNEL_TBS;
+        else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = PRS_KERNEL_TB2;
         else want = PRS_KERNEL_TILED;
     }
     return want;
@@ -264,7 +268,7 @@ int step_twice(prs_ctx* h) {
     return PRS_OK;
 }
 
-// S steps in one pass (n -> n+S), 3D only; the caller guarantees tb2_supported(h).
+// S steps in one pass (n -> n+S); the caller guarantees tbs_supported(h).
 template <typename T, int ARITH, int S>
 cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     constexpr int TY = 16;
@@ -291,6 +295,30 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     return cudaGetLastError();
 }
 
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    StepCoefs<T, S> ks;
+    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
+    constexpr int XOUT = tbs_xout<T, S>();
+    const int BX = 128, warps = BX / 32;
+    const unsigned nwarps = (unsigned)((NQ + XOUT - 1) / XOUT);
+    const unsigned gx = (nwarps + warps - 1) / warps;
+    // Rows per march: long enough to amortise the 2S halo rows, short enough for >= ~8 CTAs per SM.
+    int YC;
+    if (h->opt_chunk > 0) YC = (int)std::min<int64_t>(h->opt_chunk, N);
+    else {
+        const long long want = 8LL * h->sm_count;
+        long long chunks = (want + gx - 1) / gx;
+        YC = (int)std::max<long long>(32, std::min<long long>(128, N / std::max<long long>(1, chunks)));
+        YC = std::min<int>(YC, N);
+    }
+    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
+    step2d_tbs_kernel<T, ARITH, S><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, ks);
+    return cudaGetLastError();
+}
+
 template <typename T>
 int step_many(prs_ctx* h, int S) {
     const T* p = (const T*)h->phi[h->cur];
@@ -298,7 +326,9 @@ int step_many(prs_ctx* h, int S) {
     T* pn = (T*)h->phi[h->cur ^ 1];
     T* vn = (T*)h->pd[h->cur ^ 1];
     cudaError_t e;
-#define PRS_TBS(AR) (S == 3 ? launch_tbs_3d<T, AR, 3>(h, p, v, pn, vn) : launch_tbs_3d<T, AR, 4>(h, p, v, pn, vn))
+#define PRS_TBS(AR)                                                                                                   \
+    (h->dims == 3 ? (S == 3 ? launch_tbs_3d<T, AR, 3>(h, p, v, pn, vn) : launch_tbs_3d<T, AR, 4>(h, p, v, pn, vn)) \
+                  : (S == 3 ? launch_tbs_2d<T, AR, 3>(h, p, v, pn, vn) : launch_tbs_2d<T, AR, 4>(h, p, v, pn, vn)))
     e = (h->opt_arith == PRS_ARITH_LITERAL) ? PRS_TBS(ARITH_LITERAL) : (h->opt_arith == PRS_ARITH_COEF) ? PRS_TBS(ARITH_COEF) : PRS_TBS(ARITH_FMA);
 #undef PRS_TBS
     if (e != cudaSuccess) return cuda_fail(h, e, "multi-step kernel launch");
@@ -559,7 +589,7 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
         case PRS_OPT_STEP_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
             if (value == PRS_KERNEL_TBS) {
-                if (h->dims != 3 || !tb2_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the multi-step kernel is 3D only and needs N a multiple of 16 bytes of T");
+                if (!tbs_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the multi-step kernel needs N a multiple of 16 bytes of T and N^d / that < 2^30");
                 h->opt_step_kernel = (int)value;
                 return PRS_OK;
             }

@@ -196,4 +196,103 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     if (edge >= S) march(integral_constant<int, S>{});
 }
 
+// ------------------------------------------------------------------------------------------------
+// 2D: S steps per pass with no shared memory at all.  A warp owns XOUT output vectors of x and
+// marches a chunk of rows; row index a = 0, 1, ... stands for y = y0-S+a (periodic).  Stage s at
+// iteration j advances row a = j+1-s: y-1 and y from its two-deep register window, y+1 from what
+// stage s-1 has just produced (stage 0: loaded two iterations ahead), x+-1 by warp shuffles, phidot
+// from what stage s-1 produced one iteration earlier (stage 0: loaded).  Block = 128 threads.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int ARITH, int S>
+__global__ void __launch_bounds__(128)
+step2d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
+                  T* __restrict__ phidot_out, int N, int YC, StepCoefs<T, S> coefs) {
+    using K = Pk<T>;
+    using V = typename K::V;
+    using std::integral_constant;
+    constexpr int W = K::W;
+    constexpr int XH = tbs_xhalo<T, S>(), XOUT = tbs_xout<T, S>();
+    const int lane = threadIdx.x & 31;
+    const int warp_global = (int)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int NQ = N / W;
+    if (warp_global * XOUT >= NQ) return;                           // whole warp beyond the row
+    const int qraw = XOUT * warp_global - XH + lane;
+    const int q = wrap_mod(qraw, NQ);
+    const int y0 = (int)blockIdx.y * YC;
+    const int yend = min(y0 + YC, N);
+    const int niter = (yend - y0) + 2 * S - 2;                      // >= 2S-1
+    const bool store_ok = (lane >= XH) && (lane < 32 - XH) && (qraw < NQ);
+    const V zero = {};
+
+    PackCoef<T> pc[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) pc[s].template set<2>(coefs.k[s]);
+
+    // 32-bit indices of 16-byte vectors (the host checks N^2 / W < 2^30); one load cursor for both fields
+    const V* const gA = reinterpret_cast<const V*>(phi);
+    const V* const gP = reinterpret_cast<const V*>(phidot);
+    V* const oA = reinterpret_cast<V*>(phi_out);
+    V* const oP = reinterpret_cast<V*>(phidot_out);
+    int yl = wrap_mod(y0 - S, N);
+    int il = yl * NQ + q;
+    int left_to_wrap = N - yl;
+    auto advance = [&]() {
+        il += NQ;
+        if (--left_to_wrap == 0) { il -= N * NQ; left_to_wrap = N; }
+    };
+    int io = y0 * NQ + q;
+
+    // rows a = 0, 1 into the window of stage 0; rows 2, 3 and phidot rows 1, 2 in flight
+    V wprev[S], wcur[S], qcur[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) { wprev[s] = zero; wcur[s] = zero; qcur[s] = zero; }
+    wprev[0] = __ldg(gA + il); advance();
+    wcur[0] = __ldg(gA + il);
+    V pd0 = __ldg(gP + il); advance();                               // phidot of row 1 (stage 0 at j = 0)
+    V a1 = __ldg(gA + il), pd1 = __ldg(gP + il); advance();          // row 2: y+1 of j = 0, phidot of j = 1
+    V a2 = __ldg(gA + il), pd2 = __ldg(gP + il); advance();          // row 3
+
+    auto iteration = [&](auto act_tag) {
+        constexpr int ACT = decltype(act_tag)::value;
+        // loads two iterations ahead: row a = j+4 (past the last needed row this re-reads harmlessly)
+        const V a3 = __ldg(gA + il), pd3 = __ldg(gP + il); advance();
+        V carry, qout[S];
+        {   // stage 0 on row a = j+1
+            const T left = __shfl_up_sync(0xffffffffu, K::last(wcur[0]), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[0]), 1);
+            V out;
+            packed_vector_update<T, 2, ARITH>(pc[0], wcur[0], left, right, wprev[0], a1, zero, zero, pd0, out, qout[0]);
+            wprev[0] = wcur[0]; wcur[0] = a1; carry = out;
+        }
+        static_for<1, ACT>([&](auto s_tag) {                         // stage s on row a = j+1-s
+            constexpr int s = decltype(s_tag)::value;
+            const T left = __shfl_up_sync(0xffffffffu, K::last(wcur[s]), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[s]), 1);
+            V out;
+            packed_vector_update<T, 2, ARITH>(pc[s], wcur[s], left, right, wprev[s], carry, zero, zero, qcur[s], out, qout[s]);
+            if constexpr (s == S - 1) {
+                if (store_ok) {
+                    oP[io] = qout[s];
+                    oA[io] = out;
+                }
+                io += NQ;
+            }
+            wprev[s] = wcur[s]; wcur[s] = carry; carry = out;
+        });
+        if constexpr (ACT < S) {                 // feed the window of the stage that has not started yet
+            wprev[ACT] = wcur[ACT]; wcur[ACT] = carry;
+        }
+        static_for<1, (ACT < S ? ACT + 1 : S)>([&](auto s_tag) {
+            constexpr int s = decltype(s_tag)::value;
+            qcur[s] = qout[s - 1];
+        });
+        a1 = a2; a2 = a3; pd0 = pd1; pd1 = pd2; pd2 = pd3;
+    };
+    static_for<0, 2 * S - 2>([&](auto j_tag) {
+        constexpr int j = decltype(j_tag)::value;
+        iteration(integral_constant<int, j / 2 + 1>{});
+    });
+    for (int j = 2 * S - 2; j < niter; ++j) iteration(integral_constant<int, S>{});
+}
+
 }  // namespace prs

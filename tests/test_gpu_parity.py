@@ -62,8 +62,6 @@ CASES_3D = [4, 20, 36, 64, 132]
 @pytest.mark.parametrize("dims,N", [(2, n) for n in CASES_2D] + [(3, n) for n in CASES_3D])
 @pytest.mark.parametrize("era_m", [1.0, 2.0])
 def test_20_steps_match_the_oracle(kernel, prec, dims, N, era_m):
-    if kernel == prs.KERNEL_TBS and dims == 2:
-        pytest.skip("the multi-step kernel is 3D only")
     # (a) tolerance bar against the paper's literal form, GPU in its default (FMA) form
     g, r = make_pair(dims, N, prec, kernel=kernel, era_m=era_m, seed=3)
     g.init(1.0)
@@ -110,8 +108,7 @@ def test_tiling_parameters_do_not_change_a_bit(prec, dims, N, chunk, tile_y, tb2
     phi, pd = fg.random_state(dims, N, 77, NP[prec])
     outs = []
     kernels = [(prs.KERNEL_GENERIC, 0), (prs.KERNEL_TILED, chunk), (prs.KERNEL_TB2, chunk)]
-    if dims == 3:
-        kernels.append((prs.KERNEL_TBS, chunk))
+    kernels.append((prs.KERNEL_TBS, chunk))
     for kernel, ch in kernels:
         g = prs.Simulation(dims, N, prec)
         g.set_step_kernel(kernel)
@@ -149,15 +146,16 @@ def test_two_step_kernel_equals_single_steps_bitwise(prec, dims, N, nsteps):
 
 
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
-@pytest.mark.parametrize("N", [4, 8, 20, 36, 60, 124, 200])
+@pytest.mark.parametrize("dims,N", [(3, 4), (3, 8), (3, 20), (3, 36), (3, 60), (3, 124), (3, 200),
+                                    (2, 4), (2, 8), (2, 36), (2, 120), (2, 124), (2, 260), (2, 1024)])
 @pytest.mark.parametrize("S", [3, 4])
-def test_multi_step_kernel_equals_single_steps_bitwise(prec, N, S):
-    phi, pd = fg.random_state(3, N, 5, NP[prec])
+def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
+    phi, pd = fg.random_state(dims, N, 5, NP[prec])
     for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
         for nsteps in (S, 2 * S + 1, 11):
             outs = []
             for kernel in (prs.KERNEL_TILED, prs.KERNEL_TBS):
-                g = prs.Simulation(3, N, prec, era_m=2.0)
+                g = prs.Simulation(dims, N, prec, era_m=2.0)
                 g.set_step_kernel(kernel)
                 g.set_arith(arith)
                 g.set_option(binding.OPT_TBS_STEPS, S)
@@ -233,8 +231,6 @@ def test_diagnostics_of_special_fields(prec):
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("dims,N", [(2, 136), (3, 36)])
 def test_gpu_symmetries_are_bit_exact(kernel, prec, dims, N):
-    if kernel == prs.KERNEL_TBS and dims == 2:
-        pytest.skip("the multi-step kernel is 3D only")
     dt = NP[prec]
     phi, pd = fg.random_state(dims, N, 13, dt)
 
@@ -388,7 +384,7 @@ def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m):
     g = prs.Simulation(dims, N, prec, era_m=era_m, seed=2)
     g.init(1.0)
     g.step(20)
-    assert g.get_info(binding.INFO_STEP_KERNEL) == (prs.KERNEL_TBS if dims == 3 else prs.KERNEL_TB2)
+    assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_TBS
     dg = g.diagnostics()
     gp, gv = g.copy_out()
     g.close()
