@@ -139,10 +139,11 @@ bool tbs_supported(const prs_ctx* h) {
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
     if (want == PRS_KERNEL_AUTO) {
-        // Measured on B200 (profiles/): the temporally blocked kernels (four steps per pass) win once the lattice fills the chip (4096^2, 512^3 and up); below that a launch is
-        // latency-bound and the shorter single-step march is quicker.
+        // Measured on B200 (profiles/): the four-step kernel wins from 64^2 and
+        // 128^3 up -- on small lattices because it needs a quarter of the launches, on large ones
+        // because it moves a quarter of the bytes; below that the single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        else if (h->S >= ((size_t)1 << 22) && tbs_supported(h)) want = PRS_KERNEL_TBS;
+        else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
         else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = PRS_KERNEL_TB2;
         else want = PRS_KERNEL_TILED;
     }
@@ -288,7 +289,14 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
     // Chunks of 128 planes: each chunk re-reads 2S halo planes (measured 1024^3 FP32, S = 4: 64 planes
     // 1.25 ms/step, 128 planes 1.21, 256 planes 1.24 as the grid gets too coarse for 148 SMs).
-    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(128, N);
+    // ... and short enough that the grid covers the chip twice (one CTA per SM) on small lattices.
+    int ZC;
+    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, N);
+    else {
+        const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
+        ZC = (int)std::max<long long>(16, std::min<long long>(128, N / chunks));
+        ZC = std::min<int>(ZC, N);
+    }
     const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
     const dim3 block(32, TY + 2 * S, 1);
     step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks);
@@ -305,13 +313,14 @@ cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const int BX = 128, warps = BX / 32;
     const unsigned nwarps = (unsigned)((NQ + XOUT - 1) / XOUT);
     const unsigned gx = (nwarps + warps - 1) / warps;
-    // Rows per march: long enough to amortise the 2S halo rows, short enough for >= ~8 CTAs per SM.
+    // Rows per march: long enough to amortise the 2S halo rows, short enough for ~4 CTAs per SM; on
+    // launch-bound lattices (256^2: 1.6 us per step with 8-row marches, 2.6 us with 32) short wins.
     int YC;
     if (h->opt_chunk > 0) YC = (int)std::min<int64_t>(h->opt_chunk, N);
     else {
-        const long long want = 8LL * h->sm_count;
+        const long long want = 4LL * h->sm_count;
         long long chunks = (want + gx - 1) / gx;
-        YC = (int)std::max<long long>(32, std::min<long long>(128, N / std::max<long long>(1, chunks)));
+        YC = (int)std::max<long long>(8, std::min<long long>(128, N / std::max<long long>(1, chunks)));
         YC = std::min<int>(YC, N);
     }
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);

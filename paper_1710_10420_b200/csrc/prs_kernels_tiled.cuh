@@ -229,17 +229,61 @@ __device__ __forceinline__ void mask_links(unsigned c, unsigned l, unsigned r, u
     wallmask = (fx | bx | fy | by | fz | bz) & ALL;
 }
 
+// Wall sites are a few per cent of the lattice once the network has formed, so evaluating Eq. 8's
+// FP64 ratio lane by lane under a predicate keeps 32 lanes busy for a handful of sites (ncu, r01b:
+// 78 instructions per site, FP64 pipe 30 %).  Instead each warp compacts its wall sites into a small
+// shared-memory stack (ballot + popcount give every site its slot) and pops 32 at a time, so the
+// ratio is evaluated with all lanes active.  The order of the additions is fixed by the launch
+// configuration and the data, hence reproducible.
+template <typename T> struct Pair;
+template <> struct Pair<float> { typedef float2 type; };
+template <> struct Pair<double> { typedef double2 type; };
+
+constexpr int WALLQ_CAP = 32 + 32 * 4;          // below 32 before a push, at most 4 sites per lane pushed
+
 template <typename T>
-__device__ __forceinline__ void accumulate_walls(unsigned wallmask, typename VecOps<T>::V c, typename VecOps<T>::V pd,
-                                                 double V0, double I, DiagPartial& acc) {
-    using O = VecOps<T>;
+struct WallQueue {
+    typename Pair<T>::type* q;                  // this warp's stack
+    int n;                                      // entries (warp-uniform)
+    unsigned lt;                                // lanes below this one
+    __device__ __forceinline__ void init(typename Pair<T>::type* base, int lane) {
+        q = base; n = 0; lt = (1u << lane) - 1u;
+    }
+    // every lane of the warp must call (wallmask may be 0)
+    __device__ __forceinline__ void push(unsigned wallmask, typename VecOps<T>::V c, typename VecOps<T>::V pd,
+                                         double V0, double I, DiagPartial& acc) {
+        using O = VecOps<T>;
+        if (__ballot_sync(0xffffffffu, wallmask != 0u) == 0u) return;
+        acc.walls += __popc(wallmask);
+        __syncwarp();                           // pops of the previous call are done before slots are reused
 #pragma unroll
-    for (int i = 0; i < O::W; ++i)
-        if (wallmask & (1u << i)) {
-            acc.walls += 1;
-            acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(O::get(c, i), O::get(pd, i), V0, I));
+        for (int i = 0; i < O::W; ++i) {
+            const bool bit = (wallmask >> i) & 1u;
+            const unsigned m = __ballot_sync(0xffffffffu, bit);
+            if (bit) {
+                typename Pair<T>::type e;
+                e.x = O::get(c, i); e.y = O::get(pd, i);
+                q[n + __popc(m & lt)] = e;
+            }
+            n += __popc(m);
         }
-}
+        __syncwarp();
+        while (n >= 32) {
+            n -= 32;
+            const typename Pair<T>::type e = q[n + (int)__popc(lt)];
+            acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(e.x, e.y, V0, I));
+        }
+    }
+    __device__ __forceinline__ void drain(double V0, double I, DiagPartial& acc) {
+        __syncwarp();
+        const int lane = (int)__popc(lt);
+        if (lane < n) {
+            const typename Pair<T>::type e = q[lane];
+            acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(e.x, e.y, V0, I));
+        }
+        n = 0;
+    }
+};
 
 template <typename T, int TYB>
 __global__ void __launch_bounds__(32 * TYB)
@@ -252,6 +296,9 @@ diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
     const int lane = threadIdx.x;
     const int y = blockIdx.y * TYB + threadIdx.y;
     const int xraw = (blockIdx.x * 32 + lane) * W;
+    __shared__ typename Pair<T>::type wallq[TYB][WALLQ_CAP];
+    WallQueue<T> wq;
+    wq.init(wallq[threadIdx.y], lane);
     if (y < N) {                                           // warp-uniform
         const bool live = xraw < N;
         const int x = live ? xraw : N - W;
@@ -299,12 +346,13 @@ diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
             acc.links += nlinks;
             V pd_now = cur;
             if (wallmask) pd_now = O::ld(phidot + (size_t)z * NN + rc);   // consumed next iteration
-            if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+            wq.push(d_mask, d_c, d_pd, V0, I, acc);
             d_mask = wallmask; d_c = cur; d_pd = pd_now;
             m_prev = m_cur; cur = nxt; nxt = nn;
             m_up = m_up_n; m_dn = m_dn_n; s_l = s_l_n; s_r = s_r_n;
         }
-        if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+        wq.push(d_mask, d_c, d_pd, V0, I, acc);
+        wq.drain(V0, I, acc);
     }
     acc = block_reduce(acc);
     if (threadIdx.x == 0 && threadIdx.y == 0)
@@ -321,6 +369,9 @@ diag2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
     DiagPartial acc = {0ull, 0ull, 0.0};
     const int lane = threadIdx.x & 31;
     const long long xraw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * W;
+    __shared__ typename Pair<T>::type wallq[4][WALLQ_CAP];
+    WallQueue<T> wq;
+    wq.init(wallq[threadIdx.x >> 5], lane);
     if (xraw - (long long)lane * W < N) {                  // warp-uniform
         const bool live = xraw < N;
         const int x = live ? (int)xraw : N - W;
@@ -358,12 +409,13 @@ diag2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
             acc.links += nlinks;
             V pd_now = cur;
             if (wallmask) pd_now = O::ld(phidot + (size_t)y * N + x);
-            if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+            wq.push(d_mask, d_c, d_pd, V0, I, acc);
             d_mask = wallmask; d_c = cur; d_pd = pd_now;
             m_prev = m_cur; cur = nxt; nxt = nn;
             s_l = s_l_n; s_r = s_r_n;
         }
-        if (d_mask) accumulate_walls<T>(d_mask, d_c, d_pd, V0, I, acc);
+        wq.push(d_mask, d_c, d_pd, V0, I, acc);
+        wq.drain(V0, I, acc);
     }
     acc = block_reduce(acc);
     if (threadIdx.x == 0) partials[blockIdx.x + (size_t)gridDim.x * blockIdx.y] = acc;
