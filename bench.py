@@ -154,6 +154,28 @@ def oracle_sample(dims, prec, era_m, nsteps, threads, N=None, seed=1, with_init=
     return N ** dims * nsteps, dt, desc
 
 
+def reduce_over_ranks(times_ms, counts, world, device="cpu"):
+    """Replica aggregation: a job is as slow as its slowest rank, so every time
+    is the MAX over ranks; counts (kernel launches) are SUMmed.  No data-path collective: these few
+    scalars are the only thing the ranks ever exchange.  Works on any backend (nccl on the GPUs,
+    gloo in the CPU test)."""
+    if world <= 1:
+        return [float(t) for t in times_ms], [int(c) for c in counts]
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(x) for x in times_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([int(x) for x in counts], device=device, dtype=torch.int64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t.tolist()], [int(x) for x in c.tolist()]
+
+
+def aggregate_value(sites, substeps, steps, world, ms_total):
+    """Whole-job site-updates per second of `world` replicas that each did steps x substeps PRS steps."""
+    return sites * substeps * steps * world / (ms_total * 1e-3)
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -243,15 +265,8 @@ def run_gpu(args):
     launches = sim.kernel_launches - l0
     ms_total = t0.elapsed_time(t1)
     ms_kernels = sum(a.elapsed_time(b) for a, b in kev)
-    if world > 1:
-        t = torch.tensor([ms_total, ms_kernels], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_kernels = float(t[0]), float(t[1])
-        lt = torch.tensor([launches], device="cuda", dtype=torch.int64)
-        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
-        launches = int(lt[0])
-    updates = S * SUBSTEPS * args.steps * world
-    value = updates / (ms_total * 1e-3)
+    (ms_total, ms_kernels), (launches,) = reduce_over_ranks([ms_total, ms_kernels], [launches], world, "cuda")
+    value = aggregate_value(S, SUBSTEPS, args.steps, world, ms_total)
     step_kernel_launches = SUBSTEPS * args.steps
     step_kernel = sim.get_info(binding.INFO_STEP_KERNEL)
     # PRS steps the dominant kernel advances per launch; a prs_step(50) of the four-step kernel is 12
@@ -289,11 +304,8 @@ def run_gpu(args):
         b.record(stream)
         barrier()
         ms_e2e = a.elapsed_time(b)
-        if world > 1:
-            t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t[0])
-        e2e = {"value": S * SUBSTEPS * n_e2e * world / (ms_e2e * 1e-3), "unit": UNIT,
+        (ms_e2e,), _ = reduce_over_ranks([ms_e2e], [], world, "cuda")
+        e2e = {"value": aggregate_value(S, SUBSTEPS, n_e2e, world, ms_e2e), "unit": UNIT,
                "h2d_bytes_per_step": 2 * fbytes, "d2h_bytes_per_step": 2 * fbytes + 24,
                "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e,
                "what": "prs_copy_in(pinned host) + %d prs_step + prs_diagnostics + prs_copy_out(pinned host)" % SUBSTEPS}

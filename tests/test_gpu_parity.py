@@ -310,6 +310,31 @@ def test_config0_256sq_full_run_curve():
     assert abs(mu_g - mu_32) <= 0.02 and abs(mu_g - mu_64) <= 0.02
 
 
+@pytest.mark.parametrize("dims,N,era_m,every,nsamp", [
+    (2, 1024, 2.0, 10, 127),      # 2D, matter era, eta 1 -> 128
+    (3, 128, 1.0, 10, 63),        # 3D, radiation era, eta 1 -> 64 (the paper's own 3D box size)
+    (3, 128, 2.0, 10, 63),        # 3D, matter era
+])
+def test_long_run_curves_match_the_oracle(dims, N, era_m, every, nsamp):
+    """T5 at sizes the oracle runs in seconds: the whole run (default kernels and arithmetic) against
+    the oracle's literal FP32 form: rho(eta) within 2 % at every sample, fitted exponent within 0.02."""
+    g = prs.Simulation(dims, N, prs.F32, era_m=era_m, seed=3)
+    r = ref.RefSim(dims, N, ref.F32, era_m=era_m, seed=3, threads=THREADS)
+    g.init(1.0)
+    r.init(1.0)
+    eta, cg, cr = [], [], []
+    for _ in range(nsamp):
+        g.step(every)
+        r.step(every)
+        dg, dr = g.diagnostics(), r.diagnostics()
+        assert dg["eta"] == dr["eta"] and dg["step"] == dr["step"]
+        eta.append(dg["eta"]); cg.append(dg["rho"]); cr.append(dr["rho"])
+    eta, cg, cr = map(np.array, (eta, cg, cr))
+    assert np.max(np.abs(cg - cr) / cr) <= 0.02
+    assert abs(fit_mu(eta, cg, 13.2) - fit_mu(eta, cr, 13.2)) <= 0.02
+    assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_TBS
+
+
 # ------------------------------------------------------------------ state handling
 
 def test_copy_in_out_roundtrip_device_and_host_and_step_split():
