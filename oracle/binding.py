@@ -48,6 +48,7 @@ def lib():
         L.prs_ref_step_sites.argtypes = [ci, i64, ci, ci, dbl, dbl, dbl, dbl, dbl, dbl, i64,
                                          vp, vp, vp, i64, vp, vp]
         L.prs_ref_scalars.argtypes = [dbl, dbl, dbl, dbl, dbl, dbl, i64, C.POINTER(dbl)]
+        L.prs_ref_weighted_area_of.argtypes = [ci, i64, ci, vp, C.POINTER(dbl)]
         _lib = L
     return _lib
 
@@ -128,6 +129,16 @@ def diagnostics_of(phi, phidot, W0=10.0, phi0=1.0):
     _chk(lib().prs_ref_diagnostics_of(phi.ndim, phi.shape[0], prec, _ptr(phi), _ptr(phidot), W0, phi0,
                                       C.byref(d)), "prs_ref_diagnostics_of")
     return d.as_dict()
+
+
+def weighted_area_of(phi):
+    """Eq. 7 as printed: sum over crossing links of |grad phi| / sum |grad phi components| (double)."""
+    phi = np.ascontiguousarray(phi)
+    assert phi.dtype in (np.float32, np.float64)
+    prec = F32 if phi.dtype == np.float32 else F64
+    out = C.c_double()
+    _chk(lib().prs_ref_weighted_area_of(phi.ndim, phi.shape[0], prec, _ptr(phi), C.byref(out)), "prs_ref_weighted_area_of")
+    return float(out.value)
 
 
 def step_sites(phi, phidot, sites, n, eta0=1.0, arith=ARITH_LITERAL, alpha=3.0, era_m=1.0, deta=0.1,

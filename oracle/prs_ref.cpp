@@ -220,6 +220,56 @@ void diagnostics_of(int dims, int64_t N, const T* phi, const T* phidot, double W
     out->gv2 = walls ? sum / (2.0 * (double)walls) : 0.0;
 }
 
+/* ---------------------------------------------------------------- orientation-weighted area (Eq. 7) */
+
+/* PAPER.md Eq. 7 (:59-62) as printed: A/V = (Delta A / V) * sum over links of delta_pm *
+ * |grad phi| / (|phi,x| + |phi,y| + |phi,z|) -- the PRS weight that corrects plain link counting for the
+ * orientation of the wall (1 for a wall normal to an axis, 1/sqrt(d) for a fully diagonal one).
+ * The paper does not say where on a link the gradient is taken (R15); the reading here, for
+ * the link from s to s+e_k: along the link the forward difference phi(s+e_k) - phi(s); across it, for
+ * each other axis t, the mean of the central differences (phi(u+e_t) - phi(u-e_t))/2 at the two end
+ * points u = s, s+e_k.  Everything in double; weight := 1 if all components vanish.  The sum runs over
+ * sites in index order, axes x, y, z within a site, with Kahan compensation. */
+template <typename T>
+double weighted_area_of(int dims, int64_t N, const T* phi) {
+    const int64_t Nz = (dims == 3) ? N : 1;
+    const int64_t stride[3] = {1, N, N * N};
+    double sum = 0.0, comp = 0.0;
+    for (int64_t z = 0; z < Nz; ++z)
+        for (int64_t y = 0; y < N; ++y)
+            for (int64_t x = 0; x < N; ++x) {
+                const int64_t c[3] = {x, y, z};
+                auto at = [&](const int64_t q[3]) {
+                    return (double)phi[wrap(q[0], N) * stride[0] + wrap(q[1], N) * stride[1] +
+                                       (dims == 3 ? wrap(q[2], N) * stride[2] : 0)];
+                };
+                for (int k = 0; k < dims; ++k) {
+                    int64_t e[3] = {c[0], c[1], c[2]};               /* other end of the forward link */
+                    e[k] += 1;
+                    if (neg((T)at(c)) == neg((T)at(e))) continue;    /* delta_pm = 0 */
+                    double g[3] = {0.0, 0.0, 0.0};
+                    g[k] = at(e) - at(c);
+                    for (int t = 0; t < dims; ++t) {
+                        if (t == k) continue;
+                        int64_t cp[3] = {c[0], c[1], c[2]}, cm[3] = {c[0], c[1], c[2]};
+                        int64_t ep[3] = {e[0], e[1], e[2]}, em[3] = {e[0], e[1], e[2]};
+                        cp[t] += 1; cm[t] -= 1; ep[t] += 1; em[t] -= 1;
+                        const double dc = (at(cp) - at(cm)) / 2.0;   /* central difference at s       */
+                        const double de = (at(ep) - at(em)) / 2.0;   /* central difference at s + e_k */
+                        g[t] = (dc + de) / 2.0;
+                    }
+                    const double num = std::sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
+                    const double den = std::fabs(g[0]) + std::fabs(g[1]) + std::fabs(g[2]);
+                    const double w = (den == 0.0) ? 1.0 : num / den;
+                    const double yk = w - comp;
+                    const double tk = sum + yk;
+                    comp = (tk - sum) - yk;
+                    sum = tk;
+                }
+            }
+    return sum;
+}
+
 }  // namespace
 
 /* ---------------------------------------------------------------- context */
@@ -402,6 +452,14 @@ int prs_ref_diagnostics_of(int dims, int64_t N, int precision, const void* phi, 
     d.step = 0;
     d.eta = 0.0;
     *out = d;
+    return 0;
+}
+
+int prs_ref_weighted_area_of(int dims, int64_t N, int precision, const void* phi, double* area) {
+    if ((dims != 2 && dims != 3) || N < 1 || !phi || !area) return 1;
+    if (precision == PRS_REF_F32) *area = weighted_area_of<float>(dims, N, (const float*)phi);
+    else if (precision == PRS_REF_F64) *area = weighted_area_of<double>(dims, N, (const double*)phi);
+    else return 1;
     return 0;
 }
 

@@ -71,6 +71,11 @@ double prs_ref_init_value(uint64_t seed, uint64_t s, double phi0);
 int prs_ref_diagnostics_of(int dims, int64_t N, int precision, const void* phi, const void* phidot,
                            double W0, double phi0, prs_ref_diag* out);
 
+/* Orientation-weighted wall area of a caller-held snapshot: PAPER.md Eq. 7 as printed, sum over crossing
+ * links of |grad phi| / (|phi,x| + |phi,y| + |phi,z|); gradient on a link as in DESIGN.md R15.
+ * rho_weighted = *area / N^dims. */
+int prs_ref_weighted_area_of(int dims, int64_t N, int precision, const void* phi, double* area);
+
 /* One PRS step (Eqs. 3-6) evaluated ONLY at the listed sites of a caller-held state at step n
  * (time eta0 + n*deta).  phi/phidot are full fields T[N^dims]; outputs are T[nsites]. */
 int prs_ref_step_sites(int dims, int64_t N, int precision, int arith,
