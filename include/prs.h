@@ -117,6 +117,13 @@ int prs_step(prs_handle h, int64_t nsteps);
 /* Measures Eqs. 7-8 on the current state; synchronises the stream; fills *out (HOST pointer). */
 int prs_diagnostics(prs_handle h, prs_diag* out);
 
+/* Orientation-weighted wall area of the current phi^n: PAPER.md Eq. 7 as printed (:59-62), the sum over
+ * crossing forward links of |grad phi| / (|phi,x| + |phi,y| + |phi,z|) with the gradient on a link taken as
+ * in DESIGN.md R15 (forward difference along the link, mean of the two end-point central differences
+ * across it), in double.  *area = that sum (between link_count/sqrt(dims) and link_count),
+ * *rho_weighted = *area / N^dims; either pointer may be NULL (HOST pointers).  Synchronises the stream. */
+int prs_weighted_area(prs_handle h, double* area, double* rho_weighted);
+
 /* Snapshot: copies phi^n and/or phidot^{n-1/2} (T[N^dims]) to HOST or DEVICE memory (either pointer
  * may be NULL); synchronises the stream. */
 int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst);

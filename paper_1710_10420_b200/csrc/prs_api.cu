@@ -563,6 +563,42 @@ int prs_diagnostics(prs_handle h, prs_diag* out) {
     return PRS_OK;
 }
 
+int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!area && !rho_weighted) return fail(h, PRS_ERR_INVALID_ARG, "prs_weighted_area: both outputs are NULL");
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_weighted_area: call prs_init or prs_copy_in first");
+    if (h->N > (1 << 30)) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: N too large");
+    // x across the threads, y (3D) across blockIdx.y, the slowest axis marched in chunks of L sites,
+    // L as short as the partials scratch allows (one partial per block).
+    const int N = (int)h->N;
+    const unsigned gx = (unsigned)((N + 255) / 256);
+    const long long per_chunk = (long long)gx * (h->dims == 3 ? N : 1);
+    long long chunks = std::max<long long>(1, std::min<long long>(N, MAX_PARTIALS / per_chunk));
+    int L = (int)((N + chunks - 1) / chunks);
+    if (L < 8) L = std::min(8, N);
+    const unsigned nch = (unsigned)((N + L - 1) / L);
+    const dim3 grid = (h->dims == 3) ? dim3(gx, (unsigned)N, nch) : dim3(gx, nch, 1);
+    const long long blocks = (long long)grid.x * grid.y * grid.z;
+    if (blocks > MAX_PARTIALS) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: lattice too large for the reduction scratch");
+    const void* p = h->phi[h->cur];
+    if (h->precision == PRS_F32) {
+        if (h->dims == 3) weighted_area_kernel<float, 3><<<grid, 256, 0, h->stream>>>((const float*)p, N, L, h->partials);
+        else weighted_area_kernel<float, 2><<<grid, 256, 0, h->stream>>>((const float*)p, N, L, h->partials);
+    } else {
+        if (h->dims == 3) weighted_area_kernel<double, 3><<<grid, 256, 0, h->stream>>>((const double*)p, N, L, h->partials);
+        else weighted_area_kernel<double, 2><<<grid, 256, 0, h->stream>>>((const double*)p, N, L, h->partials);
+    }
+    PRS_CUDA(h, cudaGetLastError());
+    diag_finalize_kernel<<<1, 1024, 0, h->stream>>>(h->partials, (int)blocks, h->d_result);
+    PRS_CUDA(h, cudaGetLastError());
+    h->launches += 2;
+    PRS_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, h->stream));
+    PRS_CUDA(h, cudaStreamSynchronize(h->stream));
+    if (area) *area = h->h_result->sum;
+    if (rho_weighted) *rho_weighted = h->h_result->sum / (double)h->S;
+    return PRS_OK;
+}
+
 int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst) {
     if (!h) return PRS_ERR_INVALID_ARG;
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_copy_out: no state yet");

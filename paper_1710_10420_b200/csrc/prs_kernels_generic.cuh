@@ -163,6 +163,74 @@ diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, lon
     if (threadIdx.x == 0) partials[blockIdx.x] = acc;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Orientation-weighted wall area, Eq. 7 as printed (:59-62; R15): sum over crossing
+// forward links of |grad phi| / (|phi,x| + |phi,y| + |phi,z|), the gradient on the link s -> s+e_k
+// being the forward difference along the link and, across it, the mean of the central differences
+// at the two ends.  Grid-stride over sites; a thread owns the d forward links of its site, tests them
+// on the sign bits and gathers the transverse neighbours (L1 / L2 hits: they lie within one site of
+// what the warp streams anyway) only for links that cross.  (Sums in x, y, z order per site;  All arithmetic in double.  The crossing
+// links are counted again on the way (partials[].links) as a cross-check against the link count.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int DIMS>
+__global__ void __launch_bounds__(256)
+weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __restrict__ partials) {
+    using A = Ar<T>;
+    DiagPartial acc = {0ull, 0ull, 0.0};
+    // Thread = one x; blockIdx.y = y (3D) or the chunk of rows (2D); blockIdx.z = the chunk of planes
+    // (3D).  The thread marches L sites along the slowest axis, carrying the value one step ahead.
+    constexpr int M = DIMS - 1;                                      // march axis
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride[3] = {1, N, (long long)N * N};
+    if (x < N) {
+        int c[3] = {x, (DIMS == 3) ? (int)blockIdx.y : 0, 0};
+        const int m0 = (int)((DIMS == 3) ? blockIdx.z : blockIdx.y) * L;
+        const int m1 = min(m0 + L, N);
+        // value at the site displaced by a along axis i and by b along axis j (periodic)
+        auto at2 = [&](int i, int a, int j, int b) {
+            int q[3] = {c[0], c[1], c[2]};
+            q[i] += a; q[j] += b;
+            long long o = 0;
+#pragma unroll
+            for (int m = 0; m < DIMS; ++m) {
+                const int w = (q[m] < 0) ? q[m] + N : (q[m] >= N ? q[m] - N : q[m]);
+                o += w * stride[m];
+            }
+            return __ldg(phi + o);
+        };
+        c[M] = m0;
+        T pc = at2(0, 0, 0, 0);
+        for (int m = m0; m < m1; ++m) {
+            c[M] = m;
+            T pe[DIMS];
+#pragma unroll
+            for (int k = 0; k < DIMS; ++k) pe[k] = at2(k, 1, k, 0);   // forward neighbours
+            const bool me = A::neg(pc);
+#pragma unroll
+            for (int k = 0; k < DIMS; ++k) {
+                if (A::neg(pe[k]) == me) continue;
+                acc.links += 1;
+                double g[3] = {0.0, 0.0, 0.0};
+                g[k] = __dsub_rn((double)pe[k], (double)pc);
+#pragma unroll
+                for (int t = 0; t < DIMS; ++t) {
+                    if (t == k) continue;
+                    const double dc = __dmul_rn(__dsub_rn((double)at2(t, 1, k, 0), (double)at2(t, -1, k, 0)), 0.5);
+                    const double de = __dmul_rn(__dsub_rn((double)at2(t, 1, k, 1), (double)at2(t, -1, k, 1)), 0.5);
+                    g[t] = __dmul_rn(__dadd_rn(dc, de), 0.5);
+                }
+                const double num = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(g[0], g[0]), __dmul_rn(g[1], g[1])), __dmul_rn(g[2], g[2])));
+                const double den = __dadd_rn(__dadd_rn(fabs(g[0]), fabs(g[1])), fabs(g[2]));
+                acc.sum = __dadd_rn(acc.sum, (den == 0.0) ? 1.0 : __ddiv_rn(num, den));
+            }
+            pc = pe[M];                                              // the forward neighbour along the march
+        }
+    }
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0)
+        partials[blockIdx.x + gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z)] = acc;
+}
+
 // Final reduction of the per-block partials by one block, in a fixed order.
 __global__ void __launch_bounds__(1024)
 diag_finalize_kernel(const DiagPartial* __restrict__ partials, int npartials, DiagPartial* __restrict__ out) {

@@ -21,7 +21,7 @@ ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WOR
              4: "PRS_ERR_STATE", 5: "PRS_ERR_CUDA"}
 
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
-           "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
+           "prs_weighted_area", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
            "prs_device_pointers", "prs_last_error"]
 
 
@@ -57,6 +57,7 @@ def lib():
         L.prs_init.argtypes = [vp, dbl]
         L.prs_step.argtypes = [vp, i64]
         L.prs_diagnostics.argtypes = [vp, C.POINTER(Diag)]
+        L.prs_weighted_area.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
         L.prs_copy_out.argtypes = [vp, vp, vp]
         L.prs_copy_in.argtypes = [vp, vp, vp, dbl, i64]
         L.prs_sync.argtypes = [vp]
@@ -142,6 +143,12 @@ class Simulation:
         d = Diag()
         self._chk(lib().prs_diagnostics(self._h, C.byref(d)), "prs_diagnostics")
         return d.as_dict()
+
+    def weighted_area(self):
+        """(area, rho_weighted) of Eq. 7 with the PRS orientation weight."""
+        a, r = C.c_double(), C.c_double()
+        self._chk(lib().prs_weighted_area(self._h, C.byref(a), C.byref(r)), "prs_weighted_area")
+        return float(a.value), float(r.value)
 
     def copy_out_to(self, phi_dst=None, phidot_dst=None):
         """Copies into caller buffers (torch tensors or numpy arrays, host or device)."""

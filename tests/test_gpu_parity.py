@@ -225,6 +225,51 @@ def test_diagnostics_of_special_fields(prec):
     assert abs(d["sum_ratio"] - dr["sum_ratio"]) <= 1e-12 * dr["sum_ratio"]
 
 
+# ------------------------------------------------------------------ Eq. 7 with the PRS orientation weight
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 1), (2, 2), (2, 5), (2, 256), (2, 1000), (3, 2), (3, 7), (3, 64), (3, 100)])
+def test_weighted_area_matches_the_oracle_on_snapshots(prec, dims, N):
+    g = prs.Simulation(dims, N, prec, seed=4)
+    g.init(1.0)
+    for nsteps in (0, 20, 60):
+        g.step(nsteps)
+        area, rho_w = g.weighted_area()
+        gp, _ = g.copy_out()
+        want = ref.weighted_area_of(gp)                      # oracle on the GPU's exact bytes
+        assert abs(area - want) <= 1e-12 * max(want, 1.0)
+        assert rho_w == area / N ** dims
+        C = g.diagnostics()["link_count"]
+        assert C / np.sqrt(dims) - 1e-9 <= area <= C + 1e-9
+
+
+def test_weighted_area_of_special_fields():
+    N = 64
+    g = prs.Simulation(3, N, prs.F64)
+    phi = fg.kink_pair(3, N, np.pi / 10.0, dtype=np.float64)
+    g.copy_in(phi, np.zeros_like(phi))
+    assert g.weighted_area()[0] == 2.0 * N * N               # walls normal to x: weight exactly 1
+    diag = fg.plane_wave(3, N, (1, 1, 1))
+    g.copy_in(diag, np.zeros_like(diag))
+    area, _ = g.weighted_area()
+    assert abs(area / g.diagnostics()["link_count"] - 1.0 / np.sqrt(3.0)) < 5e-3
+    vac = np.full((N,) * 3, 1.0)
+    g.copy_in(vac, np.zeros_like(vac))
+    assert g.weighted_area() == (0.0, 0.0)
+
+
+@pytest.mark.parametrize("dims,N,nsteps,ratio", [(3, 256, 300, 2.0 / 3.0), (2, 2048, 400, np.pi / 4.0)])
+def test_weight_turns_the_link_count_into_the_area_of_an_isotropic_network(dims, N, nsteps, ratio):
+    # Counting links overestimates the area of an isotropically oriented wall by the mean of
+    # |n_x| + |n_y| (+ |n_z|) over directions: 4/pi in 2D, 3/2 in 3D; the PRS weight of Eq. 7 removes
+    # exactly that, so weighted / unweighted -> pi/4 and 2/3 once the network has formed.
+    g = prs.Simulation(dims, N, prs.F32, seed=6)
+    g.init(1.0)
+    g.step(nsteps)
+    area, _ = g.weighted_area()
+    assert abs(area / g.diagnostics()["link_count"] - ratio) < 0.02
+
+
 # ------------------------------------------------------------------ symmetries on the GPU (P2-P5 re-run)
 
 @pytest.mark.parametrize("kernel", KERNELS)
