@@ -33,6 +33,8 @@ def lib():
         L.prs_ref_create.argtypes = [C.POINTER(vp), ci, i64, ci, dbl, dbl, dbl, dbl, dbl, u64]
         L.prs_ref_destroy.argtypes = [vp]
         L.prs_ref_set_arith.argtypes = [vp, ci]
+        L.prs_ref_set_beta.argtypes = [vp, dbl]
+        L.prs_ref_scalars_beta.argtypes = [dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, C.POINTER(dbl)]
         L.prs_ref_set_threads.argtypes = [vp, ci]
         L.prs_ref_init.argtypes = [vp, dbl]
         L.prs_ref_step.argtypes = [vp, i64]
@@ -66,7 +68,7 @@ class RefSim:
     """One oracle simulation; same call names as the product binding."""
 
     def __init__(self, dims, N, precision=F32, alpha=3.0, era_m=1.0, deta=0.1, W0=10.0, phi0=1.0,
-                 seed=1, arith=ARITH_LITERAL, threads=1):
+                 seed=1, arith=ARITH_LITERAL, threads=1, beta=0.0):
         self.dims, self.N, self.precision = dims, int(N), precision
         self.params = dict(alpha=alpha, era_m=era_m, deta=deta, W0=W0, phi0=phi0)
         self.dtype = _DT[precision]
@@ -76,6 +78,7 @@ class RefSim:
                                   phi0, seed), "prs_ref_create")
         _chk(lib().prs_ref_set_arith(self._h, arith), "prs_ref_set_arith")
         _chk(lib().prs_ref_set_threads(self._h, threads), "prs_ref_set_threads")
+        _chk(lib().prs_ref_set_beta(self._h, beta), "prs_ref_set_beta")
 
     def close(self):
         if self._h:
@@ -155,7 +158,7 @@ def step_sites(phi, phidot, sites, n, eta0=1.0, arith=ARITH_LITERAL, alpha=3.0, 
     return po, vo
 
 
-def scalars(n, eta0=1.0, alpha=3.0, era_m=1.0, deta=0.1, W0=10.0, phi0=1.0):
+def scalars(n, eta0=1.0, alpha=3.0, era_m=1.0, deta=0.1, W0=10.0, phi0=1.0, beta=0.0):
     out = (C.c_double * 7)()
-    _chk(lib().prs_ref_scalars(alpha, era_m, deta, W0, phi0, eta0, n, out), "prs_ref_scalars")
+    _chk(lib().prs_ref_scalars_beta(alpha, beta, era_m, deta, W0, phi0, eta0, n, out), "prs_ref_scalars_beta")
     return dict(zip(("eta", "delta", "A", "B", "V0", "K", "I"), [float(v) for v in out]))

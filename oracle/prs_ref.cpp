@@ -82,13 +82,18 @@ struct Scalars {
 
 const double PI = 3.14159265358979323846;
 
+/* beta: the exponent of the scale factor in front of dV/dphi in Eq. 2 (:34; printed "alpha^beta",
+ * meant a^beta, R1).  PRS: beta = 0 (:42).  beta != 0 (e.g. the exact equations alpha = beta
+ * = 2, :36) multiplies dV/dphi at step n by a(eta_n)^beta with a = (eta/eta0)^m, m = dln a/dln eta,
+ * normalised to a(eta0) = 1 (R16); it enters only through the per-step constant K. */
 Scalars scalars_at(double alpha, double era_m, double deta, double W0, double phi0,
-                   double eta0, int64_t n) {
+                   double eta0, int64_t n, double beta = 0.0) {
     Scalars s;
     s.V0 = (PI * PI * phi0 * phi0) / (2.0 * W0 * W0);
-    s.K = 4.0 * s.V0 / (phi0 * phi0);
     s.I = 1.0 / (phi0 * phi0);
     s.eta = eta0 + (double)n * deta;                       /* never accumulated step by step */
+    s.K = 4.0 * s.V0 / (phi0 * phi0);
+    if (beta != 0.0 && era_m != 0.0) s.K = s.K * std::pow(s.eta / eta0, era_m * beta);
     s.delta = ((0.5 * alpha) * (deta / s.eta)) * era_m;    /* Eq. 6 */
     s.A = (1.0 - s.delta) / (1.0 + s.delta);
     s.B = deta / (1.0 + s.delta);
@@ -277,7 +282,7 @@ double weighted_area_of(int dims, int64_t N, const T* phi) {
 struct prs_ref_ctx {
     int dims, precision, arith, threads;
     int64_t N, S, step;
-    double alpha, era_m, deta, W0, phi0, eta0;
+    double alpha, era_m, deta, W0, phi0, eta0, beta;
     uint64_t seed;
     bool inited;
     std::vector<float> f_phi, f_pd, f_phi2, f_pd2;
@@ -289,7 +294,7 @@ namespace {
 template <typename T>
 void step_once(prs_ref_ctx* h, std::vector<T>& phi, std::vector<T>& pd, std::vector<T>& phi2,
                std::vector<T>& pd2) {
-    const Scalars sc = scalars_at(h->alpha, h->era_m, h->deta, h->W0, h->phi0, h->eta0, h->step);
+    const Scalars sc = scalars_at(h->alpha, h->era_m, h->deta, h->W0, h->phi0, h->eta0, h->step, h->beta);
     const StepCoef<T> k = make_coef<T>(sc, h->deta, h->dims, h->arith);
     const int64_t N = h->N, Nz = (h->dims == 3) ? N : 1;
     const T* p = phi.data();
@@ -343,7 +348,7 @@ int prs_ref_create(prs_ref_handle* out, int dims, int64_t N, int precision, doub
     if (!h) return 3;
     h->dims = dims; h->N = N; h->precision = precision;
     h->S = (dims == 3) ? N * N * N : N * N;
-    h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0;
+    h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0; h->beta = 0.0;
     h->seed = seed; h->arith = PRS_REF_ARITH_LITERAL; h->threads = 1;
     h->eta0 = 1.0; h->step = 0; h->inited = false;
     try {
@@ -363,6 +368,12 @@ int prs_ref_create(prs_ref_handle* out, int dims, int64_t N, int precision, doub
 int prs_ref_destroy(prs_ref_handle h) {
     if (!h) return 1;
     delete h;
+    return 0;
+}
+
+int prs_ref_set_beta(prs_ref_handle h, double beta) {
+    if (!h || !std::isfinite(beta)) return 1;
+    h->beta = beta;
     return 0;
 }
 
@@ -487,6 +498,15 @@ int prs_ref_step_sites(int dims, int64_t N, int precision, int arith, double alp
                                 &((double*)phi_next_out)[i], &((double*)phidot_next_out)[i]);
         }
     }
+    return 0;
+}
+
+int prs_ref_scalars_beta(double alpha, double beta, double era_m, double deta, double W0, double phi0,
+                         double eta0, int64_t n, double out[7]) {
+    if (!out) return 1;
+    const Scalars s = scalars_at(alpha, era_m, deta, W0, phi0, eta0, n, beta);
+    out[0] = s.eta; out[1] = s.delta; out[2] = s.A; out[3] = s.B;
+    out[4] = s.V0; out[5] = s.K; out[6] = s.I;
     return 0;
 }
 

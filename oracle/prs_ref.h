@@ -49,6 +49,8 @@ typedef struct {
 int prs_ref_create(prs_ref_handle* out, int dims, int64_t N, int precision,
                    double alpha, double era_m, double deta, double W0, double phi0, uint64_t seed);
 int prs_ref_destroy(prs_ref_handle h);
+int prs_ref_set_beta(prs_ref_handle h, double beta);    /* default 0 (PRS); a^beta multiplies dV/dphi,   *
+                                                          * a = (eta/eta0)^m normalised at eta0          */
 int prs_ref_set_arith(prs_ref_handle h, int arith);      /* default LITERAL                     */
 int prs_ref_set_threads(prs_ref_handle h, int nthreads); /* default 1; >1 = OpenMP outer loop,  *
                                                           * results bit-identical (Jacobi step) */
@@ -87,6 +89,9 @@ int prs_ref_step_sites(int dims, int64_t N, int precision, int arith,
 
 /* Per-step scalars (Eq. 6 and the derived coefficients), all in double: out[0]=eta_n,
  * out[1]=delta_n, out[2]=A, out[3]=B, out[4]=V0, out[5]=K=4V0/phi0^2, out[6]=I=1/phi0^2. */
+/* The same with the scale-factor exponent beta of Eq. 2: K becomes K * (eta_n/eta0)^(m*beta). */
+int prs_ref_scalars_beta(double alpha, double beta, double era_m, double deta, double W0, double phi0,
+                         double eta0, int64_t n, double out[7]);
 int prs_ref_scalars(double alpha, double era_m, double deta, double W0, double phi0,
                     double eta0, int64_t n, double out[7]);
 

@@ -227,6 +227,48 @@ def test_uniform_field_follows_the_scalar_recurrence(dims, N):
     assert abs(p.flat[0] - c) < 1e-14 and abs(v.flat[0] - w) < 1e-14
 
 
+# ------------------------------------------------------------------ the scale-factor exponent beta of Eq. 2
+
+def test_beta_scalars_closed_form():
+    # a = (eta/eta0)^m with a(eta0) = 1; K_n = (4 V0 / phi0^2) * a^beta.  eta0 = 1, deta = 1/2, n = 6 ->
+    # eta = 4; m = 2, beta = 2 -> a^beta = 4^4 = 256 exactly; W0 = pi -> 4 V0 = 2.
+    s = ref.scalars(6, eta0=1.0, alpha=2.0, era_m=2.0, deta=0.5, W0=np.pi, phi0=1.0, beta=2.0)
+    assert s["eta"] == 4.0 and s["K"] == 512.0 and s["delta"] == 0.5 * 2.0 * (0.5 / 4.0) * 2.0
+    assert ref.scalars(6, era_m=2.0, deta=0.5, W0=np.pi, beta=0.0)["K"] == 2.0          # PRS: no factor
+    assert ref.scalars(6, era_m=0.0, deta=0.5, W0=np.pi, beta=2.0)["K"] == 2.0          # no expansion: a = 1
+    assert ref.scalars(0, eta0=3.0, era_m=1.0, deta=0.5, W0=np.pi, beta=2.0)["K"] == 2.0  # a(eta0) = 1
+
+
+@pytest.mark.parametrize("arith", [ref.ARITH_LITERAL, ref.ARITH_COEF, ref.ARITH_FMA])
+def test_beta_zero_changes_nothing_and_beta_two_does(arith):
+    phi, pd = fg.random_state(3, 6, 31, np.float64)
+    a = run(3, 6, ref.F64, phi, pd, 10, arith=arith)
+    b = run(3, 6, ref.F64, phi, pd, 10, arith=arith, beta=0.0)
+    c = run(3, 6, ref.F64, phi, pd, 10, arith=arith, alpha=2.0, beta=2.0)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    assert not np.array_equal(a[0], c[0])
+
+
+@pytest.mark.parametrize("dims,N", [(2, 6), (3, 5)])
+@pytest.mark.parametrize("alpha,beta,m", [(2.0, 2.0, 1.0), (2.0, 2.0, 2.0), (3.0, 1.0, 2.0)])
+def test_uniform_field_follows_the_scalar_recurrence_with_the_scale_factor(dims, N, alpha, beta, m):
+    # as P6, with dV/dphi multiplied by a^beta = (eta_n/eta0)^(m beta) (Eq. 2, :34-36)
+    c0, v0, deta, eta0, W0 = 0.3, 0.05, 0.1, 2.0, 10.0
+    V0 = np.pi ** 2 / (2 * W0 ** 2)
+    phi = np.full((N,) * dims, c0)
+    pd = np.full((N,) * dims, v0)
+    p, v = run(dims, N, ref.F64, phi, pd, 40, eta0=eta0, alpha=alpha, era_m=m, beta=beta)
+    c, w = c0, v0
+    for n in range(40):
+        eta = eta0 + n * deta
+        delta = 0.5 * alpha * deta / eta * m
+        dV = (eta / eta0) ** (m * beta) * 4 * V0 * c * (c * c - 1.0)
+        w = ((1 - delta) * w - deta * dV) / (1 + delta)
+        c = c + deta * w
+    assert np.all(p == p.flat[0]) and np.all(v == v.flat[0])
+    assert abs(p.flat[0] - c) < 1e-13 and abs(v.flat[0] - w) < 1e-13
+
+
 # ------------------------------------------------------------------ P7: free discrete wave (exact eigenmode)
 
 def _lattice_k2(N, modes):
