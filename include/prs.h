@@ -132,6 +132,11 @@ int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst);
  * that eta_n = eta0 + n*deta; synchronises the stream. */
 int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, double eta0, int64_t step);
 
+/* Exponent beta of the scale factor in front of dV/dphi in Eq. 2.  Default 0 (PRS, :42);
+ * beta = 2 with alpha = 2 gives the exact equations of motion.  a(eta) = (eta/eta0)^era_m, a(eta0) = 1 with
+ * eta0 the time given to prs_init / prs_copy_in (R16); takes effect from the next prs_step. */
+int prs_set_beta(prs_handle h, double beta);
+
 /* Blocks until everything queued for h has finished; reports a pending asynchronous CUDA fault. */
 int prs_sync(prs_handle h);
 

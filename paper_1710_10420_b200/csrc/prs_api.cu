@@ -60,7 +60,7 @@ struct prs_ctx {
     int dims, precision;
     int64_t N;
     size_t S;
-    double alpha, era_m, deta, W0, phi0;
+    double alpha, era_m, deta, W0, phi0, beta;
     uint64_t seed;
     cudaStream_t stream;
     char* ws;
@@ -103,9 +103,11 @@ template <typename T>
 StepCoef<T> coef_at(const prs_ctx* h, int64_t n) {
     const double pi = 3.14159265358979323846;
     const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0);
-    const double K = 4.0 * V0 / (h->phi0 * h->phi0);
+    double K = 4.0 * V0 / (h->phi0 * h->phi0);
     const double I = 1.0 / (h->phi0 * h->phi0);
     const double eta = h->eta0 + (double)n * h->deta;
+    // Eq. 2 (:34) with beta != 0: dV/dphi times a^beta, a = (eta/eta0)^m (R16)
+    if (h->beta != 0.0 && h->era_m != 0.0) K = K * std::pow(eta / h->eta0, h->era_m * h->beta);
     const double delta = ((0.5 * h->alpha) * (h->deta / eta)) * h->era_m;
     StepCoef<T> k;
     k.K = (T)K;
@@ -467,7 +469,7 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     prs_ctx* h = new (std::nothrow) prs_ctx();
     if (!h) return PRS_ERR_INVALID_ARG;
     h->dims = dims; h->precision = precision; h->N = N; h->S = sites_of(dims, N);
-    h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0; h->seed = seed;
+    h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0; h->seed = seed; h->beta = 0.0;
     h->stream = (cudaStream_t)cuda_stream;
     h->ws = (char*)workspace;
     h->phi[0] = h->ws + L.off_phi[0]; h->phi[1] = h->ws + L.off_phi[1];
@@ -619,6 +621,13 @@ int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, doubl
     PRS_CUDA(h, cudaMemcpyAsync(h->pd[h->cur], phidot_src, bytes, cudaMemcpyDefault, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     h->eta0 = eta0; h->step = step; h->inited = true;
+    return PRS_OK;
+}
+
+int prs_set_beta(prs_handle h, double beta) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!std::isfinite(beta)) return fail(h, PRS_ERR_INVALID_ARG, "prs_set_beta: beta must be finite");
+    h->beta = beta;
     return PRS_OK;
 }
 

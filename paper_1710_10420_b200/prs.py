@@ -21,7 +21,7 @@ ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WOR
              4: "PRS_ERR_STATE", 5: "PRS_ERR_CUDA"}
 
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
-           "prs_weighted_area", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
+           "prs_weighted_area", "prs_set_beta", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
            "prs_device_pointers", "prs_last_error"]
 
 
@@ -58,6 +58,7 @@ def lib():
         L.prs_step.argtypes = [vp, i64]
         L.prs_diagnostics.argtypes = [vp, C.POINTER(Diag)]
         L.prs_weighted_area.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
+        L.prs_set_beta.argtypes = [vp, dbl]
         L.prs_copy_out.argtypes = [vp, vp, vp]
         L.prs_copy_in.argtypes = [vp, vp, vp, dbl, i64]
         L.prs_sync.argtypes = [vp]
@@ -143,6 +144,9 @@ class Simulation:
         d = Diag()
         self._chk(lib().prs_diagnostics(self._h, C.byref(d)), "prs_diagnostics")
         return d.as_dict()
+
+    def set_beta(self, beta):
+        self._chk(lib().prs_set_beta(self._h, beta), "prs_set_beta")
 
     def weighted_area(self):
         """(area, rho_weighted) of Eq. 7 with the PRS orientation weight."""

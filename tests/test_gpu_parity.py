@@ -225,6 +225,33 @@ def test_diagnostics_of_special_fields(prec):
     assert abs(d["sum_ratio"] - dr["sum_ratio"]) <= 1e-12 * dr["sum_ratio"]
 
 
+# ------------------------------------------------------------------ Eq. 2 with beta != 0 (exact equations)
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 132), (3, 36)])
+def test_exact_equations_alpha_beta_two_match_the_oracle(kernel, prec, dims, N):
+    g = prs.Simulation(dims, N, prec, alpha=2.0, era_m=2.0, seed=8)
+    g.set_step_kernel(kernel)
+    g.set_beta(2.0)
+    r = ref.RefSim(dims, N, prec, alpha=2.0, era_m=2.0, seed=8, beta=2.0, arith=ref.ARITH_FMA, threads=THREADS)
+    g.init(1.5)
+    r.init(1.5)
+    g.step(20)
+    r.step(20)
+    a, b = g.copy_out(), r.copy_out()
+    assert a[0].tobytes() == b[0].tobytes() and a[1].tobytes() == b[1].tobytes()
+    lit = ref.RefSim(dims, N, prec, alpha=2.0, era_m=2.0, seed=8, beta=2.0, threads=THREADS)
+    lit.init(1.5)
+    lit.step(20)
+    c = lit.copy_out()
+    assert maxdiff(a[0], c[0]) <= TOL[prec] and maxdiff(a[1], c[1]) <= TOL[prec]
+    pr = ref.RefSim(dims, N, prec, alpha=2.0, era_m=2.0, seed=8, arith=ref.ARITH_FMA, threads=THREADS)   # beta = 0
+    pr.init(1.5)
+    pr.step(20)
+    assert pr.copy_out()[0].tobytes() != a[0].tobytes()
+
+
 # ------------------------------------------------------------------ Eq. 7 with the PRS orientation weight
 
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
@@ -403,7 +430,7 @@ def test_copy_in_out_roundtrip_device_and_host_and_step_split():
     # device_pointers view equals copy_out
     pp, pv = g.device_pointers()
     assert pp and pv and pp != pv
-    assert g.kernel_launches >= 7
+    assert g.kernel_launches >= 3              # 3 steps = a two-step launch + a single step, 4 steps = one four-step launch
 
 
 def test_error_paths_on_device():
