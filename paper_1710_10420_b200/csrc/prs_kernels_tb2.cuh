@@ -3,25 +3,29 @@
 // site-update halves to 8 B (FP32) / 16 B (FP64); the per-site arithmetic is the same sequence of
 // individually rounded operations as two single steps, so the result is bit-identical to them.
 //
-// With half the HBM traffic the kernel is bound by instruction issue, not by memory, so the design
-// goal is instructions per site-update: packed FP32 arithmetic (prs_pack.cuh: FADD2 / FMUL2 round two
-// sites per instruction), each thread's own column kept in a register window (only neighbour rows go
-// through shared memory), no integer division and no 64-bit address arithmetic inside the march.
+// With half the HBM traffic the first version was bound by instruction issue, not by memory, so the
+// design goal became instructions per site-update: packed FP32 arithmetic (prs_pack.cuh: FADD2 / FMUL2
+// / FFMA2 round two sites per instruction), each thread's own column kept in a register window (only
+// neighbour rows go through shared memory), no integer division and only 32-bit cursor arithmetic inside
+// the march, one copy of the march per kind of row.  In that state it is HBM-bound again
+// (profiles/r01b_*), which is why prs_kernels_tbs.cuh goes on to four steps per pass; this kernel now
+// serves the leftovers of a prs_step call and the PRS_KERNEL_TB2 option.
 //
 // 3D scheme.  A CTA owns TY rows x 30 vectors of x (120 floats / 60 doubles) of output and marches a
 // chunk of z planes.  It is 32 lanes wide and TY+4 warps tall: lane 0 / lane 31 and the two outer
 // rows on each side are halo.  Plane index a = 0, 1, ... stands for z = z0-2+a (periodic).  In
 // iteration j every thread
-//   (0) waits for its cp.async group j (phi^n plane a = j+2, phidot^{n-1/2} plane z0-1+j), then the
+//   (0) waits for its cp.async group j (phi^n plane a = j+2 and the phidot plane of z = z0+j), then the
 //       CTA barrier makes every thread's group j visible and retires all reads of iteration j-1;
-//   (1) issues one 16-byte cp.async for its own column of phi^n plane a = j+2+PF and of the phidot
-//       plane PF ahead, straight into shared-memory rings (no register staging);
+//   (1) issues one 16-byte cp.async for its own column of phi^n plane a = j+4 and of the phidot plane
+//       of the same z, straight into four-slot shared-memory rings (no register staging; the march is
+//       unrolled four times, so every slot index is an immediate);
 //   (2) stage 1 (rows 1..TY+2): phi^{n+1}, phidot^{n+1/2} on plane a = j+1 from its register window
 //       (z-1, z), its own column of the ring (z+1), the neighbouring rows of the ring (y+-1) and warp
 //       shuffles (x+-1); publishes phi^{n+1} to a two-slot shared plane;
 //   (3) stage 2 (rows 2..TY+1, j >= 2): phi^{n+2}, phidot^{n+3/2} on plane a = j from its register
-//       window of phi^{n+1} (three planes deep), the neighbouring rows of the plane published one
-//       iteration ago and shuffles; lanes 1..30 store to HBM.
+//       window of phi^{n+1}, the neighbouring rows of the plane published one iteration ago and
+//       shuffles; lanes 1..30 store to HBM.
 // Values at the halo rim that lack a neighbour are computed from stand-ins and never used.
 //
 // 2D scheme.  Same idea with the march along y and no shared memory at all: both register windows
