@@ -199,12 +199,28 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __res
             return __ldg(phi + o);
         };
         c[M] = m0;
-        T pc = at2(0, 0, 0, 0);
-        for (int m = m0; m < m1; ++m) {
-            c[M] = m;
-            T pe[DIMS];
+        // Hot path: linear offset o of the site, constant offsets to its x+1 (and y+1) neighbours, and
+        // the offset to the next site of the march (negative at the periodic seam).
+        long long o = 0;
 #pragma unroll
-            for (int k = 0; k < DIMS; ++k) pe[k] = at2(k, 1, k, 0);   // forward neighbours
+        for (int m = 0; m < DIMS; ++m) o += c[m] * stride[m];
+        const long long dx = (c[0] == N - 1) ? -(long long)(N - 1) : 1;
+        const long long dy = (DIMS == 3) ? ((c[1] == N - 1) ? -(long long)(N - 1) * N : (long long)N) : 0;
+        auto dm = [&](int m) { return (m == N - 1) ? -(long long)(N - 1) * stride[M] : stride[M]; };
+        auto forward = [&](long long at, int m, T* out) {
+            out[0] = __ldg(phi + at + dx);
+            if (DIMS == 3) out[1] = __ldg(phi + at + dy);
+            out[M] = __ldg(phi + at + dm(m));
+        };
+        T pc = __ldg(phi + o);
+        T pe[DIMS], pn[DIMS];
+        forward(o, m0, pe);
+        for (int m = m0; m < m1; ++m) {
+            // the forward neighbours of the next site of the march are requested before this site is
+            // worked on (one iteration of latency hiding; past the end this re-reads harmlessly)
+            const long long on = o + dm(m);
+            forward(on, (m + 1 == N) ? 0 : m + 1, pn);
+            c[M] = m;
             const bool me = A::neg(pc);
 #pragma unroll
             for (int k = 0; k < DIMS; ++k) {
@@ -224,6 +240,9 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __res
                 acc.sum = __dadd_rn(acc.sum, (den == 0.0) ? 1.0 : __ddiv_rn(num, den));
             }
             pc = pe[M];                                              // the forward neighbour along the march
+#pragma unroll
+            for (int k = 0; k < DIMS; ++k) pe[k] = pn[k];
+            o = on;
         }
     }
     acc = block_reduce(acc);
