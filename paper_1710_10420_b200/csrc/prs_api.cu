@@ -128,14 +128,16 @@ bool tiled_supported(const prs_ctx* h) {
     return h->N % W == 0 && h->N >= W && h->N <= (1 << 30);
 }
 
-// The 3D two-step kernel addresses 16-byte vectors with 32-bit indices (cursor overshoot included).
+// The temporally blocked kernels address 16-byte vectors with unsigned 32-bit indices whose load cursor
+// overshoots by up to one lattice length before it wraps: N^d / W <= 2^31 (2048^3 FP32 just fits).
 bool tb2_supported(const prs_ctx* h) {
     if (!tiled_supported(h)) return false;
-    return h->dims == 2 || h->S / (size_t)vec_width(h->precision) < ((size_t)1 << 30);
+    return h->dims == 2 || h->S / (size_t)vec_width(h->precision) <= ((size_t)1 << 31);
 }
-// So do the multi-step kernels, in 2D as well.
 bool tbs_supported(const prs_ctx* h) {
-    return tiled_supported(h) && h->S / (size_t)vec_width(h->precision) < ((size_t)1 << 30);
+    if (!tiled_supported(h)) return false;
+    const size_t nv = h->S / (size_t)vec_width(h->precision);
+    return h->dims == 3 ? nv <= ((size_t)1 << 31) : nv < ((size_t)1 << 30);     // the 2D kernel's cursors are signed
 }
 
 int resolve_step_kernel(const prs_ctx* h) {
@@ -540,7 +542,7 @@ int prs_step(prs_handle h, int64_t nsteps) {
             left -= 4;
         }
     }
-    if (kernel == PRS_KERNEL_TB2 || kernel == PRS_KERNEL_TBS) {
+    if ((kernel == PRS_KERNEL_TB2 || kernel == PRS_KERNEL_TBS) && tb2_supported(h)) {
         for (; left >= 2; left -= 2) {
             const int rc = (h->precision == PRS_F32) ? step_twice<float>(h) : step_twice<double>(h);
             if (rc != PRS_OK) return rc;

@@ -93,20 +93,20 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     c1.template set<3>(k1);
     c2.template set<3>(k2);
 
-    // All global addresses are 32-bit indices of 16-byte vectors (the host checks N^3 / W < 2^31):
+    // All global addresses are unsigned 32-bit indices of 16-byte vectors (the host checks N^3 / W <= 2^31):
     // one IMAD.WIDE forms an address, one IADD advances a cursor.
     const V* const gA = reinterpret_cast<const V*>(phi);
     const V* const gP = reinterpret_cast<const V*>(phidot);
     V* const oA = reinterpret_cast<V*>(phi_out);
     V* const oP = reinterpret_cast<V*>(phidot_out);
-    const int NNv = N * NQ;                                          // vectors per plane
-    const int colv = y * NQ + q;                                     // this thread's column within a plane
+    const unsigned NNv = (unsigned)N * (unsigned)NQ;                 // vectors per plane
+    const unsigned colv = (unsigned)y * (unsigned)NQ + (unsigned)q;  // this thread's column within a plane
     // One load cursor serves both fields: issue i fetches phi^n plane a = i (z = z0-2+i, periodic)
     // and the phidot plane of the same z, which stage 1 needs one iteration later than phi^n.
     int zl = wrap_mod(z0 - 2, N);
-    int il = zl * NNv + colv;
+    unsigned il = (unsigned)zl * NNv + colv;
     int left_to_wrap = N - zl;                                       // issues until z wraps to 0
-    int io = z0 * NNv + colv;                                        // store cursor (plane a = j, from j = 2)
+    unsigned io = (unsigned)z0 * NNv + colv;                         // store cursor (plane a = j, from j = 2)
 
     // The three kinds of row run their own march, so that no per-iteration test of the row survives
     // and the register windows rotate by renaming in the unrolled code:
@@ -120,7 +120,7 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
             if (ROLE >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
             ++ni; il += NNv;
-            if (--left_to_wrap == 0) { il -= N * NNv; left_to_wrap = N; }
+            if (--left_to_wrap == 0) { il -= (unsigned)N * NNv; left_to_wrap = N; }   // modulo 2^32, exact
         };
         // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
         issue(0, 3); issue(1, 0); issue(2, 1);

@@ -83,17 +83,18 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 #pragma unroll
     for (int s = 0; s < S; ++s) pc[s].template set<3>(coefs.k[s]);
 
-    // 32-bit indices of 16-byte vectors (the host checks N^3 / W < 2^30).
+    // Unsigned 32-bit indices of 16-byte vectors (the host checks N^3 / W <= 2^31, so that the cursor,
+    // which runs one lattice length past the end before it wraps, stays below 2^32).
     const V* const gA = reinterpret_cast<const V*>(phi);
     const V* const gP = reinterpret_cast<const V*>(phidot);
     V* const oA = reinterpret_cast<V*>(phi_out);
     V* const oP = reinterpret_cast<V*>(phidot_out);
-    const int NNv = N * NQ;                                          // vectors per plane
-    const int colv = y * NQ + q;                                     // this thread's column within a plane
+    const unsigned NNv = (unsigned)N * (unsigned)NQ;                 // vectors per plane
+    const unsigned colv = (unsigned)y * (unsigned)NQ + (unsigned)q;  // this thread's column within a plane
     int zl = wrap_mod(z0 - S, N);
-    int il = zl * NNv + colv;                                        // load cursor: issue i = plane a = i
+    unsigned il = (unsigned)zl * NNv + colv;                         // load cursor: issue i = plane a = i
     int left_to_wrap = N - zl;                                       // issues until z wraps to 0
-    int io = z0 * NNv + colv;                                        // store cursor
+    unsigned io = (unsigned)z0 * NNv + colv;                         // store cursor
 
     auto march = [&](auto ns_tag) {
         constexpr int NS = decltype(ns_tag)::value;                  // stages this row runs
@@ -102,7 +103,7 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
             if (NS >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
             ++ni; il += NNv;
-            if (--left_to_wrap == 0) { il -= N * NNv; left_to_wrap = N; }
+            if (--left_to_wrap == 0) { il -= (unsigned)N * NNv; left_to_wrap = N; }   // modulo 2^32, exact
         };
         // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
         issue(0, 3); issue(1, 0); issue(2, 1);

@@ -428,6 +428,44 @@ def test_repeated_runs_are_identical(dims, N, prec):
     assert all(o == outs[0] for o in outs[1:])
 
 
+@pytest.mark.slow
+def test_largest_lattice_that_fits_2048_cubed():
+    """Maximum size: 2048^3 FP32 = 8.6e9 sites, 137 GB of workspace, link counts beyond 2^32 and byte
+    offsets beyond 2^35.  The oracle cannot hold it, so the default path (four-step kernel with unsigned
+    32-bit vector cursors at their limit, tiled diagnostics) is checked against the generic kernels,
+    whose index arithmetic is plain 64-bit: diagnostics equal, and the last 64 MiB of phi identical."""
+    import ctypes
+    import torch
+
+    free, _ = torch.cuda.mem_get_info()
+    need = prs.prs_workspace_bytes(3, 2048, prs.F32)
+    if free < need + (1 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
+    cudart = ctypes.CDLL("libcudart.so")
+    res = []
+    for kernel in (prs.KERNEL_AUTO, prs.KERNEL_GENERIC):
+        g = prs.Simulation(3, 2048, prs.F32, seed=2)
+        g.set_step_kernel(kernel)
+        if kernel == prs.KERNEL_GENERIC:
+            g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_GENERIC)
+        g.init(1.0)
+        g.step(9)                                            # two four-step launches and a single step
+        d = g.diagnostics()
+        assert g.get_info(binding.INFO_STEP_KERNEL) == (prs.KERNEL_TBS if kernel == prs.KERNEL_AUTO else kernel)
+        pp, _ = g.device_pointers()
+        tail = torch.empty(1 << 24, dtype=torch.float32, device="cuda")
+        off = (2048 ** 3 - (1 << 24)) * 4
+        rc = cudart.cudaMemcpy(ctypes.c_void_p(tail.data_ptr()), ctypes.c_void_p(pp + off), ctypes.c_size_t((1 << 24) * 4), 3)
+        assert rc == 0
+        res.append((d["link_count"], d["wall_sites"], d["sum_ratio"], tail.cpu().numpy().tobytes()))
+        g.close()
+        del g, tail
+        torch.cuda.empty_cache()
+    assert res[0][0] == res[1][0] > 2 ** 32 and res[0][1] == res[1][1]
+    assert abs(res[0][2] - res[1][2]) <= 1e-10 * res[1][2]
+    assert res[0][3] == res[1][3]
+
+
 # ------------------------------------------------------------------ state handling
 
 def test_copy_in_out_roundtrip_device_and_host_and_step_split():
