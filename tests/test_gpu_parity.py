@@ -466,6 +466,35 @@ def test_largest_lattice_that_fits_2048_cubed():
     assert res[0][3] == res[1][3]
 
 
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("PRS_LONG_RUNS") != "1",
+                    reason="full-length oracle runs take ~15 min each on 16 cores; set PRS_LONG_RUNS=1")
+@pytest.mark.parametrize("dims,N,era_m,every", [(2, 4096, 1.0, 100), (2, 4096, 2.0, 100), (3, 512, 1.0, 50)])
+def test_full_length_runs_match_the_oracle(dims, N, era_m, every):
+    """T5 at BASELINE.json's configs[1] and configs[3] in full: eta from 1 to N/2, diagnostics at the
+    configs' cadence, the GPU's default path against the oracle's literal FP32 form on the host cores.
+    rho(eta) within 2 % at every sample, fitted exponent within 0.02 (fit for eta >= 32); the last
+    measured outcome is recorded in DESIGN.md section 10."""
+    nsamp = int(round((N / 2 - 1.0) / 0.1)) // every
+    g = prs.Simulation(dims, N, prs.F32, era_m=era_m, seed=1)
+    r = ref.RefSim(dims, N, ref.F32, era_m=era_m, seed=1, threads=THREADS)
+    g.init(1.0)
+    r.init(1.0)
+    eta, cg, cr, worst = [], [], [], 0.0
+    for _ in range(nsamp):
+        g.step(every)
+        r.step(every)
+        dg, dr = g.diagnostics(), r.diagnostics()
+        assert dg["eta"] == dr["eta"]
+        eta.append(dg["eta"]); cg.append(dg["rho"]); cr.append(dr["rho"])
+        worst = max(worst, abs(dg["rho"] - dr["rho"]) / dr["rho"])
+    eta, cg, cr = map(np.array, (eta, cg, cr))
+    mu_g, mu_r = fit_mu(eta, cg, 32.0), fit_mu(eta, cr, 32.0)
+    print("LONGRUN dims=%d N=%d era_m=%g samples=%d worst_rel_rho=%.3e mu_gpu=%.5f mu_oracle=%.5f identical_samples=%d"
+          % (dims, N, era_m, nsamp, worst, mu_g, mu_r, int(np.sum(cg == cr))))
+    assert worst <= 0.02 and abs(mu_g - mu_r) <= 0.02
+
+
 # ------------------------------------------------------------------ state handling
 
 def test_copy_in_out_roundtrip_device_and_host_and_step_split():
