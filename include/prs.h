@@ -71,6 +71,9 @@ enum {
     PRS_KERNEL_TILED   = 2,    /* shared-memory tiled, one step per pass over HBM                  */
     PRS_KERNEL_TB2     = 3,    /* temporally blocked: two steps per pass over HBM (same per-site   *
                                 * arithmetic, bit-identical to two single steps)                   */
+    PRS_KERNEL_CLUSTER = 5,    /* small 2D boxes (N = 64, 128, 256): the state stays in the shared   *
+                                * memory of one 8-CTA thread-block cluster for up to 32 steps per    *
+                                * launch; bit-identical to single steps                              */
     PRS_KERNEL_TBS     = 4     /* PRS_OPT_TBS_STEPS steps per pass over HBM (2D and 3D), bit-identical *
                                 * to single steps; leftovers of a prs_step call go through TB2 and  *
                                 * TILED                                                             */

@@ -16,6 +16,7 @@
 #include "prs_kernels_tiled.cuh"
 #include "prs_kernels_tb2.cuh"
 #include "prs_kernels_tbs.cuh"
+#include "prs_kernels_cluster.cuh"
 
 using namespace prs;
 
@@ -140,6 +141,13 @@ bool tbs_supported(const prs_ctx* h) {
     return h->dims == 3 ? nv <= ((size_t)1 << 31) : nv < ((size_t)1 << 30);     // the 2D kernel's cursors are signed
 }
 
+// The cluster-resident small-box kernel: 2D, whole rows per 1024-thread sweep, state in 8 CTAs' shared memory.
+bool cluster_supported(const prs_ctx* h) {
+    if (h->dims != 2 || (h->N != 64 && h->N != 128 && h->N != 256)) return false;
+    const size_t smem = (h->precision == PRS_F32) ? cluster_smem_bytes<float>((int)h->N) : cluster_smem_bytes<double>((int)h->N);
+    return smem <= 227 * 1024;
+}
+
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
     if (want == PRS_KERNEL_AUTO) {
@@ -147,6 +155,7 @@ int resolve_step_kernel(const prs_ctx* h) {
         // 128^3 up -- on small lattices because it needs a quarter of the launches, on large ones
         // because it moves a quarter of the bytes; below that the single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
+        else if (h->N == 64 && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;   // 0.8 vs 1.1 us per step
         else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
         else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = PRS_KERNEL_TB2;
         else want = PRS_KERNEL_TILED;
@@ -355,6 +364,40 @@ int step_many(prs_ctx* h, int S) {
     return PRS_OK;
 }
 
+// Up to CLUSTER_MAX_STEPS steps inside one cluster-resident launch (2D small boxes).
+template <typename T, int ARITH>
+cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int nsteps) {
+    ClusterCoefs<T> ks;
+    for (int s = 0; s < nsteps; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
+    for (int s = nsteps; s < CLUSTER_MAX_STEPS; ++s) ks.k[s] = ks.k[0];
+    const size_t smem = cluster_smem_bytes<T>((int)h->N);
+    static bool configured = false;            // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(step2d_cluster_kernel<T, ARITH>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    step2d_cluster_kernel<T, ARITH><<<CLUSTER_CTAS, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N, nsteps, ks);
+    return cudaGetLastError();
+}
+
+template <typename T>
+int step_cluster(prs_ctx* h, int nsteps) {
+    const T* p = (const T*)h->phi[h->cur];
+    const T* v = (const T*)h->pd[h->cur];
+    T* pn = (T*)h->phi[h->cur ^ 1];
+    T* vn = (T*)h->pd[h->cur ^ 1];
+    const cudaError_t e = (h->opt_arith == PRS_ARITH_LITERAL) ? launch_cluster<T, ARITH_LITERAL>(h, p, v, pn, vn, nsteps)
+                        : (h->opt_arith == PRS_ARITH_COEF)  ? launch_cluster<T, ARITH_COEF>(h, p, v, pn, vn, nsteps)
+                                                            : launch_cluster<T, ARITH_FMA>(h, p, v, pn, vn, nsteps);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cluster kernel launch");
+    h->launches += 1;
+    h->cur ^= 1;
+    h->step += nsteps;
+    return PRS_OK;
+}
+
 template <typename T>
 int step_once(prs_ctx* h, int kernel) {
     const StepCoef<T> k = coef_at<T>(h, h->step);
@@ -530,6 +573,14 @@ int prs_step(prs_handle h, int64_t nsteps) {
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
     const int kernel = resolve_step_kernel(h);
     int64_t left = nsteps;
+    if (kernel == PRS_KERNEL_CLUSTER) {
+        while (left > 0) {
+            const int n = (int)std::min<int64_t>(left, CLUSTER_MAX_STEPS);
+            const int rc = (h->precision == PRS_F32) ? step_cluster<float>(h, n) : step_cluster<double>(h, n);
+            if (rc != PRS_OK) return rc;
+            left -= n;
+        }
+    }
     if (kernel == PRS_KERNEL_TBS) {
         const int S = h->opt_tbs_steps;
         for (; left >= S; left -= S) {
@@ -654,6 +705,11 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
     switch (option) {
         case PRS_OPT_STEP_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
+            if (value == PRS_KERNEL_CLUSTER) {
+                if (!cluster_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the cluster-resident kernel takes 2D lattices of 64, 128 or 256 sites per side");
+                h->opt_step_kernel = (int)value;
+                return PRS_OK;
+            }
             if (value == PRS_KERNEL_TBS) {
                 if (!tbs_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the multi-step kernel needs N a multiple of 16 bytes of T and N^d / that < 2^30");
                 h->opt_step_kernel = (int)value;

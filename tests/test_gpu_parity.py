@@ -175,6 +175,41 @@ def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
                 break                             # the other forms: one length is enough
 
 
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("N", [64, 128, 256])
+def test_cluster_resident_kernel_equals_single_steps_bitwise(prec, N):
+    """Small-box kernel (state in the shared memory of one 8-CTA cluster, neighbour rows through
+    distributed shared memory, one cluster barrier per step): 1, 2, 31, 32, 33 and 75 steps (launches of
+    at most 32) against the single-step kernel, all arithmetic forms; and against the oracle."""
+    phi, pd = fg.random_state(2, N, 5, NP[prec])
+    for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
+        for nsteps in (1, 2, 31, 32, 33, 75) if arith == prs.ARITH_FMA else (33,):
+            outs = []
+            for kernel in (prs.KERNEL_TILED, prs.KERNEL_CLUSTER):
+                g = prs.Simulation(2, N, prec, era_m=2.0)
+                g.set_step_kernel(kernel)
+                g.set_arith(arith)
+                g.copy_in(phi, pd, eta0=1.0, step=3)
+                g.step(nsteps)
+                outs.append(g.copy_out())
+                if kernel == prs.KERNEL_CLUSTER:
+                    assert g.kernel_launches == (nsteps + 31) // 32
+            assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
+    g = prs.Simulation(2, N, prec, seed=3)
+    g.set_step_kernel(prs.KERNEL_CLUSTER)
+    r = ref.RefSim(2, N, prec, seed=3, arith=ref.ARITH_FMA)
+    g.init(1.0)
+    r.init(1.0)
+    g.step(40)
+    r.step(40)
+    a, b = g.copy_out(), r.copy_out()
+    assert a[0].tobytes() == b[0].tobytes() and a[1].tobytes() == b[1].tobytes()
+    with pytest.raises(prs.PrsError):
+        prs.Simulation(2, 96, prec).set_step_kernel(prs.KERNEL_CLUSTER)
+    with pytest.raises(prs.PrsError):
+        prs.Simulation(3, 64, prec).set_step_kernel(prs.KERNEL_CLUSTER)
+
+
 # ------------------------------------------------------------------ T3: diagnostics on snapshots
 
 @pytest.mark.parametrize("diag_kernel", [prs.KERNEL_GENERIC, prs.KERNEL_TILED])
