@@ -58,8 +58,8 @@ BYTES_PER_SITE_UPDATE = {0: 16, 1: 32}        # read phi, phidot; write phidot, 
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     # profiles/r01c_ncu_step3d_tbs4_f32_1024.md: 9.485 GB read + 8.558 GB written per four-step launch
     ("3d_1024_f32_rad", "tbs"): 18_043_506_000,
-    # profiles/r01c_ncu_step3d_tbs4_f64_1024.md: 20.726 GB read + 17.164 GB written per four-step launch
-    ("3d_1024_f64_rad", "tbs"): 37_889_208_000,
+    # profiles/r01d_ncu_step3d_tbs4_f64_1024.md: 19.655 GB read + 17.151 GB written per four-step launch
+    ("3d_1024_f64_rad", "tbs"): 36_806_144_000,
     # profiles/r01b_ncu_step3d_tb2_f32_1024.md: 9.136 GB read + 8.552 GB written per two-step launch
     ("3d_1024_f32_rad", "tb2"): 17_687_191_000,
     # profiles/r01b_ncu_step3d_tb2_f64_1024.md: 18.451 GB read + 17.144 GB written per two-step launch
