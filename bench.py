@@ -271,7 +271,8 @@ def run_gpu(args):
     step_kernel = sim.get_info(binding.INFO_STEP_KERNEL)
     # PRS steps the dominant kernel advances per launch; a prs_step(50) of the four-step kernel is 12
     # four-step launches and one two-step launch, so launch_ms is the time per steps_per_launch steps
-    steps_per_launch = {prs.KERNEL_TB2: 2, prs.KERNEL_TBS: 4 if dims == 3 else 6}.get(step_kernel, 1)
+    tbs_steps = 4 if dims == 3 else (8 if prec == 0 else 6)          # the library's defaults (prs.h, PRS_OPT_TBS_STEPS)
+    steps_per_launch = {prs.KERNEL_TB2: 2, prs.KERNEL_TBS: tbs_steps}.get(step_kernel, 1)
     launch_ms = ms_kernels / (step_kernel_launches / steps_per_launch)
     achieved = S * steps_per_launch * bpu / (launch_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak_gbs()

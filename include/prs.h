@@ -63,7 +63,7 @@ enum {
     PRS_OPT_TILE_Y      = 5,   /* tuning: rows per CTA of the 3D tiled kernel, 4 / 8 / 16          */
     PRS_OPT_TB2_TILE_Y  = 6,   /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
     PRS_OPT_TBS_STEPS   = 7    /* steps per pass of the multi-step kernel: 3 or 4, in 2D also 6 or 8;
-                                * default 4 in 3D, 6 in 2D                                          */
+                                * default 4 in 3D, in 2D 8 (FP32) or 6 (FP64)                       */
 };
 enum {
     PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */

@@ -1,21 +1,17 @@
 // prs_api.cu -- host side of libprs: context, workspace carving, per-step scalars, kernel selection
 // and launch, and the C ABI declared in include/prs.h.  No device memory is allocated here: the
 // caller's workspace holds everything (see prs.h, "Memory and ownership").
-#include "../../include/prs.h"
+// The temporally blocked kernels are compiled in translation units of their own (prs_instances.cu);
+// this one holds the single-step, cluster, diagnostics and initial-condition kernels.
+#include "prs_host.cuh"
 
-#include <cmath>
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <new>
-#include <string>
 
-#include <cuda_runtime.h>
-
-#include "prs_arith.cuh"
 #include "prs_kernels_generic.cuh"
 #include "prs_kernels_tiled.cuh"
-#include "prs_kernels_tb2.cuh"
-#include "prs_kernels_tbs.cuh"
 #include "prs_kernels_cluster.cuh"
 
 using namespace prs;
@@ -57,30 +53,6 @@ Layout layout_of(int dims, int64_t N, int precision) {
 
 }  // namespace
 
-struct prs_ctx {
-    int dims, precision;
-    int64_t N;
-    size_t S;
-    double alpha, era_m, deta, W0, phi0, beta;
-    uint64_t seed;
-    cudaStream_t stream;
-    char* ws;
-    void* phi[2];
-    void* pd[2];
-    int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
-    DiagPartial* partials;
-    DiagPartial* d_result;
-    DiagPartial* h_result;                    // pinned host, 24 bytes
-    double eta0;
-    int64_t step;
-    bool inited;
-    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps;
-    int last_step_kernel, last_diag_kernel;
-    int64_t launches;
-    int sm_count;
-    std::string err;
-};
-
 namespace {
 
 int fail(prs_ctx* h, int code, const std::string& msg) {
@@ -97,30 +69,6 @@ int cuda_fail(prs_ctx* h, cudaError_t e, const char* where) {
         cudaError_t e_ = (call);                                 \
         if (e_ != cudaSuccess) return cuda_fail((h), e_, #call); \
     } while (0)
-
-// Per-step scalars, Eq. 6 (:55) and the constants of Eq. 1 (:30); all in double, rounded to
-// the field type once.  eta_n = eta0 + n*deta is formed from n each time, never accumulated.
-template <typename T>
-StepCoef<T> coef_at(const prs_ctx* h, int64_t n) {
-    const double pi = 3.14159265358979323846;
-    const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0);
-    double K = 4.0 * V0 / (h->phi0 * h->phi0);
-    const double I = 1.0 / (h->phi0 * h->phi0);
-    const double eta = h->eta0 + (double)n * h->deta;
-    // Eq. 2 (:34) with beta != 0: dV/dphi times a^beta, a = (eta/eta0)^m (R16)
-    if (h->beta != 0.0 && h->era_m != 0.0) K = K * std::pow(eta / h->eta0, h->era_m * h->beta);
-    const double delta = ((0.5 * h->alpha) * (h->deta / eta)) * h->era_m;
-    StepCoef<T> k;
-    k.K = (T)K;
-    k.I = (T)I;
-    k.deta = (T)h->deta;
-    const T dT = (T)delta;
-    k.omd = T(1) - dT;
-    k.opd = T(1) + dT;
-    k.A = (T)((1.0 - delta) / (1.0 + delta));
-    k.B = (T)(h->deta / (1.0 + delta));
-    return k;
-}
 
 inline int vec_width(int precision) { return precision == PRS_F32 ? 4 : 2; }
 
@@ -217,52 +165,6 @@ cudaError_t launch_tiled2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     return cudaGetLastError();
 }
 
-template <typename T, int ARITH, int TY>
-cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
-                             const StepCoef<T>& k2) {
-    constexpr int W = VecOps<T>::W;
-    const int N = (int)h->N, NQ = N / W;
-    const size_t smem = tb2_smem_bytes<T, TY>();
-    static bool configured = false;            // per instantiation
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step3d_tb2_kernel<T, ARITH, TY>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    const unsigned gx = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT), gy = (unsigned)((N + TY - 1) / TY);
-    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
-    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
-    const dim3 block(32, TY + 4, 1);
-    step3d_tb2_kernel<T, ARITH, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, k1, k2);
-    return cudaGetLastError();
-}
-
-template <typename T, int ARITH>
-cudaError_t launch_tb2_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
-                          const StepCoef<T>& k2) {
-    switch (h->opt_tb2_tile_y) {
-        case 4: return launch_tb2_3d_ty<T, ARITH, 4>(h, p, v, pn, vn, k1, k2);
-        case 8: return launch_tb2_3d_ty<T, ARITH, 8>(h, p, v, pn, vn, k1, k2);
-        case 28: return launch_tb2_3d_ty<T, ARITH, 28>(h, p, v, pn, vn, k1, k2);
-        default: return launch_tb2_3d_ty<T, ARITH, 12>(h, p, v, pn, vn, k1, k2);
-    }
-}
-
-template <typename T, int ARITH>
-cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
-                          const StepCoef<T>& k2) {
-    constexpr int W = VecOps<T>::W;
-    const int N = (int)h->N, NQ = N / W;
-    const int BX = 128, warps = BX / 32;
-    const unsigned nwarps = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT);
-    const unsigned gx = (nwarps + warps - 1) / warps;
-    int YC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
-    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
-    step2d_tb2_kernel<T, ARITH><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k1, k2);
-    return cudaGetLastError();
-}
-
 // Two steps in one pass (n -> n+2); the caller guarantees the lattice is supported.
 template <typename T>
 int step_twice(prs_ctx* h) {
@@ -283,66 +185,6 @@ int step_twice(prs_ctx* h) {
 }
 
 // S steps in one pass (n -> n+S); the caller guarantees tbs_supported(h).
-template <typename T, int ARITH, int S>
-cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
-    // output rows per CTA: measured 1024^3, chunk 128: FP32 TY = 16 1.21 ms/step (20: 1.25, 12: 1.30);
-    // FP64 TY = 20 2.41 ms/step (16: 2.52, 12: 2.60)
-    constexpr int TY = (sizeof(T) == 8) ? 20 : 16;
-    constexpr int W = VecOps<T>::W;
-    const int N = (int)h->N, NQ = N / W;
-    StepCoefs<T, S> ks;
-    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
-    const size_t smem = tbs_smem_bytes<T, S, TY>();
-    static bool configured = false;            // per instantiation
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step3d_tbs_kernel<T, ARITH, S, TY>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    constexpr int XOUT = tbs_xout<T, S>();
-    const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
-    // Chunks of 128 planes: each chunk re-reads 2S halo planes (measured 1024^3 FP32, S = 4: 64 planes
-    // 1.25 ms/step, 128 planes 1.21, 256 planes 1.24 as the grid gets too coarse for 148 SMs).
-    // ... and short enough that the grid covers the chip twice (one CTA per SM) on small lattices.
-    int ZC;
-    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, N);
-    else {
-        const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
-        ZC = (int)std::max<long long>(16, std::min<long long>(128, N / chunks));
-        ZC = std::min<int>(ZC, N);
-    }
-    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
-    const dim3 block(32, TY + 2 * S, 1);
-    step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks);
-    return cudaGetLastError();
-}
-
-template <typename T, int ARITH, int S>
-cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
-    constexpr int W = VecOps<T>::W;
-    const int N = (int)h->N, NQ = N / W;
-    StepCoefs<T, S> ks;
-    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
-    constexpr int XOUT = tbs_xout<T, S>();
-    const int BX = 128, warps = BX / 32;
-    const unsigned nwarps = (unsigned)((NQ + XOUT - 1) / XOUT);
-    const unsigned gx = (nwarps + warps - 1) / warps;
-    // Rows per march: long enough to amortise the 2S halo rows, short enough for ~8 CTAs per SM (4096^2: 31 rows 0.89 ms per 50 steps, 62 rows 1.03); on
-    // launch-bound lattices (256^2: 1.6 us per step with 8-row marches, 2.6 us with 32) short wins.
-    int YC;
-    if (h->opt_chunk > 0) YC = (int)std::min<int64_t>(h->opt_chunk, N);
-    else {
-        const long long want = 8LL * h->sm_count;
-        long long chunks = (want + gx - 1) / gx;
-        YC = (int)std::max<long long>(8, std::min<long long>(128, N / std::max<long long>(1, chunks)));
-        YC = std::min<int>(YC, N);
-    }
-    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
-    step2d_tbs_kernel<T, ARITH, S><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, ks);
-    return cudaGetLastError();
-}
-
 template <typename T>
 int step_many(prs_ctx* h, int S) {
     const T* p = (const T*)h->phi[h->cur];
@@ -528,7 +370,8 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
     h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_FMA; h->opt_diag_kernel = PRS_KERNEL_AUTO;
     h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
-    h->opt_tbs_steps = (dims == 2) ? 6 : 4;     // measured: 16384^2 FP32 1.32e12 (S = 4), 1.67e12 (6), 1.52e12 (8) site-updates/s
+    // measured, 16384^2, site-updates/s: FP32 1.29e12 (S = 4), 1.76e12 (6), 1.95e12 (8); FP64 6.8e11 (4), 9.5e11 (6), 8.9e11 (8)
+    h->opt_tbs_steps = (dims == 3) ? 4 : (precision == PRS_F32 ? 8 : 6);
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     h->h_result = nullptr;
     int dev = attr.device;

@@ -1,0 +1,83 @@
+// prs_host.cuh -- what the translation units of libprs share on the host side: the context behind a
+// prs_handle, the per-step scalars, and the declarations of the launchers whose kernels are compiled
+// in translation units of their own (prs_instances.cu, one compiler run per precision and kernel
+// family, so that the library builds in parallel).  prs_api.cu sees only these declarations.
+#pragma once
+
+#include "../../include/prs.h"
+
+#include <cmath>
+#include <cstdint>
+#include <string>
+
+#include <cuda_runtime.h>
+
+#include "prs_arith.cuh"
+
+struct prs_ctx {
+    int dims, precision;
+    int64_t N;
+    size_t S;
+    double alpha, era_m, deta, W0, phi0, beta;
+    uint64_t seed;
+    cudaStream_t stream;
+    char* ws;
+    void* phi[2];
+    void* pd[2];
+    int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
+    prs::DiagPartial* partials;
+    prs::DiagPartial* d_result;
+    prs::DiagPartial* h_result;               // pinned host, 24 bytes
+    double eta0;
+    int64_t step;
+    bool inited;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps;
+    int last_step_kernel, last_diag_kernel;
+    int64_t launches;
+    int sm_count;
+    std::string err;
+};
+
+namespace prs {
+
+// Per-step scalars, Eq. 6 (:55) and the constants of Eq. 1 (:30); all in double, rounded to
+// the field type once.  eta_n = eta0 + n*deta is formed from n each time, never accumulated.
+template <typename T>
+StepCoef<T> coef_at(const prs_ctx* h, int64_t n) {
+    const double pi = 3.14159265358979323846;
+    const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0);
+    double K = 4.0 * V0 / (h->phi0 * h->phi0);
+    const double I = 1.0 / (h->phi0 * h->phi0);
+    const double eta = h->eta0 + (double)n * h->deta;
+    // Eq. 2 (:34) with beta != 0: dV/dphi times a^beta, a = (eta/eta0)^m (R16)
+    if (h->beta != 0.0 && h->era_m != 0.0) K = K * std::pow(eta / h->eta0, h->era_m * h->beta);
+    const double delta = ((0.5 * h->alpha) * (h->deta / eta)) * h->era_m;
+    StepCoef<T> k;
+    k.K = (T)K;
+    k.I = (T)I;
+    k.deta = (T)h->deta;
+    const T dT = (T)delta;
+    k.omd = T(1) - dT;
+    k.opd = T(1) + dT;
+    k.A = (T)((1.0 - delta) / (1.0 + delta));
+    k.B = (T)(h->deta / (1.0 + delta));
+    return k;
+}
+
+// Launchers defined in prs_launch_tb2.cuh / prs_launch_tbs.cuh and instantiated in prs_instances.cu.
+// p, v: phi^n and phidot^{n-1/2}; pn, vn: where the advanced fields go; all device pointers in the
+// context's workspace.  Each returns the launch error; the caller does the book-keeping.
+
+// two steps per pass (n -> n+2) with the scalars of steps n and n+1
+template <typename T, int ARITH>
+cudaError_t launch_tb2_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1, const StepCoef<T>& k2);
+template <typename T, int ARITH>
+cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1, const StepCoef<T>& k2);
+
+// S steps per pass (n -> n+S); the scalars are formed inside from h->step
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn);
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn);
+
+}  // namespace prs

@@ -204,10 +204,12 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 // stage s-1 has just produced (stage 0: loaded two iterations ahead), x+-1 by warp shuffles, phidot
 // from what stage s-1 produced one iteration earlier (stage 0: loaded).  Block = 128 threads.
 // ------------------------------------------------------------------------------------------------
+constexpr int TBS2D_L2_AHEAD = 8;
+
 template <typename T, int ARITH, int S>
 __global__ void __launch_bounds__(128)
 step2d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
-                  T* __restrict__ phidot_out, int N, int YC, StepCoefs<T, S> coefs) {
+                  T* __restrict__ phidot_out, int N, int YC, int l2_ahead, StepCoefs<T, S> coefs) {
     using K = Pk<T>;
     using V = typename K::V;
     using std::integral_constant;
@@ -243,57 +245,84 @@ step2d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     };
     int io = y0 * NQ + q;
 
-    // rows a = 0, 1 into the window of stage 0; rows 2, 3 and phidot rows 1, 2 in flight
-    V wprev[S], wcur[S], qcur[S];
+    // Everything that rotates does so by static indices (no register moves): the phi rows a = j..j+3
+    // of stage 0 sit in a four-slot ring A (slot a & 3), its phidot rows j+1..j+3 in the ring P; the
+    // two-deep windows w[s] and the phidot hand-over h[s] of the later stages alternate by the parity of
+    // j.  The steady loop is unrolled four times so that every slot number is a compile-time constant.
+    V A[4], P[4], w[S][2], h[S][2];
 #pragma unroll
-    for (int s = 0; s < S; ++s) { wprev[s] = zero; wcur[s] = zero; qcur[s] = zero; }
-    wprev[0] = __ldg(gA + il); advance();
-    wcur[0] = __ldg(gA + il);
-    V pd0 = __ldg(gP + il); advance();                               // phidot of row 1 (stage 0 at j = 0)
-    V a1 = __ldg(gA + il), pd1 = __ldg(gP + il); advance();          // row 2: y+1 of j = 0, phidot of j = 1
-    V a2 = __ldg(gA + il), pd2 = __ldg(gP + il); advance();          // row 3
+    for (int s = 0; s < S; ++s) { w[s][0] = zero; w[s][1] = zero; h[s][0] = zero; h[s][1] = zero; }
+    A[0] = __ldg(gA + il); advance();
+    A[1] = __ldg(gA + il); P[1] = __ldg(gP + il); advance();
+    A[2] = __ldg(gA + il); P[2] = __ldg(gP + il); advance();
+    A[3] = __ldg(gA + il); P[3] = __ldg(gP + il); advance();
+    P[0] = zero;
+    // a second cursor l2_ahead rows past the load cursor pulls those rows into L2, so that the
+    // register loads (two iterations ahead of their use) see L2 latency rather than DRAM latency
+    int ypf = wrap_mod(y0 - S + 4 + l2_ahead, N);
+    int ipf = ypf * NQ + q;
+    int pf_to_wrap = N - ypf;
+    auto prefetch_ahead = [&]() {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(gA + ipf));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(gP + ipf));
+        ipf += NQ;
+        if (--pf_to_wrap == 0) { ipf -= N * NQ; pf_to_wrap = N; }
+    };
 
-    auto iteration = [&](auto act_tag) {
+    auto iteration = [&](auto u_tag, auto act_tag) {
+        constexpr int U = decltype(u_tag)::value & 3, PAR = U & 1;
         constexpr int ACT = decltype(act_tag)::value;
-        // loads two iterations ahead: row a = j+4 (past the last needed row this re-reads harmlessly)
-        const V a3 = __ldg(gA + il), pd3 = __ldg(gP + il); advance();
-        V carry, qout[S];
-        {   // stage 0 on row a = j+1
-            const T left = __shfl_up_sync(0xffffffffu, K::last(wcur[0]), 1);
-            const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[0]), 1);
-            V out;
-            packed_vector_update<T, 2, ARITH>(pc[0], wcur[0], left, right, wprev[0], a1, zero, zero, pd0, out, qout[0]);
-            wprev[0] = wcur[0]; wcur[0] = a1; carry = out;
+        V carry;
+        {   // stage 0 on row a = j+1: rows j, j+1, j+2 of the ring, phidot row j+1
+            const V& cur = A[(U + 1) & 3];
+            const T left = __shfl_up_sync(0xffffffffu, K::last(cur), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(cur), 1);
+            packed_vector_update<T, 2, ARITH>(pc[0], cur, left, right, A[U], A[(U + 2) & 3], zero, zero,
+                                              P[(U + 1) & 3], carry, h[1 % S][PAR ^ 1]);
         }
+        // loads two iterations ahead: row a = j+4 takes the slot of row j (past the last needed row
+        // this re-reads harmlessly)
+        A[U] = __ldg(gA + il); P[U] = __ldg(gP + il); advance();
+        prefetch_ahead();
         static_for<1, ACT>([&](auto s_tag) {                         // stage s on row a = j+1-s
             constexpr int s = decltype(s_tag)::value;
-            const T left = __shfl_up_sync(0xffffffffu, K::last(wcur[s]), 1);
-            const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[s]), 1);
+            const V& cur = w[s][PAR ^ 1];
+            const T left = __shfl_up_sync(0xffffffffu, K::last(cur), 1);
+            const T right = __shfl_down_sync(0xffffffffu, K::first(cur), 1);
             V out;
-            packed_vector_update<T, 2, ARITH>(pc[s], wcur[s], left, right, wprev[s], carry, zero, zero, qcur[s], out, qout[s]);
             if constexpr (s == S - 1) {
+                V qo;
+                packed_vector_update<T, 2, ARITH>(pc[s], cur, left, right, w[s][PAR], carry, zero, zero, h[s][PAR], out, qo);
                 if (store_ok) {
-                    oP[io] = qout[s];
+                    oP[io] = qo;
                     oA[io] = out;
                 }
                 io += NQ;
+            } else {
+                packed_vector_update<T, 2, ARITH>(pc[s], cur, left, right, w[s][PAR], carry, zero, zero, h[s][PAR], out,
+                                                  h[s + 1][PAR ^ 1]);
             }
-            wprev[s] = wcur[s]; wcur[s] = carry; carry = out;
+            w[s][PAR] = carry; carry = out;
         });
-        if constexpr (ACT < S) {                 // feed the window of the stage that has not started yet
-            wprev[ACT] = wcur[ACT]; wcur[ACT] = carry;
-        }
-        static_for<1, (ACT < S ? ACT + 1 : S)>([&](auto s_tag) {
-            constexpr int s = decltype(s_tag)::value;
-            qcur[s] = qout[s - 1];
-        });
-        a1 = a2; a2 = a3; pd0 = pd1; pd1 = pd2; pd2 = pd3;
+        if constexpr (ACT < S) w[ACT][PAR] = carry;   // feed the window of the stage that has not started yet
     };
-    static_for<0, 2 * S - 2>([&](auto j_tag) {
+    // start-up: stage s joins at iteration 2s; then single iterations up to a multiple of four
+    constexpr int J0 = (2 * S - 2 + 3) / 4 * 4;
+    static_for<0, J0>([&](auto j_tag) {
         constexpr int j = decltype(j_tag)::value;
-        iteration(integral_constant<int, j / 2 + 1>{});
+        constexpr int ACT = (j / 2 + 1 < S) ? j / 2 + 1 : S;
+        if (j < niter) iteration(integral_constant<int, j>{}, integral_constant<int, ACT>{});
     });
-    for (int j = 2 * S - 2; j < niter; ++j) iteration(integral_constant<int, S>{});
+    int j = J0;
+    for (; j + 4 <= niter; j += 4) {
+        iteration(integral_constant<int, 0>{}, integral_constant<int, S>{});
+        iteration(integral_constant<int, 1>{}, integral_constant<int, S>{});
+        iteration(integral_constant<int, 2>{}, integral_constant<int, S>{});
+        iteration(integral_constant<int, 3>{}, integral_constant<int, S>{});
+    }
+    if (j < niter) iteration(integral_constant<int, 0>{}, integral_constant<int, S>{});
+    if (j + 1 < niter) iteration(integral_constant<int, 1>{}, integral_constant<int, S>{});
+    if (j + 2 < niter) iteration(integral_constant<int, 2>{}, integral_constant<int, S>{});
 }
 
 }  // namespace prs

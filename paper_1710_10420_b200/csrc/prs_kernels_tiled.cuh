@@ -14,6 +14,7 @@
 #pragma once
 
 #include "prs_arith.cuh"
+#include "prs_kernels_generic.cuh"   // warp_reduce / block_reduce
 
 namespace prs {
 

@@ -1,0 +1,58 @@
+// prs_launch_tb2.cuh -- grid sizing and launch of the two-step kernels (prs_kernels_tb2.cuh).
+// Included only by the translation unit that instantiates them (prs_instances.cu).
+#pragma once
+
+#include <algorithm>
+
+#include "prs_host.cuh"
+#include "prs_kernels_tb2.cuh"
+
+namespace prs {
+
+template <typename T, int ARITH, int TY>
+cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
+                             const StepCoef<T>& k2) {
+    constexpr int W = Pk<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    const size_t smem = tb2_smem_bytes<T, TY>();
+    static bool configured = false;            // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(step3d_tb2_kernel<T, ARITH, TY>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const unsigned gx = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT), gy = (unsigned)((N + TY - 1) / TY);
+    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
+    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const dim3 block(32, TY + 4, 1);
+    step3d_tb2_kernel<T, ARITH, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, k1, k2);
+    return cudaGetLastError();
+}
+
+template <typename T, int ARITH>
+cudaError_t launch_tb2_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
+                          const StepCoef<T>& k2) {
+    switch (h->opt_tb2_tile_y) {
+        case 4: return launch_tb2_3d_ty<T, ARITH, 4>(h, p, v, pn, vn, k1, k2);
+        case 8: return launch_tb2_3d_ty<T, ARITH, 8>(h, p, v, pn, vn, k1, k2);
+        case 28: return launch_tb2_3d_ty<T, ARITH, 28>(h, p, v, pn, vn, k1, k2);
+        default: return launch_tb2_3d_ty<T, ARITH, 12>(h, p, v, pn, vn, k1, k2);
+    }
+}
+
+template <typename T, int ARITH>
+cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k1,
+                          const StepCoef<T>& k2) {
+    constexpr int W = Pk<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    const int BX = 128, warps = BX / 32;
+    const unsigned nwarps = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT);
+    const unsigned gx = (nwarps + warps - 1) / warps;
+    int YC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
+    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
+    step2d_tb2_kernel<T, ARITH><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k1, k2);
+    return cudaGetLastError();
+}
+
+}  // namespace prs

@@ -1,0 +1,77 @@
+// prs_launch_tbs.cuh -- grid sizing and launch of the S-step kernels (prs_kernels_tbs.cuh).
+// Included only by the translation unit that instantiates them (prs_instances.cu).
+#pragma once
+
+#include <algorithm>
+
+#include "prs_host.cuh"
+#include "prs_kernels_tbs.cuh"
+
+namespace prs {
+
+// S steps in one pass (n -> n+S); the caller guarantees tbs_supported(h).
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
+    // output rows per CTA: measured 1024^3, chunk 128: FP32 TY = 16 1.21 ms/step (20: 1.25, 12: 1.30);
+    // FP64 TY = 20 2.41 ms/step (16: 2.52, 12: 2.60)
+    constexpr int TY = (sizeof(T) == 8) ? 20 : 16;
+    constexpr int W = Pk<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    StepCoefs<T, S> ks;
+    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
+    const size_t smem = tbs_smem_bytes<T, S, TY>();
+    static bool configured = false;            // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(step3d_tbs_kernel<T, ARITH, S, TY>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    constexpr int XOUT = tbs_xout<T, S>();
+    const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
+    // Chunks of 128 planes: each chunk re-reads 2S halo planes (measured 1024^3 FP32, S = 4: 64 planes
+    // 1.25 ms/step, 128 planes 1.21, 256 planes 1.24 as the grid gets too coarse for 148 SMs).
+    // ... and short enough that the grid covers the chip twice (one CTA per SM) on small lattices.
+    int ZC;
+    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, N);
+    else {
+        const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
+        ZC = (int)std::max<long long>(16, std::min<long long>(128, N / chunks));
+        ZC = std::min<int>(ZC, N);
+    }
+    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const dim3 block(32, TY + 2 * S, 1);
+    step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks);
+    return cudaGetLastError();
+}
+
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
+    constexpr int W = Pk<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    StepCoefs<T, S> ks;
+    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
+    constexpr int XOUT = tbs_xout<T, S>();
+    const int BX = 128, warps = BX / 32;
+    const unsigned nwarps = (unsigned)((NQ + XOUT - 1) / XOUT);
+    const unsigned gx = (nwarps + warps - 1) / warps;
+    // Rows per march: long enough to amortise the 2S halo rows, short enough for ~8 CTAs per SM
+    // (4096^2: 31 rows 0.89 ms per 50 steps, 62 rows 1.03); on launch-bound lattices (256^2: 1.6 us per
+    // step with 8-row marches, 2.6 us with 32) short wins.
+    int YC;
+    if (h->opt_chunk > 0) YC = (int)std::min<int64_t>(h->opt_chunk, N);
+    else {
+        const long long want = 8LL * h->sm_count;
+        long long chunks = (want + gx - 1) / gx;
+        YC = (int)std::max<long long>(8, std::min<long long>(128, N / std::max<long long>(1, chunks)));
+        YC = std::min<int>(YC, N);
+    }
+    const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
+    // rows of L2 prefetch ahead of the load cursor: measured 16384^2 FP32 S = 6, ms per step:
+    // none 0.180, 4 rows 0.154, 8 rows 0.153, 16 rows 0.163, 32 rows 0.215
+    const int l2_ahead = std::min(TBS2D_L2_AHEAD, N);
+    step2d_tbs_kernel<T, ARITH, S><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, l2_ahead, ks);
+    return cudaGetLastError();
+}
+
+}  // namespace prs
