@@ -66,6 +66,10 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     ("3d_1024_f64_rad", "tb2"): 35_594_988_000,
     # profiles/r01a_ncu_step3d_tiled_f32_1024.md: 8.867 GB read + 8.549 GB written per single-step launch
     ("3d_1024_f32_rad", "tiled"): 17_415_889_000,
+    # profiles/r01e_ncu_step2d_tbs8_f32_16384.md: 2.572 GB read + 2.109 GB written per eight-step launch
+    ("2d_16384_f32_rad", "tbs"): 4_680_775_000,
+    # profiles/r01e_ncu_step2d_tbs6_f64_16384.md: 5.133 GB read + 4.260 GB written per six-step launch
+    ("2d_16384_f64_rad", "tbs"): 9_392_606_000,
 }
 
 
