@@ -530,6 +530,14 @@ def test_full_length_runs_match_the_oracle(dims, N, era_m, every):
     assert worst <= 0.02 and abs(mu_g - mu_r) <= 0.02
 
 
+def test_driver_smoke_entry_point_passes():
+    """__graft_entry__.smoke() is what the driver runs on the GPU box before the bench: all four step
+    kernels against the oracle on three small lattices."""
+    import __graft_entry__ as entry
+
+    entry.smoke()
+
+
 # ------------------------------------------------------------------ state handling
 
 def test_copy_in_out_roundtrip_device_and_host_and_step_split():
