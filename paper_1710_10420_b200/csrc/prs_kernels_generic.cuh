@@ -167,84 +167,127 @@ diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, lon
 // Orientation-weighted wall area, Eq. 7 as printed (:59-62; R15): sum over crossing
 // forward links of |grad phi| / (|phi,x| + |phi,y| + |phi,z|), the gradient on the link s -> s+e_k
 // being the forward difference along the link and, across it, the mean of the central differences
-// at the two ends.  Grid-stride over sites; a thread owns the d forward links of its site, tests them
-// on the sign bits and gathers the transverse neighbours (L1 / L2 hits: they lie within one site of
-// what the warp streams anyway) only for links that cross.  (Sums in x, y, z order per site;  All arithmetic in double.  The crossing
-// links are counted again on the way (partials[].links) as a cross-check against the link count.
+// at the two ends.  All arithmetic in double.
+//
+// Thread = one x; it marches L sites along the slowest axis, carrying the value one step ahead, and
+// tests the d forward links of each site on the sign bits.  Crossing links are rare late in a run, so
+// the gathers and the FP64 square root and division would run with a few lanes of a warp active: each
+// warp instead pushes its crossing links (coordinates + direction, 8 bytes) on a small stack in shared
+// memory (ballot + prefix count) and works them off 32 at a time with every lane busy.  The transverse
+// neighbours are L1 / L2 hits: they lie within one site of what the warp streams anyway.  The
+// crossing links are counted again on the way (partials[].links) as a cross-check against a6.
 // ------------------------------------------------------------------------------------------------
+constexpr int WAREA_THREADS = 256;
+constexpr int WAREA_STACK = 64;                  // entries per warp: < 32 left over + up to 32 pushed at once
+
+// Eq. 7's weight of one crossing link; entry = x | y << 20 | z << 40 | k << 60 (site and link axis).
+// The axis is data, different from lane to lane: everything is selected arithmetically, nothing branches.
 template <typename T, int DIMS>
-__global__ void __launch_bounds__(256)
+__device__ __forceinline__ double link_weight(const T* __restrict__ phi, int N, unsigned long long entry) {
+    const int k = (int)(entry >> 60);
+    const int c0 = (int)(entry & 0xfffff), c1 = (int)((entry >> 20) & 0xfffff), c2 = (int)((entry >> 40) & 0xfffff);
+    const long long NN = (long long)N * N;
+    // offset to the periodic neighbour at distance d = -1, 0, +1 along axis a
+    auto hop = [&](int a, int d) -> long long {
+        const int ca = (a == 0) ? c0 : (a == 1 ? c1 : c2);
+        const long long st = (a == 0) ? 1 : (a == 1 ? (long long)N : NN);
+        int w = ca + d;
+        w = (w < 0) ? w + N : (w >= N ? w - N : w);
+        return (long long)(w - ca) * st;
+    };
+    const T* const site = phi + ((long long)c0 + (long long)c1 * N + (long long)c2 * NN);
+    const long long ek = hop(k, 1);
+    // along the link: forward difference; across it: mean of the central differences at the two ends
+    const double gk = __dsub_rn((double)__ldg(site + ek), (double)__ldg(site));
+    auto across = [&](int t) {
+        const long long ep = hop(t, 1), em = hop(t, -1);
+        const double dc = __dmul_rn(__dsub_rn((double)__ldg(site + ep), (double)__ldg(site + em)), 0.5);
+        const double de = __dmul_rn(__dsub_rn((double)__ldg(site + ep + ek), (double)__ldg(site + em + ek)), 0.5);
+        return __dmul_rn(__dadd_rn(dc, de), 0.5);
+    };
+    double g0, g1, g2 = 0.0;                                         // in x, y, z order whatever k is
+    if (DIMS == 2) {
+        const double gt = across(1 - k);
+        g0 = (k == 0) ? gk : gt;
+        g1 = (k == 0) ? gt : gk;
+    } else {
+        const int ta = (k == 0) ? 1 : 0, tb = (k == 2) ? 1 : 2;      // the other two axes, ta < tb
+        const double ga = across(ta), gb = across(tb);
+        g0 = (k == 0) ? gk : ga;
+        g1 = (k == 1) ? gk : (k == 0 ? ga : gb);
+        g2 = (k == 2) ? gk : gb;
+    }
+    const double num = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(g0, g0), __dmul_rn(g1, g1)), __dmul_rn(g2, g2)));
+    const double den = __dadd_rn(__dadd_rn(fabs(g0), fabs(g1)), fabs(g2));
+    return (den == 0.0) ? 1.0 : __ddiv_rn(num, den);
+}
+
+template <typename T, int DIMS>
+__global__ void __launch_bounds__(WAREA_THREADS)
 weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __restrict__ partials) {
     using A = Ar<T>;
+    __shared__ unsigned long long stack_all[WAREA_THREADS / 32][WAREA_STACK];
+    unsigned long long* const stack = stack_all[threadIdx.x >> 5];
+    const unsigned lane = threadIdx.x & 31, lt_mask = (1u << lane) - 1u;
+    int held = 0;                                                    // entries on the warp's stack (uniform)
     DiagPartial acc = {0ull, 0ull, 0.0};
-    // Thread = one x; blockIdx.y = y (3D) or the chunk of rows (2D); blockIdx.z = the chunk of planes
-    // (3D).  The thread marches L sites along the slowest axis, carrying the value one step ahead.
+    // blockIdx.y = y (3D) or the chunk of rows (2D); blockIdx.z = the chunk of planes (3D)
     constexpr int M = DIMS - 1;                                      // march axis
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = x < N;
+    const int xs = live ? x : 0;                                     // lanes past the row idle along on x = 0
     const long long stride[3] = {1, N, (long long)N * N};
-    if (x < N) {
-        int c[3] = {x, (DIMS == 3) ? (int)blockIdx.y : 0, 0};
-        const int m0 = (int)((DIMS == 3) ? blockIdx.z : blockIdx.y) * L;
-        const int m1 = min(m0 + L, N);
-        // value at the site displaced by a along axis i and by b along axis j (periodic)
-        auto at2 = [&](int i, int a, int j, int b) {
-            int q[3] = {c[0], c[1], c[2]};
-            q[i] += a; q[j] += b;
-            long long o = 0;
+    int c[3] = {xs, (DIMS == 3) ? (int)blockIdx.y : 0, 0};
+    const int m0 = (int)((DIMS == 3) ? blockIdx.z : blockIdx.y) * L;
+    const int m1 = min(m0 + L, N);
+    c[M] = m0;
+    // Linear offset o of the site, constant offsets to its x+1 (and y+1) neighbours, and the offset to
+    // the next site of the march (negative at the periodic seam).
+    long long o = 0;
 #pragma unroll
-            for (int m = 0; m < DIMS; ++m) {
-                const int w = (q[m] < 0) ? q[m] + N : (q[m] >= N ? q[m] - N : q[m]);
-                o += w * stride[m];
-            }
-            return __ldg(phi + o);
-        };
-        c[M] = m0;
-        // Hot path: linear offset o of the site, constant offsets to its x+1 (and y+1) neighbours, and
-        // the offset to the next site of the march (negative at the periodic seam).
-        long long o = 0;
+    for (int m = 0; m < DIMS; ++m) o += c[m] * stride[m];
+    const long long dx = (c[0] == N - 1) ? -(long long)(N - 1) : 1;
+    const long long dy = (DIMS == 3) ? ((c[1] == N - 1) ? -(long long)(N - 1) * N : (long long)N) : 0;
+    auto dm = [&](int m) { return (m == N - 1) ? -(long long)(N - 1) * stride[M] : stride[M]; };
+    auto forward = [&](long long at, int m, T* out) {
+        out[0] = __ldg(phi + at + dx);
+        if (DIMS == 3) out[1] = __ldg(phi + at + dy);
+        out[M] = __ldg(phi + at + dm(m));
+    };
+    auto work_off = [&](int n) {                                     // the top n <= 32 entries of the stack
+        __syncwarp();
+        if ((int)lane < n) acc.sum = __dadd_rn(acc.sum, link_weight<T, DIMS>(phi, N, stack[held - n + (int)lane]));
+        held -= n;
+        __syncwarp();
+    };
+    T pc = __ldg(phi + o);
+    T pe[DIMS], pn[DIMS];
+    forward(o, m0, pe);
+    const unsigned long long site_xy = (unsigned long long)c[0] | ((DIMS == 3) ? ((unsigned long long)c[1] << 20) : 0ull);
+    for (int m = m0; m < m1; ++m) {
+        // the forward neighbours of the next site of the march are requested before this site is
+        // worked on (one iteration of latency hiding; past the end this re-reads harmlessly)
+        const long long on = o + dm(m);
+        forward(on, (m + 1 == N) ? 0 : m + 1, pn);
+        const bool me = A::neg(pc);
+        const unsigned long long site = site_xy | ((unsigned long long)m << (20 * M));
 #pragma unroll
-        for (int m = 0; m < DIMS; ++m) o += c[m] * stride[m];
-        const long long dx = (c[0] == N - 1) ? -(long long)(N - 1) : 1;
-        const long long dy = (DIMS == 3) ? ((c[1] == N - 1) ? -(long long)(N - 1) * N : (long long)N) : 0;
-        auto dm = [&](int m) { return (m == N - 1) ? -(long long)(N - 1) * stride[M] : stride[M]; };
-        auto forward = [&](long long at, int m, T* out) {
-            out[0] = __ldg(phi + at + dx);
-            if (DIMS == 3) out[1] = __ldg(phi + at + dy);
-            out[M] = __ldg(phi + at + dm(m));
-        };
-        T pc = __ldg(phi + o);
-        T pe[DIMS], pn[DIMS];
-        forward(o, m0, pe);
-        for (int m = m0; m < m1; ++m) {
-            // the forward neighbours of the next site of the march are requested before this site is
-            // worked on (one iteration of latency hiding; past the end this re-reads harmlessly)
-            const long long on = o + dm(m);
-            forward(on, (m + 1 == N) ? 0 : m + 1, pn);
-            c[M] = m;
-            const bool me = A::neg(pc);
-#pragma unroll
-            for (int k = 0; k < DIMS; ++k) {
-                if (A::neg(pe[k]) == me) continue;
+        for (int k = 0; k < DIMS; ++k) {
+            const bool cross = live && (A::neg(pe[k]) != me);
+            const unsigned votes = __ballot_sync(0xffffffffu, cross);
+            if (cross) {
                 acc.links += 1;
-                double g[3] = {0.0, 0.0, 0.0};
-                g[k] = __dsub_rn((double)pe[k], (double)pc);
-#pragma unroll
-                for (int t = 0; t < DIMS; ++t) {
-                    if (t == k) continue;
-                    const double dc = __dmul_rn(__dsub_rn((double)at2(t, 1, k, 0), (double)at2(t, -1, k, 0)), 0.5);
-                    const double de = __dmul_rn(__dsub_rn((double)at2(t, 1, k, 1), (double)at2(t, -1, k, 1)), 0.5);
-                    g[t] = __dmul_rn(__dadd_rn(dc, de), 0.5);
-                }
-                const double num = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(g[0], g[0]), __dmul_rn(g[1], g[1])), __dmul_rn(g[2], g[2])));
-                const double den = __dadd_rn(__dadd_rn(fabs(g[0]), fabs(g[1])), fabs(g[2]));
-                acc.sum = __dadd_rn(acc.sum, (den == 0.0) ? 1.0 : __ddiv_rn(num, den));
+                stack[held + __popc(votes & lt_mask)] = site | ((unsigned long long)k << 60);
             }
-            pc = pe[M];                                              // the forward neighbour along the march
-#pragma unroll
-            for (int k = 0; k < DIMS; ++k) pe[k] = pn[k];
-            o = on;
+            held += __popc(votes);
+            if (held >= 32) work_off(32);
         }
+        pc = pe[M];                                                  // the forward neighbour along the march
+#pragma unroll
+        for (int k = 0; k < DIMS; ++k) pe[k] = pn[k];
+        o = on;
     }
+    work_off(held);
     acc = block_reduce(acc);
     if (threadIdx.x == 0)
         partials[blockIdx.x + gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z)] = acc;
