@@ -312,45 +312,48 @@ diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
         const size_t rl = (size_t)y * N + (x == 0 ? N - 1 : x - 1);
         const size_t rr = (size_t)y * N + (x + W >= N ? 0 : x + W);
         const int zprev = (z0 == 0) ? N - 1 : z0 - 1;
+        // Plane offsets are kept incrementally (o_cur = z NN, o_n = (z+1) NN, periodic): no 64-bit
+        // multiplications in the loop.  Everything loaded for plane z+1 (y neighbours, edge scalars) and
+        // z+2 (own column) is turned into sign masks one iteration later, when it has long arrived.
+        size_t o_cur = (size_t)z0 * NN;
+        int zn = (z0 + 1 == N) ? 0 : z0 + 1;
+        size_t o_n = (size_t)zn * NN;
         unsigned m_prev = sign_mask<T>(O::ld(phi + (size_t)zprev * NN + rc));
-        V cur = O::ld(phi + (size_t)z0 * NN + rc);
-        V nxt = O::ld(phi + (size_t)((z0 + 1 == N) ? 0 : z0 + 1) * NN + rc);
-        unsigned m_up = sign_mask<T>(O::ld(phi + (size_t)z0 * NN + rp));
-        unsigned m_dn = sign_mask<T>(O::ld(phi + (size_t)z0 * NN + rm));
-        unsigned s_l = 0, s_r = 0;
-        if (edge_l) s_l = Ar<T>::neg(__ldg(phi + (size_t)z0 * NN + rl));
-        if (edge_r) s_r = Ar<T>::neg(__ldg(phi + (size_t)z0 * NN + rr));
+        V cur = O::ld(phi + o_cur + rc);
+        V nxt = O::ld(phi + o_n + rc);
+        V up = O::ld(phi + o_cur + rp), dn = O::ld(phi + o_cur + rm);
+        T e_l = T(0), e_r = T(0);
+        if (edge_l) e_l = __ldg(phi + o_cur + rl);
+        if (edge_r) e_r = __ldg(phi + o_cur + rr);
+        unsigned m_cur = sign_mask<T>(cur);
         // deferred wall work of the previous plane
         unsigned d_mask = 0;
         V d_c = cur, d_pd = cur;
         for (int z = z0; z < z1; ++z) {
-            V nn = nxt;
-            unsigned m_up_n = m_up, m_dn_n = m_dn, s_l_n = s_l, s_r_n = s_r;
-            const int zn = (z + 1 == N) ? 0 : z + 1;
-            if (z + 1 < z1) {
-                const int znn = (zn + 1 == N) ? 0 : zn + 1;
-                const size_t pn = (size_t)zn * NN;
-                nn = O::ld(phi + (size_t)znn * NN + rc);
-                m_up_n = sign_mask<T>(O::ld(phi + pn + rp));
-                m_dn_n = sign_mask<T>(O::ld(phi + pn + rm));
-                if (edge_l) s_l_n = Ar<T>::neg(__ldg(phi + pn + rl));
-                if (edge_r) s_r_n = Ar<T>::neg(__ldg(phi + pn + rr));
-            }
-            const unsigned m_cur = sign_mask<T>(cur), m_nxt = sign_mask<T>(nxt);
+            // requests for the next iteration (past the end of the chunk these re-read harmlessly)
+            const bool seam = (zn + 1 == N);
+            const size_t o_nn = seam ? 0 : o_n + NN;
+            const V nn = O::ld(phi + o_nn + rc);
+            const V up_n = O::ld(phi + o_n + rp), dn_n = O::ld(phi + o_n + rm);
+            T e_l_n = T(0), e_r_n = T(0);
+            if (edge_l) e_l_n = __ldg(phi + o_n + rl);
+            if (edge_r) e_r_n = __ldg(phi + o_n + rr);
+            const unsigned m_nxt = sign_mask<T>(nxt), m_up = sign_mask<T>(up), m_dn = sign_mask<T>(dn);
             unsigned l = __shfl_up_sync(0xffffffffu, (m_cur >> (W - 1)) & 1u, 1);
             unsigned r = __shfl_down_sync(0xffffffffu, m_cur & 1u, 1);
-            if (edge_l) l = s_l;
-            if (edge_r) r = s_r;
+            if (edge_l) l = Ar<T>::neg(e_l);
+            if (edge_r) r = Ar<T>::neg(e_r);
             unsigned nlinks, wallmask;
             mask_links<W, 3>(m_cur, l, r, m_dn, m_up, m_prev, m_nxt, nlinks, wallmask);
             if (!live) { nlinks = 0; wallmask = 0; }
             acc.links += nlinks;
             V pd_now = cur;
-            if (wallmask) pd_now = O::ld(phidot + (size_t)z * NN + rc);   // consumed next iteration
+            if (wallmask) pd_now = O::ld(phidot + o_cur + rc);       // consumed next iteration
             wq.push(d_mask, d_c, d_pd, V0, I, acc);
             d_mask = wallmask; d_c = cur; d_pd = pd_now;
-            m_prev = m_cur; cur = nxt; nxt = nn;
-            m_up = m_up_n; m_dn = m_dn_n; s_l = s_l_n; s_r = s_r_n;
+            m_prev = m_cur; m_cur = m_nxt; cur = nxt; nxt = nn;
+            up = up_n; dn = dn_n; e_l = e_l_n; e_r = e_r_n;
+            o_cur = o_n; o_n = o_nn; zn = seam ? 0 : zn + 1;
         }
         wq.push(d_mask, d_c, d_pd, V0, I, acc);
         wq.drain(V0, I, acc);
@@ -381,39 +384,43 @@ diag2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
         const bool edge_l = (lane == 0), edge_r = (lane == 31) || (x + W >= N);
         const int xl = (x == 0) ? N - 1 : x - 1, xr = (x + W >= N) ? 0 : x + W;
         const int yprev = (y0 == 0) ? N - 1 : y0 - 1;
+        // row offsets kept incrementally (o_cur = y N, o_n = (y+1) N, periodic), as in the 3D kernel
+        size_t o_cur = (size_t)y0 * N;
+        int yn = (y0 + 1 == N) ? 0 : y0 + 1;
+        size_t o_n = (size_t)yn * N;
         unsigned m_prev = sign_mask<T>(O::ld(phi + (size_t)yprev * N + x));
-        V cur = O::ld(phi + (size_t)y0 * N + x);
-        V nxt = O::ld(phi + (size_t)((y0 + 1 == N) ? 0 : y0 + 1) * N + x);
-        unsigned s_l = 0, s_r = 0;
-        if (edge_l) s_l = Ar<T>::neg(__ldg(phi + (size_t)y0 * N + xl));
-        if (edge_r) s_r = Ar<T>::neg(__ldg(phi + (size_t)y0 * N + xr));
+        V cur = O::ld(phi + o_cur + x);
+        V nxt = O::ld(phi + o_n + x);
+        T e_l = T(0), e_r = T(0);
+        if (edge_l) e_l = __ldg(phi + o_cur + xl);
+        if (edge_r) e_r = __ldg(phi + o_cur + xr);
+        unsigned m_cur = sign_mask<T>(cur);
         unsigned d_mask = 0;
         V d_c = cur, d_pd = cur;
         for (int y = y0; y < y1; ++y) {
-            V nn = nxt;
-            unsigned s_l_n = s_l, s_r_n = s_r;
-            const int yn = (y + 1 == N) ? 0 : y + 1;
-            if (y + 1 < y1) {
-                const int ynn = (yn + 1 == N) ? 0 : yn + 1;
-                nn = O::ld(phi + (size_t)ynn * N + x);
-                if (edge_l) s_l_n = Ar<T>::neg(__ldg(phi + (size_t)yn * N + xl));
-                if (edge_r) s_r_n = Ar<T>::neg(__ldg(phi + (size_t)yn * N + xr));
-            }
-            const unsigned m_cur = sign_mask<T>(cur), m_nxt = sign_mask<T>(nxt);
+            // requests for the next iteration (past the end of the chunk these re-read harmlessly)
+            const bool seam = (yn + 1 == N);
+            const size_t o_nn = seam ? 0 : o_n + N;
+            const V nn = O::ld(phi + o_nn + x);
+            T e_l_n = T(0), e_r_n = T(0);
+            if (edge_l) e_l_n = __ldg(phi + o_n + xl);
+            if (edge_r) e_r_n = __ldg(phi + o_n + xr);
+            const unsigned m_nxt = sign_mask<T>(nxt);
             unsigned l = __shfl_up_sync(0xffffffffu, (m_cur >> (W - 1)) & 1u, 1);
             unsigned r = __shfl_down_sync(0xffffffffu, m_cur & 1u, 1);
-            if (edge_l) l = s_l;
-            if (edge_r) r = s_r;
+            if (edge_l) l = Ar<T>::neg(e_l);
+            if (edge_r) r = Ar<T>::neg(e_r);
             unsigned nlinks, wallmask;
             mask_links<W, 2>(m_cur, l, r, m_prev, m_nxt, m_cur, m_cur, nlinks, wallmask);
             if (!live) { nlinks = 0; wallmask = 0; }
             acc.links += nlinks;
             V pd_now = cur;
-            if (wallmask) pd_now = O::ld(phidot + (size_t)y * N + x);
+            if (wallmask) pd_now = O::ld(phidot + o_cur + x);
             wq.push(d_mask, d_c, d_pd, V0, I, acc);
             d_mask = wallmask; d_c = cur; d_pd = pd_now;
-            m_prev = m_cur; cur = nxt; nxt = nn;
-            s_l = s_l_n; s_r = s_r_n;
+            m_prev = m_cur; m_cur = m_nxt; cur = nxt; nxt = nn;
+            e_l = e_l_n; e_r = e_r_n;
+            o_cur = o_n; o_n = o_nn; yn = seam ? 0 : yn + 1;
         }
         wq.push(d_mask, d_c, d_pd, V0, I, acc);
         wq.drain(V0, I, acc);
