@@ -93,7 +93,9 @@ enum {
     PRS_INFO_KERNEL_LAUNCHES = 1,  /* kernels launched on behalf of this handle since creation     */
     PRS_INFO_STEP_KERNEL     = 2,  /* PRS_KERNEL_* actually used by the last prs_step              */
     PRS_INFO_STEP            = 3,  /* n                                                            */
-    PRS_INFO_DIAG_KERNEL     = 4   /* PRS_KERNEL_* actually used by the last prs_diagnostics       */
+    PRS_INFO_DIAG_KERNEL     = 4,  /* PRS_KERNEL_* actually used by the last prs_diagnostics       */
+    PRS_INFO_HALO_VALID      = 5,  /* slab: steps the halo planes can still feed (0 = exchange)    */
+    PRS_INFO_HALO_PLANES     = 6   /* slab: halo planes per side (4); 0 on a whole lattice         */
 };
 
 /* Bytes of device workspace needed; 0 if the arguments are invalid. */
@@ -151,6 +153,34 @@ int prs_get_info(prs_handle h, int info, int64_t* value);
 /* DEVICE pointers to the current phi^n and phidot^{n-1/2} arrays (valid until the next prs_step /
  * prs_copy_in / prs_init): lets a caller (e.g. a torch tensor view) read the state without a copy. */
 int prs_device_pointers(prs_handle h, void** phi, void** phidot);
+
+/* ---- z slabs: one 3D lattice sharded over several GPUs ("the
+ * bottleneck at larger box sizes will be the amount of memory available") -------------------------------
+ * A slab handle owns the nz planes z_begin <= z < z_begin + nz of a periodic N^3 lattice (N % 4 == 0,
+ * 4 <= nz <= N, 0 <= z_begin < N) plus 4 halo planes below and above them, copies of the neighbouring slabs'
+ * outermost owned planes of BOTH fields.  Eqs. 3-5 are applied to halo sites as well, from the planes
+ * beyond them, so each step uses up one halo plane per side and every owned site sees exactly the
+ * operations of the unsharded lattice: the owned planes stay bit-identical to it.  prs_step(h, k) needs
+ * k <= PRS_INFO_HALO_VALID (else PRS_ERR_STATE); k = 4 is one pass of the four-step kernel.  The caller
+ * moves the halo planes between slabs -- any transport: NCCL send/recv, peer copies over NVLink -- :
+ *   prs_slab_halo_regions  DEVICE pointers into the CURRENT arrays (they change with every prs_step), each
+ *                          *bytes = 4*N*N*sizeof(T) long and contiguous: send[0], send[1] = phi's lowest / highest
+ *                          four owned planes, for the z-1 / z+1 neighbour; recv[0], recv[1] = phi's lower / upper
+ *                          halo, to be filled with the z-1 neighbour's send[1] / the z+1 neighbour's send[0];
+ *                          [2], [3] the same for phidot.  Neighbours are periodic (one slab: itself).
+ *   prs_slab_halo_filled   declares the halo planes current: PRS_INFO_HALO_VALID = 4.
+ * prs_init fills the halo planes itself (the initial condition is a function of the global site), so a
+ * fresh slab can take four steps at once.  prs_diagnostics needs PRS_INFO_HALO_VALID >= 1 and returns this
+ * slab's partial sums (link_count, wall_sites, sum_ratio; rho = link_count / N^3, this slab's share): add
+ * them over the slabs.  prs_copy_out / prs_copy_in move the owned planes, T[nz*N*N]; prs_copy_in leaves
+ * the halo stale.  prs_weighted_area is not available on a slab (PRS_ERR_UNSUPPORTED).  Everything else
+ * as for prs_create. */
+size_t prs_slab_workspace_bytes(int64_t N, int64_t nz, int precision);      /* 0 if args invalid */
+int prs_create_slab(prs_handle* out, int64_t N, int64_t z_begin, int64_t nz, int precision,
+                    double alpha, double era_m, double deta, double W0, double phi0, uint64_t seed,
+                    void* workspace, size_t workspace_bytes, void* cuda_stream);
+int prs_slab_halo_regions(prs_handle h, void* send[4], void* recv[4], size_t* bytes);
+int prs_slab_halo_filled(prs_handle h);
 
 const char* prs_last_error(prs_handle h);
 

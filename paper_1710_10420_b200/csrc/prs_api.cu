@@ -37,9 +37,11 @@ struct Layout {
     size_t field_bytes, off_phi[2], off_pd[2], off_partials, off_result, total;
 };
 
-Layout layout_of(int dims, int64_t N, int precision) {
+constexpr int SLAB_HALO = 4;                 // halo planes per side = the most steps one 3D launch takes
+
+Layout layout_of_sites(size_t sites, int precision) {
     Layout L;
-    L.field_bytes = align_up(sites_of(dims, N) * (precision == PRS_F32 ? 4 : 8));
+    L.field_bytes = align_up(sites * (precision == PRS_F32 ? 4 : 8));
     size_t o = 0;
     L.off_phi[0] = o; o += L.field_bytes;
     L.off_phi[1] = o; o += L.field_bytes;
@@ -50,6 +52,19 @@ Layout layout_of(int dims, int64_t N, int precision) {
     L.total = o;
     return L;
 }
+
+Layout layout_of(int dims, int64_t N, int precision) { return layout_of_sites(sites_of(dims, N), precision); }
+
+// A z slab: 3D, N a multiple of 4 (whole Philox quads and 16-byte vectors per row), at least SLAB_HALO
+// owned planes (a neighbour's halo is filled from one rank only).
+inline bool slab_args_ok(int64_t N, int64_t nz, int64_t z_begin, int precision) {
+    if (!args_ok(3, N, precision)) return false;
+    if (N % 4 != 0) return false;
+    if (nz < SLAB_HALO || nz > N) return false;
+    if (z_begin < 0 || z_begin >= N) return false;
+    return true;
+}
+inline size_t slab_sites(int64_t N, int64_t nz) { return (size_t)N * N * (size_t)(nz + 2 * SLAB_HALO); }
 
 }  // namespace
 
@@ -117,7 +132,7 @@ template <typename T, int DIMS, int ARITH>
 cudaError_t launch_generic(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, const StepCoef<T>& k) {
     const unsigned blocks = (unsigned)((h->S + 255) / 256);
     step_generic_kernel<T, DIMS, ARITH><<<blocks, 256, 0, h->stream>>>(p, v, pn, vn, (long long)h->N,
-                                                                         (long long)h->S, k);
+                                                                         (long long)h->NZ, (long long)h->S, k);
     return cudaGetLastError();
 }
 
@@ -270,6 +285,7 @@ bool diag_tiled_supported(const prs_ctx* h) {
 }
 
 int resolve_diag_kernel(const prs_ctx* h) {
+    if (h->slab) return PRS_KERNEL_GENERIC;
     int want = h->opt_diag_kernel;
     if (want == PRS_KERNEL_AUTO) want = diag_tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
     return want;
@@ -313,13 +329,16 @@ int diag_launch(prs_ctx* h) {
             diag2d_tiled_kernel<T><<<grid, 128, 0, h->stream>>>(p, v, N, YC, V0, I, h->partials);
         }
     } else {
-        blocks = (long long)((h->S + 255) / 256);
+        // a z slab measures its owned planes only (their z neighbours are halo planes, never the wrap)
+        const long long NN = (long long)h->N * h->N;
+        const long long s0 = h->slab ? h->halo * NN : 0, s1 = h->slab ? (h->halo + h->nz_own) * NN : (long long)h->S;
+        blocks = (s1 - s0 + 255) / 256;
         const long long cap = std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 8);
         if (blocks > cap) blocks = cap;
         if (h->dims == 3)
-            diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+            diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->NZ, s0, s1, V0, I, h->partials);
         else
-            diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->S, V0, I, h->partials);
+            diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->NZ, s0, s1, V0, I, h->partials);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics kernel launch");
@@ -340,17 +359,17 @@ size_t prs_workspace_bytes(int dims, int64_t N, int precision) {
     return layout_of(dims, N, precision).total;
 }
 
-int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha, double era_m, double deta,
-               double W0, double phi0, uint64_t seed, void* workspace, size_t workspace_bytes,
-               void* cuda_stream) {
-    if (!out) return PRS_ERR_INVALID_ARG;
-    if (!args_ok(dims, N, precision)) return PRS_ERR_INVALID_ARG;
+// Shared by prs_create and prs_create_slab: checks the physics arguments and the workspace, builds the context
+// over `sites` local sites.
+static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int precision, double alpha, double era_m,
+                         double deta, double W0, double phi0, uint64_t seed, void* workspace, size_t workspace_bytes,
+                         void* cuda_stream) {
     if (!(deta > 0.0) || !(W0 > 0.0) || !(phi0 > 0.0) || !(alpha >= 0.0) || !(era_m >= 0.0))
         return PRS_ERR_INVALID_ARG;
     if (!std::isfinite(deta) || !std::isfinite(W0) || !std::isfinite(phi0) || !std::isfinite(alpha) ||
         !std::isfinite(era_m))
         return PRS_ERR_INVALID_ARG;
-    const Layout L = layout_of(dims, N, precision);
+    const Layout L = layout_of_sites(sites, precision);
     if (!workspace || workspace_bytes < L.total || ((uintptr_t)workspace % ALIGN) != 0) return PRS_ERR_WORKSPACE;
     cudaPointerAttributes attr;
     if (cudaPointerGetAttributes(&attr, workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
@@ -359,7 +378,8 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     }
     prs_ctx* h = new (std::nothrow) prs_ctx();
     if (!h) return PRS_ERR_INVALID_ARG;
-    h->dims = dims; h->precision = precision; h->N = N; h->S = sites_of(dims, N);
+    h->dims = dims; h->precision = precision; h->N = N; h->S = sites;
+    h->slab = false; h->NZ = N; h->nz_own = N; h->halo = 0; h->z_begin = 0; h->halo_valid = 0;
     h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0; h->seed = seed; h->beta = 0.0;
     h->stream = (cudaStream_t)cuda_stream;
     h->ws = (char*)workspace;
@@ -385,6 +405,34 @@ int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha
     return PRS_OK;
 }
 
+int prs_create(prs_handle* out, int dims, int64_t N, int precision, double alpha, double era_m, double deta,
+               double W0, double phi0, uint64_t seed, void* workspace, size_t workspace_bytes,
+               void* cuda_stream) {
+    if (!out) return PRS_ERR_INVALID_ARG;
+    if (!args_ok(dims, N, precision)) return PRS_ERR_INVALID_ARG;
+    return create_common(out, dims, N, sites_of(dims, N), precision, alpha, era_m, deta, W0, phi0, seed, workspace,
+                         workspace_bytes, cuda_stream);
+}
+
+size_t prs_slab_workspace_bytes(int64_t N, int64_t nz, int precision) {
+    if (!slab_args_ok(N, nz, 0, precision)) return 0;
+    return layout_of_sites(slab_sites(N, nz), precision).total;
+}
+
+int prs_create_slab(prs_handle* out, int64_t N, int64_t z_begin, int64_t nz, int precision, double alpha, double era_m,
+                    double deta, double W0, double phi0, uint64_t seed, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream) {
+    if (!out) return PRS_ERR_INVALID_ARG;
+    if (!slab_args_ok(N, nz, z_begin, precision)) return PRS_ERR_INVALID_ARG;
+    const int rc = create_common(out, 3, N, slab_sites(N, nz), precision, alpha, era_m, deta, W0, phi0, seed, workspace,
+                                 workspace_bytes, cuda_stream);
+    if (rc != PRS_OK) return rc;
+    prs_ctx* h = *out;
+    h->slab = true; h->halo = SLAB_HALO; h->nz_own = nz; h->NZ = nz + 2 * SLAB_HALO; h->z_begin = z_begin;
+    h->halo_valid = 0;
+    return PRS_OK;
+}
+
 int prs_destroy(prs_handle h) {
     if (!h) return PRS_ERR_INVALID_ARG;
     if (h->h_result) cudaFreeHost(h->h_result);
@@ -400,7 +448,14 @@ int prs_init(prs_handle h, double eta0) {
     const long long cap = (long long)h->sm_count * 32;
     if (blocks > cap) blocks = cap;
     h->cur = 0;
-    if (h->precision == PRS_F32)
+    if (h->slab) {
+        const long long NN = (long long)h->N * h->N, zg0 = (long long)h->z_begin - h->halo;
+        if (h->precision == PRS_F32)
+            init_slab_kernel<float><<<(unsigned)blocks, 256, 0, h->stream>>>((float*)h->phi[0], (float*)h->pd[0], NN, (long long)h->NZ, (long long)h->N, zg0, h->seed, h->phi0);
+        else
+            init_slab_kernel<double><<<(unsigned)blocks, 256, 0, h->stream>>>((double*)h->phi[0], (double*)h->pd[0], NN, (long long)h->NZ, (long long)h->N, zg0, h->seed, h->phi0);
+        h->halo_valid = (int)h->halo;          // the halo planes were generated too: no exchange needed yet
+    } else if (h->precision == PRS_F32)
         init_kernel<float><<<(unsigned)blocks, 256, 0, h->stream>>>((float*)h->phi[0], (float*)h->pd[0], (long long)h->S, h->seed, h->phi0);
     else
         init_kernel<double><<<(unsigned)blocks, 256, 0, h->stream>>>((double*)h->phi[0], (double*)h->pd[0], (long long)h->S, h->seed, h->phi0);
@@ -414,6 +469,27 @@ int prs_step(prs_handle h, int64_t nsteps) {
     if (!h) return PRS_ERR_INVALID_ARG;
     if (nsteps < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_step: nsteps must be >= 0");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
+    if (h->slab) {
+        // Each step uses up one halo plane per side (the halo sites are advanced redundantly from the
+        // planes beyond them).  nsteps = 4 goes through the four-step kernel, which writes the owned
+        // planes only; fewer through single generic steps over all planes.
+        if (nsteps > h->halo_valid)
+            return fail(h, PRS_ERR_STATE, "prs_step: a slab can advance at most as many steps as its halo is valid for; exchange the halo planes first (prs_slab_halo_regions / prs_slab_halo_filled)");
+        const bool tbs_ok = h->opt_step_kernel != PRS_KERNEL_GENERIC && tbs_supported(h);
+        if (nsteps == SLAB_HALO && tbs_ok) {
+            const int rc = (h->precision == PRS_F32) ? step_many<float>(h, SLAB_HALO) : step_many<double>(h, SLAB_HALO);
+            if (rc != PRS_OK) return rc;
+            h->last_step_kernel = PRS_KERNEL_TBS;
+        } else {
+            for (int64_t i = 0; i < nsteps; ++i) {
+                const int rc = (h->precision == PRS_F32) ? step_once<float>(h, PRS_KERNEL_GENERIC) : step_once<double>(h, PRS_KERNEL_GENERIC);
+                if (rc != PRS_OK) return rc;
+            }
+            if (nsteps > 0) h->last_step_kernel = PRS_KERNEL_GENERIC;
+        }
+        h->halo_valid -= (int)nsteps;
+        return PRS_OK;
+    }
     const int kernel = resolve_step_kernel(h);
     int64_t left = nsteps;
     if (kernel == PRS_KERNEL_CLUSTER) {
@@ -455,6 +531,8 @@ int prs_diagnostics(prs_handle h, prs_diag* out) {
     if (!h) return PRS_ERR_INVALID_ARG;
     if (!out) return fail(h, PRS_ERR_INVALID_ARG, "prs_diagnostics: out is NULL");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_diagnostics: call prs_init or prs_copy_in first");
+    if (h->slab && h->halo_valid < 1)
+        return fail(h, PRS_ERR_STATE, "prs_diagnostics: the slab's halo planes are stale; exchange them first");
     const int rc = (h->precision == PRS_F32) ? diag_launch<float>(h) : diag_launch<double>(h);
     if (rc != PRS_OK) return rc;
     PRS_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, h->stream));
@@ -465,7 +543,8 @@ int prs_diagnostics(prs_handle h, prs_diag* out) {
     d.link_count = h->h_result->links;
     d.wall_sites = h->h_result->walls;
     d.sum_ratio = h->h_result->sum;
-    d.rho = (double)d.link_count / (double)h->S;
+    // a slab reports its own partial sums; rho is its share of the global density (the shares add up)
+    d.rho = (double)d.link_count / (h->slab ? (double)h->N * (double)h->N * (double)h->N : (double)h->S);
     d.gv2 = d.wall_sites ? d.sum_ratio / (2.0 * (double)d.wall_sites) : 0.0;
     *out = d;
     return PRS_OK;
@@ -476,6 +555,7 @@ int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
     if (!area && !rho_weighted) return fail(h, PRS_ERR_INVALID_ARG, "prs_weighted_area: both outputs are NULL");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_weighted_area: call prs_init or prs_copy_in first");
     if (h->N > (1 << 30)) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: N too large");
+    if (h->slab) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: not available on a slab");
     // x across the threads, y (3D) across blockIdx.y, the slowest axis marched in chunks of L sites,
     // L as short as the partials scratch allows (one partial per block).
     const int N = (int)h->N;
@@ -510,9 +590,12 @@ int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
 int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst) {
     if (!h) return PRS_ERR_INVALID_ARG;
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_copy_out: no state yet");
-    const size_t bytes = h->S * (h->precision == PRS_F32 ? 4 : 8);
-    if (phi_dst) PRS_CUDA(h, cudaMemcpyAsync(phi_dst, h->phi[h->cur], bytes, cudaMemcpyDefault, h->stream));
-    if (phidot_dst) PRS_CUDA(h, cudaMemcpyAsync(phidot_dst, h->pd[h->cur], bytes, cudaMemcpyDefault, h->stream));
+    // a slab copies its owned planes (contiguous: z is the slowest axis)
+    const size_t esz = (h->precision == PRS_F32 ? 4 : 8);
+    const size_t bytes = (h->slab ? (size_t)h->N * h->N * h->nz_own : h->S) * esz;
+    const size_t off = h->slab ? (size_t)h->N * h->N * h->halo * esz : 0;
+    if (phi_dst) PRS_CUDA(h, cudaMemcpyAsync(phi_dst, (char*)h->phi[h->cur] + off, bytes, cudaMemcpyDefault, h->stream));
+    if (phidot_dst) PRS_CUDA(h, cudaMemcpyAsync(phidot_dst, (char*)h->pd[h->cur] + off, bytes, cudaMemcpyDefault, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     return PRS_OK;
 }
@@ -522,11 +605,14 @@ int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, doubl
     if (!phi_src || !phidot_src) return fail(h, PRS_ERR_INVALID_ARG, "prs_copy_in: both fields are required");
     if (!(eta0 > 0.0) || !std::isfinite(eta0) || step < 0)
         return fail(h, PRS_ERR_INVALID_ARG, "prs_copy_in: eta0 must be > 0 and step >= 0");
-    const size_t bytes = h->S * (h->precision == PRS_F32 ? 4 : 8);
-    PRS_CUDA(h, cudaMemcpyAsync(h->phi[h->cur], phi_src, bytes, cudaMemcpyDefault, h->stream));
-    PRS_CUDA(h, cudaMemcpyAsync(h->pd[h->cur], phidot_src, bytes, cudaMemcpyDefault, h->stream));
+    const size_t esz = (h->precision == PRS_F32 ? 4 : 8);
+    const size_t bytes = (h->slab ? (size_t)h->N * h->N * h->nz_own : h->S) * esz;
+    const size_t off = h->slab ? (size_t)h->N * h->N * h->halo * esz : 0;
+    PRS_CUDA(h, cudaMemcpyAsync((char*)h->phi[h->cur] + off, phi_src, bytes, cudaMemcpyDefault, h->stream));
+    PRS_CUDA(h, cudaMemcpyAsync((char*)h->pd[h->cur] + off, phidot_src, bytes, cudaMemcpyDefault, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     h->eta0 = eta0; h->step = step; h->inited = true;
+    h->halo_valid = 0;                            // a slab's halo planes now belong to the old state
     return PRS_OK;
 }
 
@@ -545,6 +631,10 @@ int prs_sync(prs_handle h) {
 
 int prs_set_option(prs_handle h, int option, int64_t value) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    if (h->slab && option == PRS_OPT_STEP_KERNEL && value != PRS_KERNEL_AUTO && value != PRS_KERNEL_GENERIC && value != PRS_KERNEL_TBS)
+        return fail(h, PRS_ERR_UNSUPPORTED, "a slab steps with the generic or the four-step kernel");
+    if (h->slab && (option == PRS_OPT_DIAG_KERNEL || option == PRS_OPT_TBS_STEPS) && value != PRS_KERNEL_AUTO && !(option == PRS_OPT_TBS_STEPS && value == SLAB_HALO))
+        return fail(h, PRS_ERR_UNSUPPORTED, "not configurable on a slab");
     switch (option) {
         case PRS_OPT_STEP_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_step_kernel = (int)value; return PRS_OK; }
@@ -607,6 +697,8 @@ int prs_get_info(prs_handle h, int info, int64_t* value) {
         case PRS_INFO_STEP_KERNEL: *value = h->last_step_kernel; return PRS_OK;
         case PRS_INFO_STEP: *value = h->step; return PRS_OK;
         case PRS_INFO_DIAG_KERNEL: *value = h->last_diag_kernel; return PRS_OK;
+        case PRS_INFO_HALO_VALID: *value = h->slab ? h->halo_valid : 0; return PRS_OK;
+        case PRS_INFO_HALO_PLANES: *value = h->slab ? h->halo : 0; return PRS_OK;
         default: return fail(h, PRS_ERR_INVALID_ARG, "unknown info key");
     }
 }
@@ -616,6 +708,31 @@ int prs_device_pointers(prs_handle h, void** phi, void** phidot) {
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_device_pointers: no state yet");
     if (phi) *phi = h->phi[h->cur];
     if (phidot) *phidot = h->pd[h->cur];
+    return PRS_OK;
+}
+
+int prs_slab_halo_regions(prs_handle h, void* send[4], void* recv[4], size_t* bytes) {
+    if (!h || !send || !recv || !bytes) return PRS_ERR_INVALID_ARG;
+    if (!h->slab) return fail(h, PRS_ERR_STATE, "prs_slab_halo_regions: not a slab");
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_slab_halo_regions: no state yet");
+    const size_t plane = (size_t)h->N * h->N * (h->precision == PRS_F32 ? 4 : 8);
+    const size_t H = (size_t)h->halo, nz = (size_t)h->nz_own;
+    char* const f[2] = {(char*)h->phi[h->cur], (char*)h->pd[h->cur]};
+    for (int i = 0; i < 2; ++i) {
+        send[2 * i + 0] = f[i] + H * plane;              // lowest owned planes  -> the z-1 neighbour's upper halo
+        send[2 * i + 1] = f[i] + nz * plane;             // highest owned planes -> the z+1 neighbour's lower halo
+        recv[2 * i + 0] = f[i];                          // lower halo <- the z-1 neighbour's highest owned planes
+        recv[2 * i + 1] = f[i] + (H + nz) * plane;       // upper halo <- the z+1 neighbour's lowest owned planes
+    }
+    *bytes = H * plane;
+    return PRS_OK;
+}
+
+int prs_slab_halo_filled(prs_handle h) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!h->slab) return fail(h, PRS_ERR_STATE, "prs_slab_halo_filled: not a slab");
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_slab_halo_filled: no state yet");
+    h->halo_valid = (int)h->halo;
     return PRS_OK;
 }
 

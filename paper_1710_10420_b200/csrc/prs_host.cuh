@@ -35,6 +35,12 @@ struct prs_ctx {
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;
+    // z slab of a sharded 3D lattice (prs_create_slab): the arrays hold NZ = nz_own + 2*halo planes of
+    // N x N sites, local plane l = global plane (z_begin - halo + l) mod N; S counts the local sites.
+    // halo_valid = how many more steps the halo planes can feed before they must be exchanged again.
+    bool slab;
+    int64_t NZ, nz_own, halo, z_begin;
+    int halo_valid;
     std::string err;
 };
 

@@ -63,13 +63,47 @@ init_kernel(T* __restrict__ phi, T* __restrict__ phidot, long long S, unsigned l
     }
 }
 
+// Initial condition of a z slab (prs_create_slab): local plane l holds global plane (zg0 + l) mod N,
+// halo planes included, so a freshly initialised slab needs no halo exchange.  The Philox counter is
+// the GLOBAL site index >> 2, as in init_kernel: the field does not depend on the decomposition.
+// NN = N*N is a multiple of 4 (the host checks N % 4 == 0).
+template <typename T>
+__global__ void __launch_bounds__(256)
+init_slab_kernel(T* __restrict__ phi, T* __restrict__ phidot, long long NN, long long nplanes, long long N,
+                 long long zg0, unsigned long long seed, double phi0) {
+    const long long qpp = NN >> 2;                                   // quads per plane
+    const long long nquads = qpp * nplanes;
+    const uint2 key = make_uint2((unsigned int)(seed & 0xffffffffull), (unsigned int)(seed >> 32));
+    for (long long ql = blockIdx.x * (long long)blockDim.x + threadIdx.x; ql < nquads;
+         ql += (long long)gridDim.x * blockDim.x) {
+        const long long l = ql / qpp, r = ql - l * qpp;
+        const long long zg = ((zg0 + l) % N + N) % N;
+        const long long q = zg * qpp + r;                            // global quad
+        const uint4 w = philox4x32_10(
+            make_uint4((unsigned int)(q & 0xffffffffll), (unsigned int)((unsigned long long)q >> 32), 0u, 0u), key);
+        const T v0 = init_value_from_word<T>(w.x, phi0), v1 = init_value_from_word<T>(w.y, phi0);
+        const T v2 = init_value_from_word<T>(w.z, phi0), v3 = init_value_from_word<T>(w.w, phi0);
+        if (sizeof(T) == 4) {
+            reinterpret_cast<float4*>(phi)[ql] = make_float4((float)v0, (float)v1, (float)v2, (float)v3);
+            reinterpret_cast<float4*>(phidot)[ql] = make_float4(0.f, 0.f, 0.f, 0.f);
+        } else {
+            reinterpret_cast<double2*>(phi)[2 * ql] = make_double2((double)v0, (double)v1);
+            reinterpret_cast<double2*>(phi)[2 * ql + 1] = make_double2((double)v2, (double)v3);
+            reinterpret_cast<double2*>(phidot)[2 * ql] = make_double2(0.0, 0.0);
+            reinterpret_cast<double2*>(phidot)[2 * ql + 1] = make_double2(0.0, 0.0);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
-// Generic step: one thread per site, neighbours by modulo wrap (Eqs. 3-5).
+// Generic step: one thread per site, neighbours by modulo wrap (Eqs. 3-5).  The lattice is
+// N x N x NZ (NZ = N unless the handle is a z slab of a sharded lattice, prs_create_slab: there the
+// wrap in z only ever feeds the outermost halo planes, which lose their validity with each step anyway).
 // ------------------------------------------------------------------------------------------------
 template <typename T, int DIMS, int ARITH>
 __global__ void __launch_bounds__(256)
 step_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
-                    T* __restrict__ phidot_next, long long N, long long S, StepCoef<T> k) {
+                    T* __restrict__ phidot_next, long long N, long long NZ, long long S, StepCoef<T> k) {
     const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (s >= S) return;
     const long long x = s % N;
@@ -84,8 +118,8 @@ step_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
     if (DIMS == 3) {
         const long long NN = N * N;
         const long long pil = s - z * NN;
-        zmv = phi[pil + (z == 0 ? N - 1 : z - 1) * NN];
-        zpv = phi[pil + (z == N - 1 ? 0 : z + 1) * NN];
+        zmv = phi[pil + (z == 0 ? NZ - 1 : z - 1) * NN];       // NZ planes: N on a cubic lattice, the slab's
+        zpv = phi[pil + (z == NZ - 1 ? 0 : z + 1) * NN];       // planes (halo included) on a z slab
     }
     T pn, vn;
     site_update<T, DIMS, ARITH>(k, phi[s], phi[xm], phi[xp], phi[ym], phi[yp], zmv, zpv, phidot[s], pn, vn);
@@ -130,11 +164,12 @@ __device__ __forceinline__ DiagPartial block_reduce(DiagPartial p) {
 // all 2d links for the wall-site predicate (Eq. 8's N).
 template <typename T, int DIMS>
 __global__ void __launch_bounds__(256)
-diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, long long N, long long S,
-                    double V0, double I, DiagPartial* __restrict__ partials) {
+diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, long long N, long long NZ,
+                    long long s0, long long S, double V0, double I, DiagPartial* __restrict__ partials) {
     using A = Ar<T>;
     DiagPartial acc = {0ull, 0ull, 0.0};
-    for (long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x; s < S;
+    // sites s0 <= s < S of an N x N x NZ lattice (cubic: NZ = N, s0 = 0; z slab: the owned planes)
+    for (long long s = s0 + blockIdx.x * (long long)blockDim.x + threadIdx.x; s < S;
          s += (long long)gridDim.x * blockDim.x) {
         const long long x = s % N;
         const long long yz = s / N;
@@ -150,8 +185,8 @@ diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, lon
         bool zp = false, zm = false;
         if (DIMS == 3) {
             const long long NN = N * N, pil = s - z * NN;
-            zp = A::neg(phi[pil + (z == N - 1 ? 0 : z + 1) * NN]) != me;
-            zm = A::neg(phi[pil + (z == 0 ? N - 1 : z - 1) * NN]) != me;
+            zp = A::neg(phi[pil + (z == NZ - 1 ? 0 : z + 1) * NN]) != me;
+            zm = A::neg(phi[pil + (z == 0 ? NZ - 1 : z - 1) * NN]) != me;
         }
         acc.links += (unsigned)xp + (unsigned)yp + (unsigned)zp;
         if (xp | xm | yp | ym | zp | zm) {

@@ -44,6 +44,14 @@ struct StepCoefs {
     StepCoef<T> k[S];
 };
 
+// z extent of the 3D march: the lattice has nz planes (periodic wrap of the load cursor) and the grid
+// writes planes lo <= z < hi.  Cubic lattice: {N, 0, N}.  z slab of a sharded lattice (prs_create_slab):
+// nz = owned + 2 halo planes, [lo, hi) = the owned planes, so the cursor never wraps.
+struct ZRange {
+    int nz, lo, hi;
+    unsigned wrap;          // nz * (vectors per plane): what the load cursor steps back by at the seam
+};
+
 template <typename T, int S> __host__ __device__ constexpr int tbs_xhalo() { return (S + Pk<T>::W - 1) / Pk<T>::W; }
 template <typename T, int S> __host__ __device__ constexpr int tbs_xout() { return 32 - 2 * tbs_xhalo<T, S>(); }
 template <typename T, int S, int TY>
@@ -54,7 +62,7 @@ constexpr size_t tbs_smem_bytes() {
 template <typename T, int ARITH, int S, int TY>
 __global__ void __launch_bounds__(32 * (TY + 2 * S), 1)
 step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
-                  T* __restrict__ phidot_out, int N, int ZC, StepCoefs<T, S> coefs) {
+                  T* __restrict__ phidot_out, int N, int ZC, StepCoefs<T, S> coefs, ZRange zr) {
     using K = Pk<T>;
     using V = typename K::V;
     using std::integral_constant;
@@ -74,8 +82,8 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const int q = wrap_mod(qraw, NQ);
     const int yraw = TY * (int)blockIdx.y - S + row;
     const int y = wrap_mod(yraw, N);
-    const int z0 = (int)blockIdx.z * ZC;
-    const int zend = min(z0 + ZC, N);
+    const int z0 = zr.lo + (int)blockIdx.z * ZC;
+    const int zend = min(z0 + ZC, zr.hi);
     const int niter = (zend - z0) + 2 * S - 2;                       // >= 2S-1
     const bool store_ok = (yraw < N) && (lane >= XH) && (lane < 32 - XH) && (qraw < NQ);
 
@@ -91,9 +99,9 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     V* const oP = reinterpret_cast<V*>(phidot_out);
     const unsigned NNv = (unsigned)N * (unsigned)NQ;                 // vectors per plane
     const unsigned colv = (unsigned)y * (unsigned)NQ + (unsigned)q;  // this thread's column within a plane
-    int zl = wrap_mod(z0 - S, N);
+    int zl = wrap_mod(z0 - S, zr.nz);
     unsigned il = (unsigned)zl * NNv + colv;                         // load cursor: issue i = plane a = i
-    int left_to_wrap = N - zl;                                       // issues until z wraps to 0
+    int left_to_wrap = zr.nz - zl;                                   // issues until z wraps to 0
     unsigned io = (unsigned)z0 * NNv + colv;                         // store cursor
 
     auto march = [&](auto ns_tag) {
@@ -103,7 +111,7 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
             if (NS >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
             ++ni; il += NNv;
-            if (--left_to_wrap == 0) { il -= (unsigned)N * NNv; left_to_wrap = N; }   // modulo 2^32, exact
+            if (--left_to_wrap == 0) { il -= zr.wrap; left_to_wrap = zr.nz; }   // modulo 2^32, exact
         };
         // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
         issue(0, 3); issue(1, 0); issue(2, 1);

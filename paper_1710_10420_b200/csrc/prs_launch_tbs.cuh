@@ -32,16 +32,22 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     // Chunks of 128 planes: each chunk re-reads 2S halo planes (measured 1024^3 FP32, S = 4: 64 planes
     // 1.25 ms/step, 128 planes 1.21, 256 planes 1.24 as the grid gets too coarse for 148 SMs).
     // ... and short enough that the grid covers the chip twice (one CTA per SM) on small lattices.
+    // z slab (prs_create_slab): the lattice is N x N x (owned + 2 halo) planes and only the owned planes
+    // are written; the S halo planes on either side are what the S stages consume
+    ZRange zr = {N, 0, N, 0u};
+    if (h->slab) zr = {(int)h->NZ, (int)h->halo, (int)(h->halo + h->nz_own), 0u};
+    zr.wrap = (unsigned)zr.nz * ((unsigned)N * (unsigned)NQ);
+    const int nzo = zr.hi - zr.lo;
     int ZC;
-    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, N);
+    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, nzo);
     else {
         const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
-        ZC = (int)std::max<long long>(16, std::min<long long>(128, N / chunks));
-        ZC = std::min<int>(ZC, N);
+        ZC = (int)std::max<long long>(16, std::min<long long>(128, nzo / chunks));
+        ZC = std::min<int>(ZC, nzo);
     }
-    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, TY + 2 * S, 1);
-    step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks);
+    step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
     return cudaGetLastError();
 }
 

@@ -22,7 +22,8 @@ ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WOR
 
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
            "prs_weighted_area", "prs_set_beta", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
-           "prs_device_pointers", "prs_last_error"]
+           "prs_device_pointers", "prs_last_error",
+           "prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled"]
 
 
 class PrsError(RuntimeError):

@@ -1,0 +1,173 @@
+"""GPU parity of the slab-sharded lattice (include/prs.h "z slabs"; paper_1710_10420_b200/sharded.py).
+
+All slabs of a lattice run on the one GPU of the test box, one after the other (their kernels never
+wait on one another; halo planes move by device copies ordered by events).  The bar: after any mix of
+step counts the owned planes of the slabs, put together, equal the unsharded lattice BIT FOR BIT (and so
+the CPU oracle's FMA form), the link and wall-site counts add up exactly, and the velocity sum agrees to
+the rounding of a differently ordered double sum."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import paper_1710_10420_b200 as prs  # noqa: E402
+from oracle import binding as ref  # noqa: E402
+from paper_1710_10420_b200 import sharded  # noqa: E402
+
+STEPS = [4, 4, 1, 3, 4, 2, 5, 13]          # whole passes, remainders, a fresh halo, a used-up one
+
+
+def same_diag(a, b):
+    assert a["link_count"] == b["link_count"] and a["wall_sites"] == b["wall_sites"], (a, b)
+    assert a["step"] == b["step"] and a["eta"] == b["eta"]
+    assert abs(a["sum_ratio"] - b["sum_ratio"]) <= 1e-12 * abs(b["sum_ratio"])
+    assert abs(a["rho"] - b["rho"]) <= 1e-15 and abs(a["gv2"] - b["gv2"]) <= 1e-12 * abs(b["gv2"])
+
+
+@pytest.mark.parametrize("N,world", [(64, 1), (64, 2), (64, 4), (64, 16), (132, 3), (128, 8)])
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("kernel", [prs.KERNEL_AUTO, prs.KERNEL_GENERIC])
+def test_slabs_put_together_equal_the_unsharded_lattice_bitwise(N, world, prec, kernel):
+    kw = dict(seed=11, era_m=2.0)
+    whole = prs.Simulation(3, N, prec, **kw)
+    group = sharded.SlabGroup(N, [0] * world, prec, **kw)
+    for s in group.slabs:
+        s.set_step_kernel(kernel)
+    whole.init(1.0)
+    group.init(1.0)
+    wp, wv = whole.copy_out()
+    gp, gv = group.copy_out()
+    assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes()
+    same_diag(group.diagnostics(), whole.diagnostics())
+    for k in STEPS:
+        whole.step(k)
+        group.step(k)
+        wp, wv = whole.copy_out()
+        gp, gv = group.copy_out()
+        assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes(), k
+        same_diag(group.diagnostics(), whole.diagnostics())
+    if kernel == prs.KERNEL_AUTO:
+        assert all(s.get_info(2) in (prs.KERNEL_TBS, prs.KERNEL_GENERIC) for s in group.slabs)
+    if N <= 64 and world in (1, 4):                # ... and the oracle's FMA form, bit for bit
+        r = ref.RefSim(3, N, prec, arith=ref.ARITH_FMA, **kw)
+        r.init(1.0)
+        r.step(sum(STEPS))
+        rp, rv = r.copy_out()
+        assert gp.tobytes() == rp.tobytes() and gv.tobytes() == rv.tobytes()
+        dr = r.diagnostics()
+        dg = group.diagnostics()
+        assert dg["link_count"] == dr["link_count"] and dg["wall_sites"] == dr["wall_sites"]
+    group.close()
+    whole.close()
+
+
+def binding_step():
+    from paper_1710_10420_b200 import prs as binding
+    return binding.INFO_STEP
+
+
+def test_four_step_kernel_is_what_a_whole_pass_on_a_slab_runs():
+    g = sharded.SlabGroup(128, [0, 0], prs.F32, seed=3)
+    g.init(1.0)
+    before = g.kernel_launches
+    g.step(8)
+    assert g.kernel_launches - before == 2 * 2                         # two passes on each of two slabs
+    assert all(s.get_info(2) == prs.KERNEL_TBS for s in g.slabs)
+    g.step(3)
+    assert all(s.get_info(2) == prs.KERNEL_GENERIC for s in g.slabs)
+    g.close()
+
+
+def test_one_rank_of_a_distributed_job_without_peers():
+    """ShardedSimulation with world = 1 (its own neighbour; no process group needed)."""
+    N = 64
+    whole = prs.Simulation(3, N, prs.F64, seed=5)
+    one = sharded.ShardedSimulation(N, prs.F64, rank=0, world=1, seed=5)
+    whole.init(1.0)
+    one.init(1.0)
+    whole.step(21)
+    one.step(21)
+    wp, wv = whole.copy_out()
+    gp, gv = one.copy_out()
+    assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes()
+    same_diag(one.diagnostics(), whole.diagnostics())
+    one.close()
+    whole.close()
+
+
+def test_restoring_a_slab_from_a_snapshot():
+    N, world = 64, 2
+    a = sharded.SlabGroup(N, [0] * world, prs.F32, seed=9)
+    a.init(1.0)
+    a.step(10)
+    b = sharded.SlabGroup(N, [0] * world, prs.F32, seed=12345)
+    for sa, sb in zip(a.slabs, b.slabs):
+        p, v = sa.copy_out()
+        sb.copy_in(p, v, eta0=1.0, step=10)
+        assert sb.halo_valid == 0                                       # the halo belongs to no state yet
+    a.step(9)
+    b.step(9)
+    ap, av = a.copy_out()
+    bp, bv = b.copy_out()
+    assert ap.tobytes() == bp.tobytes() and av.tobytes() == bv.tobytes()
+    same_diag(a.diagnostics(), b.diagnostics())
+    a.close()
+    b.close()
+
+
+def test_slab_error_paths():
+    s = sharded.SlabSimulation(64, 16, 16, prs.F32)
+    with pytest.raises(prs.PrsError) as e:
+        s.step(1)                                                       # no state yet
+    assert e.value.code == 4
+    with pytest.raises(prs.PrsError) as e:
+        s.halo_regions()
+    assert e.value.code == 4
+    s.init(1.0)
+    assert s.halo_valid == 4
+    with pytest.raises(prs.PrsError) as e:
+        s.step(5)                                                       # more than the halo is good for
+    assert e.value.code == 4
+    s.step(4)
+    assert s.halo_valid == 0
+    with pytest.raises(prs.PrsError) as e:
+        s.step(1)
+    assert e.value.code == 4
+    with pytest.raises(prs.PrsError) as e:
+        s.diagnostics()                                                 # stale halo
+    assert e.value.code == 4
+    with pytest.raises(prs.PrsError) as e:
+        s.weighted_area()
+    assert e.value.code == 2
+    with pytest.raises(prs.PrsError) as e:
+        s.set_step_kernel(prs.KERNEL_TB2)
+    assert e.value.code == 2
+    s.halo_filled()
+    s.step(2)
+    assert s.halo_valid == 2 and s.get_info(binding_step()) == 6
+    s.close()
+    for N, z0, nz in ((66, 0, 16), (64, 0, 3), (64, 64, 16), (64, -1, 16), (64, 0, 65)):
+        with pytest.raises(prs.PrsError):
+            sharded.SlabSimulation(N, z0, nz, prs.F32)
+    whole = prs.Simulation(3, 64, prs.F32)
+    whole.init(1.0)
+    assert whole.get_info(sharded.INFO_HALO_PLANES) == 0
+    assert sharded._slab_lib().prs_slab_halo_filled(whole._h) == 4     # PRS_ERR_STATE: not a slab
+    whole.close()
+
+
+def test_eight_slabs_of_512_cubed_match_the_unsharded_lattice():
+    """A BASELINE.json lattice (512^3 FP32) as eight slabs of 64 planes: what each of eight GPUs would hold."""
+    N, world = 512, 8
+    whole = prs.Simulation(3, N, prs.F32, seed=2)
+    group = sharded.SlabGroup(N, [0] * world, prs.F32, seed=2)
+    whole.init(1.0)
+    group.init(1.0)
+    whole.step(22)
+    group.step(22)
+    wp, wv = whole.copy_out()
+    gp, gv = group.copy_out()
+    assert np.array_equal(gp.view(np.uint32), wp.view(np.uint32)) and np.array_equal(gv.view(np.uint32), wv.view(np.uint32))
+    same_diag(group.diagnostics(), whole.diagnostics())
+    group.close()
+    whole.close()
