@@ -234,6 +234,59 @@ def run_gpu(args):
     dims, N, prec, era_m = CONFIGS[args.config]
     S = N ** dims
     bpu = BYTES_PER_SITE_UPDATE[prec]
+    slabs = args.decomposition == "slabs"
+    if slabs:
+        # Opt-in: ONE lattice as z slabs -- under torchrun one slab per rank, halo planes
+        # over NCCL ("strong" scaling); in a single process --slabs R slabs one after the other on this GPU,
+        # halo planes by device copies: what each of R GPUs would compute, without the NVLink transport.
+        from paper_1710_10420_b200 import sharded
+
+        if dims != 3:
+            raise SystemExit("--decomposition slabs is for the 3D configs")
+        if world > 1:
+            sim = sharded.ShardedSimulation(N, prec, rank=rank, world=world, era_m=era_m, seed=1)
+        else:
+            sim = sharded.SlabGroup(N, [local] * args.slabs, prec, era_m=era_m, seed=1)
+        sim.init(1.0)
+        stream = torch.cuda.current_stream()
+        for _ in range(args.warmup):
+            sim.step(SUBSTEPS)
+            sim.diagnostics()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = sim.kernel_launches
+        barrier()
+        t0.record(stream)
+        for _ in range(args.steps):
+            sim.step(SUBSTEPS)
+            diag = sim.diagnostics()
+        t1.record(stream)
+        barrier()
+        clocks = sampler.stop() if rank == 0 else None
+        (ms_total,), (launches,) = reduce_over_ranks([t0.elapsed_time(t1)], [sim.kernel_launches - l0], world, "cuda")
+        value = S * SUBSTEPS * args.steps / (ms_total * 1e-3)          # one lattice, whatever the number of slabs
+        peak, peak_src = measured_peak_gbs()
+        if rank == 0:
+            print(json.dumps({
+                "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f32" if prec == 0 else "f64", "data": "synthetic",
+                "config": {"workload": args.config, "dims": dims, "N": N, "era_m": era_m, "substeps_per_step": SUBSTEPS,
+                           "diagnostics_per_step": 1,
+                           "parallelism": ("z slabs x%d, one per GPU, halo planes over NCCL" % world) if world > 1
+                           else ("z slabs x%d on one GPU one after the other, halo planes by device copies" % args.slabs),
+                           "l2": "state exceeds L2; no flush needed"},
+                "roofline": {"bound": "hbm", "achieved": value * bpu / 1e9, "peak": peak * world, "unit": "GB/s",
+                             "frac": value * bpu / 1e9 / (peak * world), "traffic": None, "peak_source": peak_src,
+                             "kernel": "whole cycle (steps, halo transport, diagnostics)"},
+                "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
+                "last_diag": {k: diag[k] for k in ("step", "eta", "link_count", "wall_sites", "rho", "gv2")}}))
+        sim.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
     sim = prs.Simulation(dims, N, prec, era_m=era_m, seed=rank + 1)
     if args.kernel:
         sim.set_step_kernel({"generic": prs.KERNEL_GENERIC, "tiled": prs.KERNEL_TILED, "tb2": prs.KERNEL_TB2,
@@ -362,6 +415,9 @@ def main():
     ap.add_argument("--config", default=DEFAULT_CONFIG, choices=sorted(CONFIGS))
     ap.add_argument("--kernel", default=None, choices=["generic", "tiled", "tb2", "tbs"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slabs"],
+                    help="replicas (default; the contract's line) or one lattice as z slabs (opt-in)")
+    ap.add_argument("--slabs", type=int, default=8, help="single process, --decomposition slabs: slabs on this GPU")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -161,7 +161,9 @@ int prs_device_pointers(prs_handle h, void** phi, void** phidot);
  * outermost owned planes of BOTH fields.  Eqs. 3-5 are applied to halo sites as well, from the planes
  * beyond them, so each step uses up one halo plane per side and every owned site sees exactly the
  * operations of the unsharded lattice: the owned planes stay bit-identical to it.  prs_step(h, k) needs
- * k <= PRS_INFO_HALO_VALID (else PRS_ERR_STATE); k = 4 is one pass of the four-step kernel.  The caller
+ * k <= PRS_INFO_HALO_VALID (else PRS_ERR_STATE); k = 4 or 3 is one pass of the multi-step kernel, which
+ * writes the owned planes only and leaves PRS_INFO_HALO_VALID = 0; k = 1, 2 go through the single-step /
+ * two-step kernels over all planes and leave PRS_INFO_HALO_VALID - k.  The caller
  * moves the halo planes between slabs -- any transport: NCCL send/recv, peer copies over NVLink -- :
  *   prs_slab_halo_regions  DEVICE pointers into the CURRENT arrays (they change with every prs_step), each
  *                          *bytes = 4*N*N*sizeof(T) long and contiguous: send[0], send[1] = phi's lowest / highest

@@ -159,12 +159,13 @@ cudaError_t launch_tiled3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     const int N = (int)h->N;
     const int ty = h->opt_tile_y;
     const unsigned gx = (unsigned)((N + 32 * W - 1) / (32 * W)), gy = (unsigned)((N + ty - 1) / ty);
-    const int ZC = pick_chunk(h, (long long)gx * gy, 32 * ty);
-    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const int NZ = (int)h->NZ;                 // = N unless the handle is a z slab: then all its planes are advanced
+    const int ZC = std::min(pick_chunk(h, (long long)gx * gy, 32 * ty), NZ);
+    const dim3 grid(gx, gy, (unsigned)((NZ + ZC - 1) / ZC));
     const dim3 block(32, ty, 1);
-    if (ty == 4) step3d_tiled_kernel<T, ARITH, 4><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
-    else if (ty == 16) step3d_tiled_kernel<T, ARITH, 16><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
-    else step3d_tiled_kernel<T, ARITH, 8><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, ZC, k);
+    if (ty == 4) step3d_tiled_kernel<T, ARITH, 4><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k);
+    else if (ty == 16) step3d_tiled_kernel<T, ARITH, 16><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k);
+    else step3d_tiled_kernel<T, ARITH, 8><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k);
     return cudaGetLastError();
 }
 
@@ -285,7 +286,6 @@ bool diag_tiled_supported(const prs_ctx* h) {
 }
 
 int resolve_diag_kernel(const prs_ctx* h) {
-    if (h->slab) return PRS_KERNEL_GENERIC;
     int want = h->opt_diag_kernel;
     if (want == PRS_KERNEL_AUTO) want = diag_tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
     return want;
@@ -317,10 +317,12 @@ int diag_launch(prs_ctx* h) {
         if (h->dims == 3) {
             constexpr int TY = 4;
             const unsigned gx = (unsigned)((N + 32 * W - 1) / (32 * W)), gy = (unsigned)((N + TY - 1) / TY);
-            const int ZC = diag_chunk(h, (long long)gx * gy);
-            const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+            // a z slab measures its owned planes only (their z neighbours are halo planes, never the wrap)
+            const int NZ = (int)h->NZ, zlo = h->slab ? (int)h->halo : 0, zhi = h->slab ? (int)(h->halo + h->nz_own) : N;
+            const int ZC = std::min(diag_chunk(h, (long long)gx * gy), zhi - zlo);
+            const dim3 grid(gx, gy, (unsigned)((zhi - zlo + ZC - 1) / ZC));
             blocks = (long long)grid.x * grid.y * grid.z;
-            diag3d_tiled_kernel<T, TY><<<grid, dim3(32, TY, 1), 0, h->stream>>>(p, v, N, ZC, V0, I, h->partials);
+            diag3d_tiled_kernel<T, TY><<<grid, dim3(32, TY, 1), 0, h->stream>>>(p, v, N, NZ, zlo, zhi, ZC, V0, I, h->partials);
         } else {
             const unsigned gx = (unsigned)((N + 128 * W - 1) / (128 * W));
             const int YC = diag_chunk(h, gx);
@@ -471,23 +473,34 @@ int prs_step(prs_handle h, int64_t nsteps) {
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
     if (h->slab) {
         // Each step uses up one halo plane per side (the halo sites are advanced redundantly from the
-        // planes beyond them).  nsteps = 4 goes through the four-step kernel, which writes the owned
-        // planes only; fewer through single generic steps over all planes.
+        // planes beyond them).  nsteps = 4 or 3 is one pass of the multi-step kernel, which writes the
+        // owned planes only (the halo is stale afterwards); 1 or 2 go through the single-step / two-step kernels
+        // over all planes (PRS_KERNEL_GENERIC: generic single steps throughout).
         if (nsteps > h->halo_valid)
             return fail(h, PRS_ERR_STATE, "prs_step: a slab can advance at most as many steps as its halo is valid for; exchange the halo planes first (prs_slab_halo_regions / prs_slab_halo_filled)");
         const bool tbs_ok = h->opt_step_kernel != PRS_KERNEL_GENERIC && tbs_supported(h);
-        if (nsteps == SLAB_HALO && tbs_ok) {
-            const int rc = (h->precision == PRS_F32) ? step_many<float>(h, SLAB_HALO) : step_many<double>(h, SLAB_HALO);
+        if ((nsteps == SLAB_HALO || nsteps == 3) && tbs_ok) {
+            const int rc = (h->precision == PRS_F32) ? step_many<float>(h, (int)nsteps) : step_many<double>(h, (int)nsteps);
             if (rc != PRS_OK) return rc;
             h->last_step_kernel = PRS_KERNEL_TBS;
+            h->halo_valid = 0;                    // the multi-step kernel writes the owned planes only
         } else {
-            for (int64_t i = 0; i < nsteps; ++i) {
-                const int rc = (h->precision == PRS_F32) ? step_once<float>(h, PRS_KERNEL_GENERIC) : step_once<double>(h, PRS_KERNEL_GENERIC);
+            // all NZ planes are advanced (the wrap in z feeds only the outermost halo planes, which lose
+            // their validity anyway), so the halo stays good for halo_valid - nsteps more steps
+            int64_t left = nsteps;
+            if (tbs_ok && tb2_supported(h))
+                for (; left >= 2; left -= 2) {
+                    const int rc = (h->precision == PRS_F32) ? step_twice<float>(h) : step_twice<double>(h);
+                    if (rc != PRS_OK) return rc;
+                }
+            const int single = tbs_ok ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
+            for (; left > 0; --left) {
+                const int rc = (h->precision == PRS_F32) ? step_once<float>(h, single) : step_once<double>(h, single);
                 if (rc != PRS_OK) return rc;
             }
-            if (nsteps > 0) h->last_step_kernel = PRS_KERNEL_GENERIC;
+            if (nsteps > 0) h->last_step_kernel = tbs_ok ? (nsteps >= 2 ? PRS_KERNEL_TB2 : PRS_KERNEL_TILED) : PRS_KERNEL_GENERIC;
+            h->halo_valid -= (int)nsteps;
         }
-        h->halo_valid -= (int)nsteps;
         return PRS_OK;
     }
     const int kernel = resolve_step_kernel(h);

@@ -65,7 +65,7 @@ constexpr size_t tb2_smem_bytes() {
 template <typename T, int ARITH, int TY>
 __global__ void __launch_bounds__(32 * (TY + 4), (32 * (TY + 4) > 512) ? 1 : 2)
 step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
-                  T* __restrict__ phidot_out, int N, int ZC, StepCoef<T> k1, StepCoef<T> k2) {
+                  T* __restrict__ phidot_out, int N, int NZ, int ZC, StepCoef<T> k1, StepCoef<T> k2) {
     using K = Pk<T>;
     using V = typename K::V;
     constexpr int W = K::W;
@@ -85,7 +85,7 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const int yraw = TY * (int)blockIdx.y - 2 + row;
     const int y = wrap_mod(yraw, N);
     const int z0 = (int)blockIdx.z * ZC;
-    const int zend = min(z0 + ZC, N);
+    const int zend = min(z0 + ZC, NZ);                                // NZ planes: N, or a slab's (prs_create_slab)
     const int niter = (zend - z0) + 2;                               // >= 3
     const bool store_ok = (yraw < N) && (lane >= 1) && (lane <= TB2_XOUT) && (qraw < NQ);
 
@@ -103,9 +103,9 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const unsigned colv = (unsigned)y * (unsigned)NQ + (unsigned)q;  // this thread's column within a plane
     // One load cursor serves both fields: issue i fetches phi^n plane a = i (z = z0-2+i, periodic)
     // and the phidot plane of the same z, which stage 1 needs one iteration later than phi^n.
-    int zl = wrap_mod(z0 - 2, N);
+    int zl = wrap_mod(z0 - 2, NZ);
     unsigned il = (unsigned)zl * NNv + colv;
-    int left_to_wrap = N - zl;                                       // issues until z wraps to 0
+    int left_to_wrap = NZ - zl;                                      // issues until z wraps to 0
     unsigned io = (unsigned)z0 * NNv + colv;                         // store cursor (plane a = j, from j = 2)
 
     // The three kinds of row run their own march, so that no per-iteration test of the row survives
@@ -120,7 +120,7 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
             if (ROLE >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
             ++ni; il += NNv;
-            if (--left_to_wrap == 0) { il -= (unsigned)N * NNv; left_to_wrap = N; }   // modulo 2^32, exact
+            if (--left_to_wrap == 0) { il -= (unsigned)NZ * NNv; left_to_wrap = NZ; }   // modulo 2^32, exact
         };
         // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
         issue(0, 3); issue(1, 0); issue(2, 1);

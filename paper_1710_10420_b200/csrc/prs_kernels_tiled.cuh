@@ -73,7 +73,7 @@ __device__ __forceinline__ void vector_update(const StepCoef<T>& k, typename Vec
 template <typename T, int ARITH, int TYB>
 __global__ void __launch_bounds__(32 * TYB)
 step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_next,
-                    T* __restrict__ phidot_next, int N, int ZC, StepCoef<T> k) {
+                    T* __restrict__ phidot_next, int N, int NZ, int ZC, StepCoef<T> k) {
     using O = VecOps<T>;
     using V = typename O::V;
     constexpr int W = O::W;
@@ -84,7 +84,7 @@ step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
     const bool live = xraw < N;
     const int x = live ? xraw : N - W;                    // dead lanes shadow a valid address
     const int z0 = blockIdx.z * ZC;
-    const int z1 = min(z0 + ZC, N);
+    const int z1 = min(z0 + ZC, NZ);                       // NZ planes: N, or a slab's (prs_create_slab)
     const size_t NN = (size_t)N * N;
     const int ym = (y == 0) ? N - 1 : y - 1, yp = (y == N - 1) ? 0 : y + 1;
     const size_t rc = (size_t)y * N + x, rm = (size_t)ym * N + x, rp = (size_t)yp * N + x;
@@ -92,8 +92,8 @@ step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
     const size_t rl = (size_t)y * N + (x == 0 ? N - 1 : x - 1);
     const size_t rr = (size_t)y * N + (x + W >= N ? 0 : x + W);
 
-    const int zprev = (z0 == 0) ? N - 1 : z0 - 1;
-    const int znext0 = (z0 + 1 == N) ? 0 : z0 + 1;
+    const int zprev = (z0 == 0) ? NZ - 1 : z0 - 1;
+    const int znext0 = (z0 + 1 == NZ) ? 0 : z0 + 1;
     V prev = O::ld(phi + (size_t)zprev * NN + rc);
     V cur = O::ld(phi + (size_t)z0 * NN + rc);
     V nxt = O::ld(phi + (size_t)znext0 * NN + rc);
@@ -108,9 +108,9 @@ step3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* 
         // ---- issue the loads of iteration z+1 first
         V nn = nxt, up_n = up, dn_n = dn, pd_n = pd;
         T el_n = el, er_n = er;
-        const int zn = (z + 1 == N) ? 0 : z + 1;
+        const int zn = (z + 1 == NZ) ? 0 : z + 1;
         if (z + 1 < z1) {
-            const int znn = (zn + 1 == N) ? 0 : zn + 1;
+            const int znn = (zn + 1 == NZ) ? 0 : zn + 1;
             const size_t pn = (size_t)zn * NN;
             nn = O::ld(phi + (size_t)znn * NN + rc);
             pd_n = O::ld(phidot + pn + rc);
@@ -288,7 +288,7 @@ struct WallQueue {
 
 template <typename T, int TYB>
 __global__ void __launch_bounds__(32 * TYB)
-diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int N, int ZC, double V0, double I,
+diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int N, int NZ, int zlo, int zhi, int ZC, double V0, double I,
                     DiagPartial* __restrict__ partials) {
     using O = VecOps<T>;
     using V = typename O::V;
@@ -303,20 +303,20 @@ diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
     if (y < N) {                                           // warp-uniform
         const bool live = xraw < N;
         const int x = live ? xraw : N - W;
-        const int z0 = blockIdx.z * ZC;
-        const int z1 = min(z0 + ZC, N);
+        const int z0 = zlo + blockIdx.z * ZC;             // planes zlo <= z < zhi of NZ (cubic: 0, N, N;
+        const int z1 = min(z0 + ZC, zhi);                 // a slab: its owned planes)
         const size_t NN = (size_t)N * N;
         const int ym = (y == 0) ? N - 1 : y - 1, yp = (y == N - 1) ? 0 : y + 1;
         const size_t rc = (size_t)y * N + x, rm = (size_t)ym * N + x, rp = (size_t)yp * N + x;
         const bool edge_l = (lane == 0), edge_r = (lane == 31) || (x + W >= N);
         const size_t rl = (size_t)y * N + (x == 0 ? N - 1 : x - 1);
         const size_t rr = (size_t)y * N + (x + W >= N ? 0 : x + W);
-        const int zprev = (z0 == 0) ? N - 1 : z0 - 1;
+        const int zprev = (z0 == 0) ? NZ - 1 : z0 - 1;
         // Plane offsets are kept incrementally (o_cur = z NN, o_n = (z+1) NN, periodic): no 64-bit
         // multiplications in the loop.  Everything loaded for plane z+1 (y neighbours, edge scalars) and
         // z+2 (own column) is turned into sign masks one iteration later, when it has long arrived.
         size_t o_cur = (size_t)z0 * NN;
-        int zn = (z0 + 1 == N) ? 0 : z0 + 1;
+        int zn = (z0 + 1 == NZ) ? 0 : z0 + 1;
         size_t o_n = (size_t)zn * NN;
         unsigned m_prev = sign_mask<T>(O::ld(phi + (size_t)zprev * NN + rc));
         V cur = O::ld(phi + o_cur + rc);
@@ -331,7 +331,7 @@ diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
         V d_c = cur, d_pd = cur;
         for (int z = z0; z < z1; ++z) {
             // requests for the next iteration (past the end of the chunk these re-read harmlessly)
-            const bool seam = (zn + 1 == N);
+            const bool seam = (zn + 1 == NZ);
             const size_t o_nn = seam ? 0 : o_n + NN;
             const V nn = O::ld(phi + o_nn + rc);
             const V up_n = O::ld(phi + o_n + rp), dn_n = O::ld(phi + o_n + rm);

@@ -23,10 +23,11 @@ cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, c
         configured = true;
     }
     const unsigned gx = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT), gy = (unsigned)((N + TY - 1) / TY);
-    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
-    const dim3 grid(gx, gy, (unsigned)((N + ZC - 1) / ZC));
+    const int NZ = (int)h->NZ;                 // = N unless the handle is a z slab: then all its planes are advanced
+    int ZC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, NZ) : (int)std::min<int64_t>(64, NZ);
+    const dim3 grid(gx, gy, (unsigned)((NZ + ZC - 1) / ZC));
     const dim3 block(32, TY + 4, 1);
-    step3d_tb2_kernel<T, ARITH, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, k1, k2);
+    step3d_tb2_kernel<T, ARITH, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k1, k2);
     return cudaGetLastError();
 }
 

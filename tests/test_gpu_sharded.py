@@ -47,7 +47,9 @@ def test_slabs_put_together_equal_the_unsharded_lattice_bitwise(N, world, prec, 
         assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes(), k
         same_diag(group.diagnostics(), whole.diagnostics())
     if kernel == prs.KERNEL_AUTO:
-        assert all(s.get_info(2) in (prs.KERNEL_TBS, prs.KERNEL_GENERIC) for s in group.slabs)
+        assert all(s.get_info(2) in (prs.KERNEL_TBS, prs.KERNEL_TB2, prs.KERNEL_TILED) for s in group.slabs)
+    else:
+        assert all(s.get_info(2) == prs.KERNEL_GENERIC for s in group.slabs)
     if N <= 64 and world in (1, 4):                # ... and the oracle's FMA form, bit for bit
         r = ref.RefSim(3, N, prec, arith=ref.ARITH_FMA, **kw)
         r.init(1.0)
@@ -73,8 +75,14 @@ def test_four_step_kernel_is_what_a_whole_pass_on_a_slab_runs():
     g.step(8)
     assert g.kernel_launches - before == 2 * 2                         # two passes on each of two slabs
     assert all(s.get_info(2) == prs.KERNEL_TBS for s in g.slabs)
-    g.step(3)
-    assert all(s.get_info(2) == prs.KERNEL_GENERIC for s in g.slabs)
+    g.step(3)                                                          # one three-step pass
+    assert all(s.get_info(2) == prs.KERNEL_TBS and s.halo_valid == 0 for s in g.slabs)
+    g.step(2)                                                          # one two-step pass over all planes
+    assert all(s.get_info(2) == prs.KERNEL_TB2 and s.halo_valid == 2 for s in g.slabs)
+    g.step(1)
+    assert all(s.get_info(2) == prs.KERNEL_TILED and s.halo_valid == 1 for s in g.slabs)
+    g.diagnostics()
+    assert all(s.get_info(4) == prs.KERNEL_TILED for s in g.slabs)       # the tiled diagnostics kernel on the owned planes
     g.close()
 
 
@@ -145,6 +153,9 @@ def test_slab_error_paths():
     s.halo_filled()
     s.step(2)
     assert s.halo_valid == 2 and s.get_info(binding_step()) == 6
+    s.halo_filled()
+    s.step(3)                                                           # a three-step pass leaves the halo stale
+    assert s.halo_valid == 0 and s.get_info(binding_step()) == 9
     s.close()
     for N, z0, nz in ((66, 0, 16), (64, 0, 3), (64, 64, 16), (64, -1, 16), (64, 0, 65)):
         with pytest.raises(prs.PrsError):
