@@ -291,6 +291,8 @@ def run_gpu(args):
     if args.kernel:
         sim.set_step_kernel({"generic": prs.KERNEL_GENERIC, "tiled": prs.KERNEL_TILED, "tb2": prs.KERNEL_TB2,
                              "tbs": prs.KERNEL_TBS}[args.kernel])
+    if args.tbs_rows != 1:
+        sim.set_option(binding.OPT_TBS_ROWS, args.tbs_rows)
     sim.init(1.0)
     stream = torch.cuda.current_stream()
 
@@ -390,7 +392,7 @@ def run_gpu(args):
                        "W0": 10.0, "substeps_per_step": SUBSTEPS, "diagnostics_per_step": 1,
                        "parallelism": "replicas x%d (no sharding, no collective)" % world,
                        "l2": "state (%.1f GiB) exceeds L2; no flush needed" % (4 * fbytes / 2 ** 30),
-                       "step_kernel": kernel_name},
+                       "step_kernel": kernel_name, "tbs_rows_per_thread": args.tbs_rows},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((args.config, kernel_name)),
                          "kernel": "step kernel", "launch_ms": launch_ms, "peak_source": peak_src,
@@ -415,6 +417,8 @@ def main():
     ap.add_argument("--config", default=DEFAULT_CONFIG, choices=sorted(CONFIGS))
     ap.add_argument("--kernel", default=None, choices=["generic", "tiled", "tb2", "tbs"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tbs-rows", type=int, default=1, choices=[1, 2],
+                    help="3D multi-step kernel: rows per thread (PRS_OPT_TBS_ROWS; 2 = step3d_tbr_kernel)")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slabs"],
                     help="replicas (default; the contract's line) or one lattice as z slabs (opt-in)")
     ap.add_argument("--slabs", type=int, default=8, help="single process, --decomposition slabs: slabs on this GPU")

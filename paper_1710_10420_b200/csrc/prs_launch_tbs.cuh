@@ -6,8 +6,12 @@
 
 #include "prs_host.cuh"
 #include "prs_kernels_tbs.cuh"
+#include "prs_kernels_tbr.cuh"
 
 namespace prs {
+
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbr_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn);
 
 // S steps in one pass (n -> n+S); the caller guarantees tbs_supported(h).
 template <typename T, int ARITH, int S>
@@ -17,6 +21,7 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     constexpr int TY = (sizeof(T) == 8) ? 20 : 16;
     constexpr int W = Pk<T>::W;
     const int N = (int)h->N, NQ = N / W;
+    if (h->opt_tbs_rows == 2) return launch_tbr_3d<T, ARITH, S>(h, p, v, pn, vn);      // PRS_OPT_TBS_ROWS
     StepCoefs<T, S> ks;
     for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     const size_t smem = tbs_smem_bytes<T, S, TY>();
@@ -48,6 +53,41 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, TY + 2 * S, 1);
     step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+    return cudaGetLastError();
+}
+
+// The same S steps with two rows per thread (prs_kernels_tbr.cuh): 16 warps, tiles of 32 rows.
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbr_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
+    constexpr int TY = 32 - 2 * S;
+    constexpr int W = Pk<T>::W;
+    const int N = (int)h->N, NQ = N / W;
+    StepCoefs<T, S> ks;
+    for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
+    const size_t smem = tbr_smem_bytes<T, S, TY>();
+    static bool configured = false;            // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(step3d_tbr_kernel<T, ARITH, S, TY>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    constexpr int XOUT = tbs_xout<T, S>();
+    const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
+    ZRange zr = {N, 0, N, 0u};
+    if (h->slab) zr = {(int)h->NZ, (int)h->halo, (int)(h->halo + h->nz_own), 0u};
+    zr.wrap = (unsigned)zr.nz * ((unsigned)N * (unsigned)NQ);
+    const int nzo = zr.hi - zr.lo;
+    int ZC;
+    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, nzo);
+    else {
+        const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
+        ZC = (int)std::max<long long>(16, std::min<long long>(128, nzo / chunks));
+        ZC = std::min<int>(ZC, nzo);
+    }
+    const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
+    const dim3 block(32, (TY + 2 * S) / 2, 1);
+    step3d_tbr_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
     return cudaGetLastError();
 }
 

@@ -176,6 +176,34 @@ def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
 
 
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("N", [4, 8, 20, 36, 60, 124, 200])
+@pytest.mark.parametrize("S", [3, 4])
+def test_two_rows_per_thread_kernel_equals_single_steps_bitwise(prec, N, S):
+    """PRS_OPT_TBS_ROWS = 2 (step3d_tbr_kernel): same stages, two adjacent rows of the tile per thread."""
+    phi, pd = fg.random_state(3, N, 6, NP[prec])
+    for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
+        for nsteps in (S, 2 * S + 1, 3 * S + 2):
+            outs = []
+            for kernel, rows in ((prs.KERNEL_TILED, 1), (prs.KERNEL_TBS, 2)):
+                g = prs.Simulation(3, N, prec, era_m=1.0)
+                g.set_step_kernel(kernel)
+                g.set_arith(arith)
+                g.set_option(binding.OPT_TBS_STEPS, S)
+                g.set_option(binding.OPT_TBS_ROWS, rows)
+                g.copy_in(phi, pd, eta0=1.0, step=2)
+                g.step(nsteps)
+                outs.append(g.copy_out())
+                g.close()
+            assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
+            if arith != prs.ARITH_FMA:
+                break
+    g = prs.Simulation(2, 64, prec)
+    with pytest.raises(prs.PrsError):
+        g.set_option(binding.OPT_TBS_ROWS, 2)                        # 3D only
+    g.close()
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("N", [64, 128, 256])
 def test_cluster_resident_kernel_equals_single_steps_bitwise(prec, N):
     """Small-box kernel (state in the shared memory of one 8-CTA cluster, neighbour rows through
