@@ -33,7 +33,7 @@ constexpr size_t tbr_smem_bytes() {
 }
 
 template <typename T, int ARITH, int S, int TY>
-__global__ void __launch_bounds__(16 * (TY + 2 * S), 1)
+__global__ void __launch_bounds__(16 * (TY + 2 * S), (TY + 2 * S <= 16) ? 2 : 1)
 step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int ZC, StepCoefs<T, S> coefs, ZRange zr) {
     using K = Pk<T>;

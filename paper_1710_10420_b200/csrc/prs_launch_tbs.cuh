@@ -57,9 +57,8 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
 }
 
 // The same S steps with two rows per thread (prs_kernels_tbr.cuh): 16 warps, tiles of 32 rows.
-template <typename T, int ARITH, int S>
-cudaError_t launch_tbr_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
-    constexpr int TY = 32 - 2 * S;
+template <typename T, int ARITH, int S, int TY>
+cudaError_t launch_tbr_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     constexpr int W = Pk<T>::W;
     const int N = (int)h->N, NQ = N / W;
     StepCoefs<T, S> ks;
@@ -89,6 +88,13 @@ cudaError_t launch_tbr_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const dim3 block(32, (TY + 2 * S) / 2, 1);
     step3d_tbr_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
     return cudaGetLastError();
+}
+
+template <typename T, int ARITH, int S>
+cudaError_t launch_tbr_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
+    // tiles of 32 rows, one CTA of 512 threads per SM (measured 1024^3 FP32 S = 3: 1.26 ms per step; tiles of
+    // 16 rows, two CTAs of 256 threads per SM: 1.43 -- what the second CTA hides costs less than its halo)
+    return launch_tbr_3d_ty<T, ARITH, S, 32 - 2 * S>(h, p, v, pn, vn);
 }
 
 template <typename T, int ARITH, int S>
