@@ -24,15 +24,20 @@ def same_diag(a, b):
     assert abs(a["rho"] - b["rho"]) <= 1e-15 and abs(a["gv2"] - b["gv2"]) <= 1e-12 * abs(b["gv2"])
 
 
-@pytest.mark.parametrize("N,world", [(64, 1), (64, 2), (64, 4), (64, 16), (132, 3), (128, 8)])
+@pytest.mark.parametrize("N,world", [(4, 1), (8, 2), (12, 3), (20, 5), (64, 1), (64, 2), (64, 4), (64, 16), (132, 3), (128, 8)])
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
-@pytest.mark.parametrize("kernel", [prs.KERNEL_AUTO, prs.KERNEL_GENERIC])
+@pytest.mark.parametrize("kernel", [prs.KERNEL_AUTO, prs.KERNEL_GENERIC, "two rows per thread"])
 def test_slabs_put_together_equal_the_unsharded_lattice_bitwise(N, world, prec, kernel):
     kw = dict(seed=11, era_m=2.0)
     whole = prs.Simulation(3, N, prec, **kw)
     group = sharded.SlabGroup(N, [0] * world, prec, **kw)
+    rows2 = kernel == "two rows per thread"
+    if rows2:
+        kernel = prs.KERNEL_AUTO
     for s in group.slabs:
         s.set_step_kernel(kernel)
+        if rows2:
+            s.set_option(8, 2)                                          # PRS_OPT_TBS_ROWS
     whole.init(1.0)
     group.init(1.0)
     wp, wv = whole.copy_out()
