@@ -134,6 +134,14 @@ def exchange_halo_tensors(send, recv, rank, world, group=None):
             recv[2 * f + 1].copy_(send[2 * f])
             recv[2 * f].copy_(send[2 * f + 1])
         return
+    if send[0].is_cuda and dist.get_backend(group) == "gloo":
+        # gloo moves host memory only: stage the blocks through the host (a transport for boxes without
+        # NCCL between the ranks' GPUs, and for the two-ranks-on-one-GPU test)
+        hs, hr = [t.cpu() for t in send], [t.new_empty(t.shape, device="cpu") for t in recv]
+        exchange_halo_tensors(hs, hr, rank, world, group)
+        for d, h in zip(recv, hr):
+            d.copy_(h)
+        return
     down, up = (rank - 1) % world, (rank + 1) % world
     if group is not None:
         down, up = dist.get_global_rank(group, down), dist.get_global_rank(group, up)
@@ -193,8 +201,9 @@ class ShardedSimulation:
         if self.slab.halo_valid < 1:
             self.exchange()
         d = self.slab.diagnostics()
-        counts = torch.tensor([d["link_count"], d["wall_sites"]], dtype=torch.int64, device=self.slab.device)
-        ratio = torch.tensor([d["sum_ratio"]], dtype=torch.float64, device=self.slab.device)
+        dev = self.slab.device if self.world > 1 and dist.get_backend(self.group) == "nccl" else "cpu"
+        counts = torch.tensor([d["link_count"], d["wall_sites"]], dtype=torch.int64, device=dev)
+        ratio = torch.tensor([d["sum_ratio"]], dtype=torch.float64, device=dev)
         if self.world > 1:
             dist.all_reduce(counts, group=self.group)
             dist.all_reduce(ratio, group=self.group)

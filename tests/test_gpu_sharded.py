@@ -210,3 +210,70 @@ def test_a_long_sharded_run_tracks_the_unsharded_one_exactly(N, world, prec):
     assert 0 < d["link_count"] < 0.2 * N ** 3                            # a network has formed
     group.close()
     whole.close()
+
+
+RANK_WORKER = r"""
+import os, sys
+sys.path.insert(0, %r)
+import numpy as np
+import torch
+import torch.distributed as dist
+import paper_1710_10420_b200 as prs
+from paper_1710_10420_b200 import sharded
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+torch.cuda.set_device(0)
+dist.init_process_group("gloo")
+sim = sharded.ShardedSimulation(%d, prs.F32, seed=5, era_m=2.0)
+sim.init(1.0)
+diags = []
+for k in (4, 9, 2, 6):
+    sim.step(k)
+    diags.append(sim.diagnostics())
+phi, pd = sim.copy_out()
+np.save(os.path.join(%r, "phi%%d.npy" %% rank), phi)
+np.save(os.path.join(%r, "pd%%d.npy" %% rank), pd)
+np.save(os.path.join(%r, "diag%%d.npy" %% rank), np.array([[d["link_count"], d["wall_sites"], d["sum_ratio"]] for d in diags]))
+dist.barrier()
+sim.close()
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_ranks_of_a_distributed_job_share_the_one_gpu(world, tmp_path):
+    """ShardedSimulation as torchrun would start it, one process per rank, all on cuda:0, halo planes and
+    the diagnostics sums over torch.distributed (gloo; blocks staged through the host).  Processes take
+    turns on the GPU; no kernel waits on another."""
+    import os
+    import subprocess
+    import sys
+
+    from tests.test_bench_replicas_cpu import free_port
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    N, port, out = 48, free_port(), str(tmp_path)
+    procs = []
+    for rank in range(world):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", RANK_WORKER % (root, N, out, out, out)], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=600) for p in procs]
+    assert [p.returncode for p in procs] == [0] * world, outs
+    whole = prs.Simulation(3, N, prs.F32, seed=5, era_m=2.0)
+    whole.init(1.0)
+    want = []
+    for k in (4, 9, 2, 6):
+        whole.step(k)
+        d = whole.diagnostics()
+        want.append([d["link_count"], d["wall_sites"], d["sum_ratio"]])
+    wp, wv = whole.copy_out()
+    whole.close()
+    gp = np.concatenate([np.load(os.path.join(out, "phi%d.npy" % r)) for r in range(world)])
+    gv = np.concatenate([np.load(os.path.join(out, "pd%d.npy" % r)) for r in range(world)])
+    assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes()
+    want = np.array(want)
+    for r in range(world):                                               # every rank holds the lattice's sums
+        got = np.load(os.path.join(out, "diag%d.npy" % r))
+        assert np.array_equal(got[:, :2], want[:, :2])
+        assert np.allclose(got[:, 2], want[:, 2], rtol=1e-12, atol=0)
