@@ -107,17 +107,17 @@ cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const int BX = 128, warps = BX / 32;
     const unsigned nwarps = (unsigned)((NQ + XOUT - 1) / XOUT);
     const unsigned gx = (nwarps + warps - 1) / warps;
-    // Rows per march: long enough to amortise the 2S halo rows, short enough for ~8 CTAs per SM
-    // (4096^2: 31 rows 0.89 ms per 50 steps, 62 rows 1.03); on launch-bound lattices (256^2: 1.6 us per
-    // step with 8-row marches, 2.6 us with 32) short wins.
+    // Rows per march: long enough to amortise the 2S halo rows, short enough to fill 148 SMs.  Measured
+    // (B200, us per step, FP32 S = 8 / FP64 S = 6, rows per march 16 | 32 | 64 | 128):
+    //   1024^2   2.06 | 2.13 | 3.34 | 5.90      2.74 | 3.08 | 3.77 | 6.50
+    //   2048^2   4.62 | 4.38 | 5.14 | 5.90      7.88 | 7.21 | 7.60 | 9.91
+    //   4096^2  16.4  | 13.2 | 12.9 | 14.6      27.0 | 22.9 | 20.9 | 22.2
+    // i.e. N/64, between 8 (launch-bound lattices: 256^2 1.6 us per step with 8-row marches, 2.6 with 32) and
+    // 128 (16384^2).  (An earlier rule aimed at 8 CTAs per SM whatever the halo cost and marched 8 rows at
+    // 2048^2: 6.15 us per step.)
     int YC;
     if (h->opt_chunk > 0) YC = (int)std::min<int64_t>(h->opt_chunk, N);
-    else {
-        const long long want = 8LL * h->sm_count;
-        long long chunks = (want + gx - 1) / gx;
-        YC = (int)std::max<long long>(8, std::min<long long>(128, N / std::max<long long>(1, chunks)));
-        YC = std::min<int>(YC, N);
-    }
+    else YC = std::min<int>(N, std::max(8, std::min(128, N / 64)));
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
     // rows of L2 prefetch ahead of the load cursor: measured 16384^2 FP32 S = 6, ms per step:
     // none 0.180, 4 rows 0.154, 8 rows 0.153, 16 rows 0.163, 32 rows 0.215

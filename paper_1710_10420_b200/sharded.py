@@ -24,8 +24,6 @@ from .prs import F32, INFO_KERNEL_LAUNCHES, PrsError, Simulation, lib
 INFO_HALO_VALID, INFO_HALO_PLANES = 5, 6
 HALO = 4                       # planes per side; also the steps of one pass of the four-step kernel
 
-SLAB_EXPORTS = ["prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled"]
-
 
 def _slab_lib():
     L = lib()
