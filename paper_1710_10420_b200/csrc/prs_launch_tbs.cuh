@@ -13,6 +13,31 @@ namespace prs {
 template <typename T, int ARITH, int S>
 cudaError_t launch_tbr_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn);
 
+// Planes per z chunk of the 3D multi-step kernels (one CTA per SM; `tiles` CTAs per chunk layer, nzo
+// planes to write).  Large grids: 128 planes (measured 1024^3 FP32, S = 4: 64 planes 1.25 ms/step, 128 planes
+// 1.21, 256 planes 1.24; each chunk re-reads 2S halo planes).  Grids of a few waves: the chunk count that
+// minimises waves x (planes marched per CTA), because with one CTA per SM a last, nearly empty wave costs
+// as much as a full one -- measured FP32: 256^3 36.6 -> 26.7 us per step (3 chunks of 86 planes = 144 CTAs,
+// one wave, instead of 8 chunks = 384 CTAs, three waves), 512^3 184 -> 173 (8 chunks of 64 instead of 4 of
+// 128: 9 waves of 74 planes instead of 5 of 138).
+inline int tbs_pick_zc(const prs_ctx* h, long long tiles, int nzo, int S) {
+    if (h->opt_chunk > 0) return (int)std::min<int64_t>(h->opt_chunk, nzo);
+    const long long sms = std::max(1, h->sm_count);
+    const int dflt = std::min(nzo, 128);
+    const long long layers = (nzo + dflt - 1) / dflt;
+    if ((tiles * layers + sms - 1) / sms > 12) return dflt;
+    int best = dflt;
+    long long best_cost = -1;
+    for (int c = 1; c <= std::max(1, nzo / 16); ++c) {
+        const int zc = (nzo + c - 1) / c;
+        const long long cnt = (nzo + zc - 1) / zc;
+        const long long waves = (tiles * cnt + sms - 1) / sms;
+        const long long cost = waves * (zc + 2 * S + 2);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = zc; }
+    }
+    return best;
+}
+
 // S steps in one pass (n -> n+S); the caller guarantees tbs_supported(h).
 template <typename T, int ARITH, int S>
 cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
@@ -34,22 +59,13 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     }
     constexpr int XOUT = tbs_xout<T, S>();
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
-    // Chunks of 128 planes: each chunk re-reads 2S halo planes (measured 1024^3 FP32, S = 4: 64 planes
-    // 1.25 ms/step, 128 planes 1.21, 256 planes 1.24 as the grid gets too coarse for 148 SMs).
-    // ... and short enough that the grid covers the chip twice (one CTA per SM) on small lattices.
     // z slab (prs_create_slab): the lattice is N x N x (owned + 2 halo) planes and only the owned planes
     // are written; the S halo planes on either side are what the S stages consume
     ZRange zr = {N, 0, N, 0u};
     if (h->slab) zr = {(int)h->NZ, (int)h->halo, (int)(h->halo + h->nz_own), 0u};
     zr.wrap = (unsigned)zr.nz * ((unsigned)N * (unsigned)NQ);
     const int nzo = zr.hi - zr.lo;
-    int ZC;
-    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, nzo);
-    else {
-        const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
-        ZC = (int)std::max<long long>(16, std::min<long long>(128, nzo / chunks));
-        ZC = std::min<int>(ZC, nzo);
-    }
+    const int ZC = tbs_pick_zc(h, (long long)gx * gy, nzo, S);
     const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, TY + 2 * S, 1);
     step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
@@ -77,13 +93,7 @@ cudaError_t launch_tbr_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     if (h->slab) zr = {(int)h->NZ, (int)h->halo, (int)(h->halo + h->nz_own), 0u};
     zr.wrap = (unsigned)zr.nz * ((unsigned)N * (unsigned)NQ);
     const int nzo = zr.hi - zr.lo;
-    int ZC;
-    if (h->opt_chunk > 0) ZC = (int)std::min<int64_t>(h->opt_chunk, nzo);
-    else {
-        const long long chunks = (2LL * h->sm_count + (long long)gx * gy - 1) / ((long long)gx * gy);
-        ZC = (int)std::max<long long>(16, std::min<long long>(128, nzo / chunks));
-        ZC = std::min<int>(ZC, nzo);
-    }
+    const int ZC = tbs_pick_zc(h, (long long)gx * gy, nzo, S);
     const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, (TY + 2 * S) / 2, 1);
     step3d_tbr_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
