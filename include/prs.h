@@ -23,6 +23,11 @@
  * (handle-owned, valid until the next call on h).  Asynchronous CUDA faults surface at the next
  * synchronising call (prs_diagnostics, prs_copy_out, prs_copy_in, prs_sync).
  * A handle is not thread-safe; distinct handles are independent.
+ *
+ * Devices: a handle belongs to the device that owns its workspace (taken from the pointer at prs_create).
+ * Every call that touches CUDA makes that device current for its duration and restores the caller's current
+ * device before it returns, so one process may drive handles on several devices in any order.  The stream
+ * passed to prs_create must belong to that device.
  */
 #ifndef PRS_H
 #define PRS_H
@@ -37,7 +42,8 @@ extern "C" {
 typedef struct prs_ctx* prs_handle;
 
 enum { PRS_OK = 0, PRS_ERR_INVALID_ARG = 1, PRS_ERR_UNSUPPORTED = 2, PRS_ERR_WORKSPACE = 3,
-       PRS_ERR_STATE = 4, PRS_ERR_CUDA = 5 };
+       PRS_ERR_STATE = 4, PRS_ERR_CUDA = 5,
+       PRS_ERR_NOMEM = 6 };   /* host-side allocation failed (context or the 24 bytes of pinned memory) */
 
 enum { PRS_F32 = 0, PRS_F64 = 1 };
 
@@ -98,7 +104,8 @@ enum {
     PRS_INFO_STEP            = 3,  /* n                                                            */
     PRS_INFO_DIAG_KERNEL     = 4,  /* PRS_KERNEL_* actually used by the last prs_diagnostics       */
     PRS_INFO_HALO_VALID      = 5,  /* slab: steps the halo planes can still feed (0 = exchange)    */
-    PRS_INFO_HALO_PLANES     = 6   /* slab: halo planes per side (4); 0 on a whole lattice         */
+    PRS_INFO_HALO_PLANES     = 6,  /* slab: halo planes per side (4); 0 on a whole lattice         */
+    PRS_INFO_DEVICE          = 7   /* ordinal of the CUDA device that owns the workspace           */
 };
 
 /* Bytes of device workspace needed; 0 if the arguments are invalid. */
@@ -178,13 +185,18 @@ int prs_device_pointers(prs_handle h, void** phi, void** phidot);
  * fresh slab can take four steps at once.  prs_diagnostics needs PRS_INFO_HALO_VALID >= 1 and returns this
  * slab's partial sums (link_count, wall_sites, sum_ratio; rho = link_count / N^3, this slab's share): add
  * them over the slabs.  prs_copy_out / prs_copy_in move the owned planes, T[nz*N*N]; prs_copy_in leaves
- * the halo stale.  prs_weighted_area is not available on a slab (PRS_ERR_UNSUPPORTED).  Everything else
- * as for prs_create. */
+ * the halo stale.  prs_weighted_area needs PRS_INFO_HALO_VALID >= 1 as well and returns the slab's partial sum
+ * (*rho_weighted = *area / N^3, this slab's share): add them over the slabs.  Everything else as for prs_create. */
 size_t prs_slab_workspace_bytes(int64_t N, int64_t nz, int precision);      /* 0 if args invalid */
 int prs_create_slab(prs_handle* out, int64_t N, int64_t z_begin, int64_t nz, int precision,
                     double alpha, double era_m, double deta, double W0, double phi0, uint64_t seed,
                     void* workspace, size_t workspace_bytes, void* cuda_stream);
 int prs_slab_halo_regions(prs_handle h, void* send[4], void* recv[4], size_t* bytes);
+/* Adds the partial diagnostics of the n parts of one lattice (prs_diagnostics of each slab, all of the same step;
+ * HOST pointers) and applies the normalisation of PAPER.md Eqs. 7-8 (:57-66): link_count, wall_sites and sum_ratio
+ * are summed (sum_ratio in the order given), rho = link_count / N^dims, gv2 = sum_ratio / (2 wall_sites) or 0;
+ * step and eta are parts[0]'s.  PRS_ERR_STATE if the parts are of different steps.  Touches no device. */
+int prs_diag_combine(const prs_diag* parts, int n, int dims, int64_t N, prs_diag* out);
 int prs_slab_halo_filled(prs_handle h);
 
 const char* prs_last_error(prs_handle h);

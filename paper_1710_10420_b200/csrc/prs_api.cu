@@ -85,6 +85,11 @@ int cuda_fail(prs_ctx* h, cudaError_t e, const char* where) {
         if (e_ != cudaSuccess) return cuda_fail((h), e_, #call); \
     } while (0)
 
+// Every exported call that touches CUDA runs with the handle's device current (the caller's is restored on return).
+#define PRS_ON_DEVICE(h)                      \
+    DeviceGuard guard_((h)->device);          \
+    if (guard_.err != cudaSuccess) return cuda_fail((h), guard_.err, "cudaSetDevice")
+
 inline int vec_width(int precision) { return precision == PRS_F32 ? 4 : 2; }
 
 bool tiled_supported(const prs_ctx* h) {
@@ -229,12 +234,10 @@ cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int
     for (int s = 0; s < nsteps; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     for (int s = nsteps; s < CLUSTER_MAX_STEPS; ++s) ks.k[s] = ks.k[0];
     const size_t smem = cluster_smem_bytes<T>((int)h->N);
-    static bool configured = false;            // per instantiation
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step2d_cluster_kernel<T, ARITH>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
+    {
+        const cudaError_t e = ensure_dynamic_smem(step2d_cluster_kernel<T, ARITH>, 227 * 1024, h->device, configured);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     step2d_cluster_kernel<T, ARITH><<<CLUSTER_CTAS, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N, nsteps, ks);
     return cudaGetLastError();
@@ -379,7 +382,7 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
         return PRS_ERR_WORKSPACE;
     }
     prs_ctx* h = new (std::nothrow) prs_ctx();
-    if (!h) return PRS_ERR_INVALID_ARG;
+    if (!h) return PRS_ERR_NOMEM;
     h->dims = dims; h->precision = precision; h->N = N; h->S = sites;
     h->slab = false; h->NZ = N; h->nz_own = N; h->halo = 0; h->z_begin = 0; h->halo_valid = 0;
     h->alpha = alpha; h->era_m = era_m; h->deta = deta; h->W0 = W0; h->phi0 = phi0; h->seed = seed; h->beta = 0.0;
@@ -397,12 +400,18 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->opt_tbs_rows = 1;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     h->h_result = nullptr;
-    int dev = attr.device;
-    if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) h->sm_count = 148;
-    if (cudaHostAlloc((void**)&h->h_result, sizeof(DiagPartial), cudaHostAllocDefault) != cudaSuccess) {
+    h->device = attr.device;                      // the device that owns the workspace: all launches go there
+    DeviceGuard guard(h->device);
+    if (guard.err != cudaSuccess) {
         cudaGetLastError();
         delete h;
         return PRS_ERR_CUDA;
+    }
+    if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) h->sm_count = 148;
+    if (cudaHostAlloc((void**)&h->h_result, sizeof(DiagPartial), cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        delete h;
+        return PRS_ERR_NOMEM;
     }
     *out = h;
     return PRS_OK;
@@ -438,6 +447,7 @@ int prs_create_slab(prs_handle* out, int64_t N, int64_t z_begin, int64_t nz, int
 
 int prs_destroy(prs_handle h) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
     if (h->h_result) cudaFreeHost(h->h_result);
     delete h;
     return PRS_OK;
@@ -445,6 +455,7 @@ int prs_destroy(prs_handle h) {
 
 int prs_init(prs_handle h, double eta0) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     if (!(eta0 > 0.0) || !std::isfinite(eta0)) return fail(h, PRS_ERR_INVALID_ARG, "prs_init: eta0 must be > 0");
     const long long nquads = (long long)((h->S + 3) / 4);
     long long blocks = (nquads + 255) / 256;
@@ -470,6 +481,7 @@ int prs_init(prs_handle h, double eta0) {
 
 int prs_step(prs_handle h, int64_t nsteps) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     if (nsteps < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_step: nsteps must be >= 0");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
     if (h->slab) {
@@ -543,6 +555,7 @@ int prs_step(prs_handle h, int64_t nsteps) {
 
 int prs_diagnostics(prs_handle h, prs_diag* out) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     if (!out) return fail(h, PRS_ERR_INVALID_ARG, "prs_diagnostics: out is NULL");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_diagnostics: call prs_init or prs_copy_in first");
     if (h->slab && h->halo_valid < 1)
@@ -566,29 +579,34 @@ int prs_diagnostics(prs_handle h, prs_diag* out) {
 
 int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     if (!area && !rho_weighted) return fail(h, PRS_ERR_INVALID_ARG, "prs_weighted_area: both outputs are NULL");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_weighted_area: call prs_init or prs_copy_in first");
     if (h->N > (1 << 30)) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: N too large");
-    if (h->slab) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: not available on a slab");
+    if (h->slab && h->halo_valid < 1)
+        return fail(h, PRS_ERR_STATE, "prs_weighted_area: the slab's halo planes are stale; exchange them first");
     // x across the threads, y (3D) across blockIdx.y, the slowest axis marched in chunks of L sites,
-    // L as short as the partials scratch allows (one partial per block).
+    // L as short as the partials scratch allows (one partial per block).  A z slab measures its owned planes
+    // (the transverse neighbours of their links lie at most one plane away: halo planes, valid for >= 1 more step).
     const int N = (int)h->N;
+    const int NM = (h->dims == 3) ? (int)h->NZ : N;
+    const int mlo = h->slab ? (int)h->halo : 0, mhi = h->slab ? (int)(h->halo + h->nz_own) : N, span = mhi - mlo;
     const unsigned gx = (unsigned)((N + 255) / 256);
     const long long per_chunk = (long long)gx * (h->dims == 3 ? N : 1);
-    long long chunks = std::max<long long>(1, std::min<long long>(N, MAX_PARTIALS / per_chunk));
-    int L = (int)((N + chunks - 1) / chunks);
-    if (L < 8) L = std::min(8, N);
-    const unsigned nch = (unsigned)((N + L - 1) / L);
+    long long chunks = std::max<long long>(1, std::min<long long>(span, MAX_PARTIALS / per_chunk));
+    int L = (int)((span + chunks - 1) / chunks);
+    if (L < 8) L = std::min(8, span);
+    const unsigned nch = (unsigned)((span + L - 1) / L);
     const dim3 grid = (h->dims == 3) ? dim3(gx, (unsigned)N, nch) : dim3(gx, nch, 1);
     const long long blocks = (long long)grid.x * grid.y * grid.z;
     if (blocks > MAX_PARTIALS) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: lattice too large for the reduction scratch");
     const void* p = h->phi[h->cur];
     if (h->precision == PRS_F32) {
-        if (h->dims == 3) weighted_area_kernel<float, 3><<<grid, 256, 0, h->stream>>>((const float*)p, N, L, h->partials);
-        else weighted_area_kernel<float, 2><<<grid, 256, 0, h->stream>>>((const float*)p, N, L, h->partials);
+        if (h->dims == 3) weighted_area_kernel<float, 3><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, h->partials);
+        else weighted_area_kernel<float, 2><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, h->partials);
     } else {
-        if (h->dims == 3) weighted_area_kernel<double, 3><<<grid, 256, 0, h->stream>>>((const double*)p, N, L, h->partials);
-        else weighted_area_kernel<double, 2><<<grid, 256, 0, h->stream>>>((const double*)p, N, L, h->partials);
+        if (h->dims == 3) weighted_area_kernel<double, 3><<<grid, 256, 0, h->stream>>>((const double*)p, N, NM, mlo, mhi, L, h->partials);
+        else weighted_area_kernel<double, 2><<<grid, 256, 0, h->stream>>>((const double*)p, N, NM, mlo, mhi, L, h->partials);
     }
     PRS_CUDA(h, cudaGetLastError());
     diag_finalize_kernel<<<1, 1024, 0, h->stream>>>(h->partials, (int)blocks, h->d_result);
@@ -597,12 +615,35 @@ int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
     PRS_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     if (area) *area = h->h_result->sum;
-    if (rho_weighted) *rho_weighted = h->h_result->sum / (double)h->S;
+    // a slab reports its own partial sum; rho_weighted is its share of the lattice's density (the shares add up)
+    if (rho_weighted) *rho_weighted = h->h_result->sum / (h->slab ? (double)h->N * (double)h->N * (double)h->N : (double)h->S);
+    return PRS_OK;
+}
+
+int prs_diag_combine(const prs_diag* parts, int n, int dims, int64_t N, prs_diag* out) {
+    if (!parts || !out || n < 1 || (dims != 2 && dims != 3) || N < 1) return PRS_ERR_INVALID_ARG;
+    prs_diag d;
+    d.step = parts[0].step;
+    d.eta = parts[0].eta;
+    d.link_count = 0;
+    d.wall_sites = 0;
+    d.sum_ratio = 0.0;
+    for (int i = 0; i < n; ++i) {
+        if (parts[i].step != d.step) return PRS_ERR_STATE;           // partial sums of different time levels
+        d.link_count += parts[i].link_count;
+        d.wall_sites += parts[i].wall_sites;
+        d.sum_ratio += parts[i].sum_ratio;                           // in the order given: reproducible
+    }
+    const double sites = (dims == 3) ? (double)N * (double)N * (double)N : (double)N * (double)N;
+    d.rho = (double)d.link_count / sites;                            // Eq. 7, Delta A = 1
+    d.gv2 = d.wall_sites ? d.sum_ratio / (2.0 * (double)d.wall_sites) : 0.0;      // Eq. 8
+    *out = d;
     return PRS_OK;
 }
 
 int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_copy_out: no state yet");
     // a slab copies its owned planes (contiguous: z is the slowest axis)
     const size_t esz = (h->precision == PRS_F32 ? 4 : 8);
@@ -616,6 +657,7 @@ int prs_copy_out(prs_handle h, void* phi_dst, void* phidot_dst) {
 
 int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, double eta0, int64_t step) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     if (!phi_src || !phidot_src) return fail(h, PRS_ERR_INVALID_ARG, "prs_copy_in: both fields are required");
     if (!(eta0 > 0.0) || !std::isfinite(eta0) || step < 0)
         return fail(h, PRS_ERR_INVALID_ARG, "prs_copy_in: eta0 must be > 0 and step >= 0");
@@ -639,6 +681,7 @@ int prs_set_beta(prs_handle h, double beta) {
 
 int prs_sync(prs_handle h) {
     if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     return PRS_OK;
 }
@@ -658,7 +701,7 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
                 return PRS_OK;
             }
             if (value == PRS_KERNEL_TBS) {
-                if (!tbs_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the multi-step kernel needs N a multiple of 16 bytes of T and N^d / that < 2^30");
+                if (!tbs_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the multi-step kernel needs N a multiple of 16 bytes of T and at most 2^31 (3D) / fewer than 2^30 (2D) such vectors in the lattice");
                 h->opt_step_kernel = (int)value;
                 return PRS_OK;
             }
@@ -718,6 +761,7 @@ int prs_get_info(prs_handle h, int info, int64_t* value) {
         case PRS_INFO_DIAG_KERNEL: *value = h->last_diag_kernel; return PRS_OK;
         case PRS_INFO_HALO_VALID: *value = h->slab ? h->halo_valid : 0; return PRS_OK;
         case PRS_INFO_HALO_PLANES: *value = h->slab ? h->halo : 0; return PRS_OK;
+        case PRS_INFO_DEVICE: *value = h->device; return PRS_OK;
         default: return fail(h, PRS_ERR_INVALID_ARG, "unknown info key");
     }
 }

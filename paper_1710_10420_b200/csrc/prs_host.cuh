@@ -6,6 +6,7 @@
 
 #include "../../include/prs.h"
 
+#include <atomic>
 #include <cmath>
 #include <cstdint>
 #include <string>
@@ -35,6 +36,8 @@ struct prs_ctx {
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;
+    int device;                               // ordinal of the device that owns the workspace; every exported call
+                                              // makes it current for its duration (DeviceGuard)
     // z slab of a sharded 3D lattice (prs_create_slab): the arrays hold NZ = nz_own + 2*halo planes of
     // N x N sites, local plane l = global plane (z_begin - halo + l) mod N; S counts the local sites.
     // halo_valid = how many more steps the halo planes can feed before they must be exchanged again.
@@ -45,6 +48,38 @@ struct prs_ctx {
 };
 
 namespace prs {
+
+// Makes the handle's device current for the lifetime of the guard and restores the caller's device afterwards,
+// so that one process can drive handles on several devices (SlabGroup) whatever device is current.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) {
+            err = cudaSetDevice(device);
+            switched = (err == cudaSuccess);
+        }
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: it is set once per
+// (kernel instantiation, device).  `done` is the instantiation's own bit mask of devices already configured
+// (devices >= 64 are configured on every launch); setting it twice from two threads is harmless.
+template <typename F>
+inline cudaError_t ensure_dynamic_smem(F* kernel, size_t bytes, int device, std::atomic<unsigned long long>& done) {
+    const unsigned long long bit = (device >= 0 && device < 64) ? (1ull << device) : 0ull;
+    if (bit && (done.load(std::memory_order_acquire) & bit)) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess && bit) done.fetch_or(bit, std::memory_order_release);
+    return e;
+}
 
 // Per-step scalars, Eq. 6 (:55) and the constants of Eq. 1 (:30); all in double, rounded to
 // the field type once.  eta_n = eta0 + n*deta is formed from n each time, never accumulated.

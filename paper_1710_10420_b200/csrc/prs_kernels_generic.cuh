@@ -218,7 +218,7 @@ constexpr int WAREA_STACK = 64;                  // entries per warp: < 32 left 
 // Eq. 7's weight of one crossing link; entry = x | y << 20 | z << 40 | k << 60 (site and link axis).
 // The axis is data, different from lane to lane: everything is selected arithmetically, nothing branches.
 template <typename T, int DIMS>
-__device__ __forceinline__ double link_weight(const T* __restrict__ phi, int N, unsigned long long entry) {
+__device__ __forceinline__ double link_weight(const T* __restrict__ phi, int N, int NM, unsigned long long entry) {
     const int k = (int)(entry >> 60);
     const int c0 = (int)(entry & 0xfffff), c1 = (int)((entry >> 20) & 0xfffff), c2 = (int)((entry >> 40) & 0xfffff);
     const long long NN = (long long)N * N;
@@ -226,8 +226,9 @@ __device__ __forceinline__ double link_weight(const T* __restrict__ phi, int N, 
     auto hop = [&](int a, int d) -> long long {
         const int ca = (a == 0) ? c0 : (a == 1 ? c1 : c2);
         const long long st = (a == 0) ? 1 : (a == 1 ? (long long)N : NN);
+        const int ext = (a == DIMS - 1) ? NM : N;                    // the march axis holds NM sites (a slab: its planes)
         int w = ca + d;
-        w = (w < 0) ? w + N : (w >= N ? w - N : w);
+        w = (w < 0) ? w + ext : (w >= ext ? w - ext : w);
         return (long long)(w - ca) * st;
     };
     const T* const site = phi + ((long long)c0 + (long long)c1 * N + (long long)c2 * NN);
@@ -259,7 +260,9 @@ __device__ __forceinline__ double link_weight(const T* __restrict__ phi, int N, 
 
 template <typename T, int DIMS>
 __global__ void __launch_bounds__(WAREA_THREADS)
-weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __restrict__ partials) {
+weighted_area_kernel(const T* __restrict__ phi, int N, int NM, int mlo, int mhi, int L, DiagPartial* __restrict__ partials) {
+    // the slowest (march) axis holds NM sites, of which mlo <= m < mhi are measured: N, 0, N on a whole lattice; on a
+    // z slab (prs_create_slab) its NZ planes and the owned range, whose z neighbours are halo planes (never the wrap)
     using A = Ar<T>;
     __shared__ unsigned long long stack_all[WAREA_THREADS / 32][WAREA_STACK];
     unsigned long long* const stack = stack_all[threadIdx.x >> 5];
@@ -273,8 +276,8 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __res
     const int xs = live ? x : 0;                                     // lanes past the row idle along on x = 0
     const long long stride[3] = {1, N, (long long)N * N};
     int c[3] = {xs, (DIMS == 3) ? (int)blockIdx.y : 0, 0};
-    const int m0 = (int)((DIMS == 3) ? blockIdx.z : blockIdx.y) * L;
-    const int m1 = min(m0 + L, N);
+    const int m0 = mlo + (int)((DIMS == 3) ? blockIdx.z : blockIdx.y) * L;
+    const int m1 = min(m0 + L, mhi);
     c[M] = m0;
     // Linear offset o of the site, constant offsets to its x+1 (and y+1) neighbours, and the offset to
     // the next site of the march (negative at the periodic seam).
@@ -283,7 +286,7 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __res
     for (int m = 0; m < DIMS; ++m) o += c[m] * stride[m];
     const long long dx = (c[0] == N - 1) ? -(long long)(N - 1) : 1;
     const long long dy = (DIMS == 3) ? ((c[1] == N - 1) ? -(long long)(N - 1) * N : (long long)N) : 0;
-    auto dm = [&](int m) { return (m == N - 1) ? -(long long)(N - 1) * stride[M] : stride[M]; };
+    auto dm = [&](int m) { return (m == NM - 1) ? -(long long)(NM - 1) * stride[M] : stride[M]; };
     auto forward = [&](long long at, int m, T* out) {
         out[0] = __ldg(phi + at + dx);
         if (DIMS == 3) out[1] = __ldg(phi + at + dy);
@@ -291,7 +294,7 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __res
     };
     auto work_off = [&](int n) {                                     // the top n <= 32 entries of the stack
         __syncwarp();
-        if ((int)lane < n) acc.sum = __dadd_rn(acc.sum, link_weight<T, DIMS>(phi, N, stack[held - n + (int)lane]));
+        if ((int)lane < n) acc.sum = __dadd_rn(acc.sum, link_weight<T, DIMS>(phi, N, NM, stack[held - n + (int)lane]));
         held -= n;
         __syncwarp();
     };
@@ -303,7 +306,7 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int L, DiagPartial* __res
         // the forward neighbours of the next site of the march are requested before this site is
         // worked on (one iteration of latency hiding; past the end this re-reads harmlessly)
         const long long on = o + dm(m);
-        forward(on, (m + 1 == N) ? 0 : m + 1, pn);
+        forward(on, (m + 1 == NM) ? 0 : m + 1, pn);
         const bool me = A::neg(pc);
         const unsigned long long site = site_xy | ((unsigned long long)m << (20 * M));
 #pragma unroll

@@ -15,12 +15,10 @@ cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, c
     constexpr int W = Pk<T>::W;
     const int N = (int)h->N, NQ = N / W;
     const size_t smem = tb2_smem_bytes<T, TY>();
-    static bool configured = false;            // per instantiation
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step3d_tb2_kernel<T, ARITH, TY>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
+    {
+        const cudaError_t e = ensure_dynamic_smem(step3d_tb2_kernel<T, ARITH, TY>, smem, h->device, configured);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     const unsigned gx = (unsigned)((NQ + TB2_XOUT - 1) / TB2_XOUT), gy = (unsigned)((N + TY - 1) / TY);
     const int NZ = (int)h->NZ;                 // = N unless the handle is a z slab: then all its planes are advanced

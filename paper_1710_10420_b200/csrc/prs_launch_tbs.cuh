@@ -50,12 +50,10 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     StepCoefs<T, S> ks;
     for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     const size_t smem = tbs_smem_bytes<T, S, TY>();
-    static bool configured = false;            // per instantiation
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step3d_tbs_kernel<T, ARITH, S, TY>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
+    {
+        const cudaError_t e = ensure_dynamic_smem(step3d_tbs_kernel<T, ARITH, S, TY>, smem, h->device, configured);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     constexpr int XOUT = tbs_xout<T, S>();
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
@@ -80,12 +78,10 @@ cudaError_t launch_tbr_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     StepCoefs<T, S> ks;
     for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     const size_t smem = tbr_smem_bytes<T, S, TY>();
-    static bool configured = false;            // per instantiation
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step3d_tbr_kernel<T, ARITH, S, TY>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
+    {
+        const cudaError_t e = ensure_dynamic_smem(step3d_tbr_kernel<T, ARITH, S, TY>, smem, h->device, configured);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     constexpr int XOUT = tbs_xout<T, S>();
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);

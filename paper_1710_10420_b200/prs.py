@@ -17,13 +17,14 @@ ARITH_LITERAL, ARITH_COEF, ARITH_FMA = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_TB2, KERNEL_TBS, KERNEL_CLUSTER = 0, 1, 2, 3, 4, 5
 OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS = 1, 2, 3, 4, 5, 6, 7, 8
 INFO_KERNEL_LAUNCHES, INFO_STEP_KERNEL, INFO_STEP, INFO_DIAG_KERNEL = 1, 2, 3, 4
+INFO_HALO_VALID, INFO_HALO_PLANES, INFO_DEVICE = 5, 6, 7
 ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WORKSPACE",
-             4: "PRS_ERR_STATE", 5: "PRS_ERR_CUDA"}
+             4: "PRS_ERR_STATE", 5: "PRS_ERR_CUDA", 6: "PRS_ERR_NOMEM"}
 
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
            "prs_weighted_area", "prs_set_beta", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
            "prs_device_pointers", "prs_last_error",
-           "prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled"]
+           "prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled", "prs_diag_combine"]
 
 
 class PrsError(RuntimeError):
@@ -66,6 +67,7 @@ def lib():
         L.prs_set_option.argtypes = [vp, ci, i64]
         L.prs_get_info.argtypes = [vp, ci, C.POINTER(i64)]
         L.prs_device_pointers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+        L.prs_diag_combine.argtypes = [C.POINTER(Diag), ci, ci, i64, C.POINTER(Diag)]
         L.prs_last_error.argtypes = [vp]
         L.prs_last_error.restype = C.c_char_p
         _lib = L
@@ -74,6 +76,19 @@ def lib():
 
 def prs_workspace_bytes(dims, N, precision):
     return int(lib().prs_workspace_bytes(dims, N, precision))
+
+
+def diag_combine(parts, dims, N):
+    """prs_diag_combine: the lattice's diagnostics from the partial sums of its slabs (dicts of prs_diag fields)."""
+    arr = (Diag * len(parts))()
+    for a, p in zip(arr, parts):
+        for k in ("step", "eta", "link_count", "wall_sites", "sum_ratio"):       # rho, gv2 are outputs
+            setattr(a, k, p[k])
+    out = Diag()
+    rc = lib().prs_diag_combine(arr, len(parts), dims, N, C.byref(out))
+    if rc != 0:
+        raise PrsError(rc, "prs_diag_combine")
+    return out.as_dict()
 
 
 def _raw_pointer(obj):

@@ -19,7 +19,7 @@ unsharded one only by the order of its double additions.
 """
 import ctypes as C
 
-from .prs import F32, INFO_KERNEL_LAUNCHES, PrsError, Simulation, lib
+from .prs import F32, INFO_KERNEL_LAUNCHES, PrsError, Simulation, diag_combine, lib
 
 INFO_HALO_VALID, INFO_HALO_PLANES = 5, 6
 HALO = 4                       # planes per side; also the steps of one pass of the four-step kernel
@@ -154,14 +154,9 @@ def exchange_halo_tensors(send, recv, rank, world, group=None):
 
 
 def combine_diagnostics(parts, N):
-    """Sums the slabs' partial diagnostics (dicts of prs_diag fields) into the lattice's."""
-    links = sum(int(p["link_count"]) for p in parts)
-    walls = sum(int(p["wall_sites"]) for p in parts)
-    ratio = 0.0
-    for p in parts:
-        ratio += float(p["sum_ratio"])
-    return {"step": parts[0]["step"], "eta": parts[0]["eta"], "link_count": links, "wall_sites": walls,
-            "sum_ratio": ratio, "rho": links / float(N) ** 3, "gv2": ratio / (2.0 * walls) if walls else 0.0}
+    """The lattice's diagnostics from the slabs' partial sums (dicts of prs_diag fields): prs_diag_combine
+    (the sums and the normalisation of Eqs. 7-8 are the library's, not this module's)."""
+    return diag_combine(parts, 3, N)
 
 
 class ShardedSimulation:
@@ -182,8 +177,13 @@ class ShardedSimulation:
         self.slab.init(eta0)
 
     def exchange(self):
+        """Halo transport on the slab's own stream: the blocks are read after the step kernels queued there and
+        the next step is queued behind the copies, whatever torch's current stream is (torch.distributed's
+        point-to-point operations and ``copy_`` order themselves against the CURRENT stream)."""
+        torch = self._torch
         send, recv = self.slab.halo_regions()
-        exchange_halo_tensors(send, recv, self.rank, self.world, self.group)
+        with torch.cuda.device(self.slab.device), torch.cuda.stream(self.slab.stream):
+            exchange_halo_tensors(send, recv, self.rank, self.world, self.group)
         self.slab.halo_filled()
 
     def step(self, nsteps=1):
@@ -208,6 +208,19 @@ class ShardedSimulation:
         links, walls = (int(v) for v in counts.tolist())
         part = dict(d, link_count=links, wall_sites=walls, sum_ratio=float(ratio.item()))
         return combine_diagnostics([part], self.N)
+
+    def weighted_area(self):
+        """(area, rho_weighted) of the whole lattice (Eq. 7 with the orientation weight), on every rank."""
+        torch, dist = self._torch, self._dist
+        if self.slab.halo_valid < 1:
+            self.exchange()
+        area, _ = self.slab.weighted_area()
+        if self.world > 1:
+            dev = self.slab.device if dist.get_backend(self.group) == "nccl" else "cpu"
+            t = torch.tensor([area], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, group=self.group)
+            area = float(t.item())
+        return area, area / float(self.N) ** 3
 
     def copy_out(self):
         """This rank's owned planes: two numpy arrays of shape (nz, N, N)."""
@@ -272,6 +285,15 @@ class SlabGroup:
         if min(s.halo_valid for s in self.slabs) < 1:
             self.exchange()
         return combine_diagnostics([s.diagnostics() for s in self.slabs], self.N)
+
+    def weighted_area(self):
+        """(area, rho_weighted) of the whole lattice: the slabs' partial sums added in slab order."""
+        if min(s.halo_valid for s in self.slabs) < 1:
+            self.exchange()
+        area = 0.0
+        for s in self.slabs:
+            area += s.weighted_area()[0]
+        return area, area / float(self.N) ** 3
 
     def copy_out(self):
         """The whole lattice: two numpy arrays of shape (N, N, N)."""

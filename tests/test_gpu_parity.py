@@ -51,6 +51,38 @@ def test_init_is_byte_identical(dims, N, prec, seed):
     assert not np.any(np.signbit(gv))
 
 
+def test_init_reproduces_the_printed_field_values():
+    """SURVEY.md Appendix B's printed field values (tests/golden/philox_field_values.txt) through prs_init +
+    prs_copy_out: seeds 42 and 0 on a small lattice in both precisions, and the printed block on the 64-bit path
+    (seed 2^32+7, q = 2^32+1, i.e. sites 4q..4q+3) through a z slab of a 4096^3 lattice whose first owned plane
+    z = 1024 starts at site 2^34 (the only way to hold such a site index on one GPU)."""
+    from paper_1710_10420_b200 import sharded
+    from tests.goldenio import read_philox_field_values
+
+    values, blocks = read_philox_field_values()
+    for prec in (prs.F32, prs.F64):
+        for seed in (42, 0):
+            for dims, N in ((2, 8), (3, 4)):
+                g = prs.Simulation(dims, N, prec, seed=seed)
+                g.init(1.0)
+                flat = g.copy_out()[0].ravel()
+                g.close()
+                for sd, site, _, phi in values:
+                    if sd == seed:
+                        assert float(flat[site]) == phi, (prec, seed, site)
+    N, z_begin = 4096, 1024
+    for seed, q, words in blocks:
+        s0 = 4 * q
+        assert z_begin * N * N <= s0 < (z_begin + 4) * N * N
+        slab = sharded.SlabSimulation(N, z_begin, 4, prs.F32, seed=seed)
+        slab.init(1.0)
+        flat = slab.copy_out()[0].ravel()                      # owned planes: global sites z_begin*N*N ...
+        slab.close()
+        off = s0 - z_begin * N * N
+        want = [(2 * (w >> 8) + 1 - (1 << 24)) / float(1 << 24) for w in words]
+        assert [float(v) for v in flat[off:off + 4]] == want
+
+
 # ------------------------------------------------------------------ T2: 20 steps from the seeded state
 
 CASES_2D = [4, 36, 132, 256, 520]

@@ -78,8 +78,9 @@ def test_product_never_imports_the_oracle():
 def test_multiply_adds_are_fused_exactly_where_the_arithmetic_form_says():
     """Bit-for-bit parity with the oracle rests on the machine code doing the operations the form
     names.  ptxas contracts packed mul.rn.f32x2 + add.rn.f32x2 into FFMA2 whatever --fmad says
-    (prs_pack.cuh works around it), so look at the SASS: no FFMA / FFMA2 / DFMA in any step kernel of
-    the COEF form (template argument ARITH = 1), and fused instructions present in every kernel of
+    (prs_pack.cuh works around it), so look at the SASS of EVERY step kernel in the library (generic,
+    tiled, two-step, the multi-step tbs / tbr kernels that are the default path, cluster-resident): no
+    FFMA / FFMA2 / DFMA in any step kernel of the COEF form (template argument ARITH = 1), and fused instructions present in every kernel of
     the FMA form (ARITH = 2).  LITERAL kernels legitimately contain FMAs inside the correctly rounded
     division routine."""
     import shutil
@@ -94,12 +95,24 @@ def test_multiply_adds_are_fused_exactly_where_the_arithmetic_form_says():
     sass = subprocess.run([cuobjdump, "-sass", prs_build.build()], stdout=subprocess.PIPE, text=True, check=True).stdout
     names = sorted(set(re.findall(r"Function : (\S+)", sass)))
     plain = subprocess.run([cufilt] + names, stdout=subprocess.PIPE, text=True, check=True).stdout.splitlines()
-    arith_of = {}
+    arith_of, step_kernels = {}, 0
     for mangled, dem in zip(names, plain):
-        m = re.search(r"prs::step_generic_kernel<\w+, \(int\)\d+, \(int\)(\d)>|prs::step\dd_(?:tiled|tb2)_kernel<\w+, \(int\)(\d)", dem)
-        if m:
-            arith_of[mangled] = int(m.group(1) or m.group(2))
-    assert sorted(set(arith_of.values())) == [0, 1, 2] and len(arith_of) >= 36
+        if not re.search(r"prs::step\w*_kernel<", dem):
+            continue
+        step_kernels += 1
+        # ARITH is the second template argument of every step kernel (single-step tiled, two-step tb2, multi-step
+        # tbs / tbr, cluster-resident) and the third of step_generic_kernel<T, DIMS, ARITH>
+        m = re.search(r"prs::step_generic_kernel<\w+, \(int\)\d+, \(int\)(\d)>", dem) or \
+            re.search(r"prs::step(?:\dd_(?:tiled|tb2|tbs|tbr|cluster|band))_kernel<\w+, \(int\)(\d)[,>]", dem)
+        assert m, "step kernel the test cannot classify: " + dem
+        arith_of[mangled] = int(m.group(1))
+    families = set(re.search(r"prs::(step\w*_kernel)<", d).group(1) for d in plain if re.search(r"prs::step\w*_kernel<", d))
+    for fam in ("step_generic_kernel", "step3d_tiled_kernel", "step2d_tiled_kernel", "step3d_tb2_kernel", "step2d_tb2_kernel",
+                "step3d_tbs_kernel", "step2d_tbs_kernel", "step3d_tbr_kernel", "step2d_cluster_kernel"):
+        assert fam in families, fam
+    assert len(arith_of) == step_kernels >= 120 and sorted(set(arith_of.values())) == [0, 1, 2]
+    for a in (0, 1, 2):                                   # every family is built in every arithmetic form
+        assert sum(1 for v in arith_of.values() if v == a) == step_kernels // 3
     cur, fused = None, {k: 0 for k in arith_of}
     for line in sass.splitlines():
         m = re.search(r"Function : (\S+)", line)

@@ -3,7 +3,7 @@ import numpy as np
 import pytest
 
 from oracle import binding as ref
-from tests.goldenio import read_philox_kat
+from tests.goldenio import read_philox_field_values, read_philox_kat
 
 
 def test_philox_known_answer_vectors():
@@ -11,6 +11,34 @@ def test_philox_known_answer_vectors():
     assert len(kats) == 3
     for ctr, key, want in kats:
         assert ref.philox4x32_10(ctr, key) == want
+
+
+def test_printed_field_values_pin_the_site_to_counter_and_word_mapping():
+    """SURVEY.md Appendix B prints twelve field values (seed 42 sites 0..3 and 20..23 with their words, seed 0
+    sites 0..3) and one block on the 64-bit path (seed 2^32+7, q = 2^32+1).  They pin init_value's mapping
+    site -> (counter, word, 24-bit shift, scale) against numbers that do not come from this repository's
+    code: a swapped word order, an off-by-one shift or a 32-bit truncation of q or of the seed fails here."""
+    values, blocks = read_philox_field_values()
+    assert len(values) == 12 and len(blocks) == 1
+    for seed, site, word, phi in values:
+        assert ref.init_value(seed, site, 1.0) == phi, (seed, site)
+        assert ref.init_value(seed, site, 1.75) == 1.75 * phi
+        if word is not None:                              # the printed word and the printed value agree
+            assert (2 * (word >> 8) + 1 - (1 << 24)) / float(1 << 24) == phi
+    # a lattice initialised by the oracle holds the same numbers at those sites (FP32 and FP64)
+    for prec in (ref.F32, ref.F64):
+        for seed in (42, 0):
+            sim = ref.RefSim(2, 8, prec, seed=seed)
+            sim.init(1.0)
+            flat = sim.copy_out()[0].ravel()
+            for sd, site, _, phi in values:
+                if sd == seed:
+                    assert float(flat[site]) == phi
+    for seed, q, words in blocks:
+        assert q >= 1 << 32 and seed >= 1 << 32
+        assert ref.philox4x32_10([q & 0xffffffff, q >> 32, 0, 0], [seed & 0xffffffff, seed >> 32]) == words
+        for j, w in enumerate(words):
+            assert ref.init_value(seed, 4 * q + j, 1.0) == (2 * (w >> 8) + 1 - (1 << 24)) / float(1 << 24)
 
 
 def test_philox_is_a_bijection_of_the_counter_on_a_sample():
