@@ -653,18 +653,20 @@ def chunked_maxdiff(a, b, chunk=1 << 26):
 
 
 FULL_SIZE_CASES = [
-    # dims, N, precision, era_m      (configs[1] .. configs[4] of BASELINE.json; both eras and both
-    #                                 precisions appear at the headline size)
-    (2, 4096, prs.F32, 1.0), (2, 4096, prs.F32, 2.0),
-    (2, 16384, prs.F32, 1.0), (2, 16384, prs.F64, 1.0),
-    (3, 512, prs.F32, 1.0),
-    (3, 1024, prs.F32, 1.0), (3, 1024, prs.F64, 2.0),
+    # dims, N, precision, era_m, literal too?   (configs[1] .. configs[4] of BASELINE.json; both eras and both
+    # precisions appear at the headline size; the other era of each precision at 1024^3 starts from a formed
+    # network in LATE_CASES below).  The north_star tolerance against the paper's LITERAL form is asserted at
+    # one case per size and precision; bit-identity with the oracle's FMA form at every case.
+    (2, 4096, prs.F32, 1.0, True), (2, 4096, prs.F32, 2.0, False),
+    (2, 16384, prs.F32, 1.0, True), (2, 16384, prs.F64, 1.0, True),
+    (3, 512, prs.F32, 1.0, True),
+    (3, 1024, prs.F32, 1.0, True), (3, 1024, prs.F64, 2.0, False),
 ]
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("dims,N,prec,era_m", FULL_SIZE_CASES)
-def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m):
+@pytest.mark.parametrize("dims,N,prec,era_m,literal", FULL_SIZE_CASES)
+def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m, literal):
     """T2 at full size: default options (the kernel selection and tiling bench.py times), seeded
     initial state, 20 steps, every site compared with the oracle run on the host cores: identical
     bits against the oracle in the same arithmetic form, within the north_star tolerance against the
@@ -686,9 +688,111 @@ def test_full_size_20_steps_match_the_oracle_everywhere(dims, N, prec, era_m):
     assert dg["link_count"] == dr["link_count"] and dg["wall_sites"] == dr["wall_sites"]
     assert abs(dg["sum_ratio"] - dr["sum_ratio"]) <= 1e-10 * dr["sum_ratio"]
     del rp, rv
+    if not literal:
+        return
     r = ref.RefSim(dims, N, prec, era_m=era_m, seed=2, arith=ref.ARITH_LITERAL, threads=THREADS)
     r.init(1.0)
     r.step(20)
     lp, lv = r.copy_out()
     r.close()
     assert chunked_maxdiff(gp, lp) <= TOL[prec] and chunked_maxdiff(gv, lv) <= TOL[prec]
+
+
+# ------------------------------------------------------------------ T3/T4 at full size on a FORMED network
+
+def steps_to(eta):
+    return int(round((eta - 1.0) / 0.1))
+
+
+def wrapped_box(a, origin, M):
+    """The M^d sub-lattice of the periodic array a whose corner is at `origin` (given in array-axis order)."""
+    idx = [(o + np.arange(M)) % n for o, n in zip(origin, a.shape)]
+    return np.ascontiguousarray(a[np.ix_(*idx)])
+
+
+LATE_CASES = [
+    # dims, N, precision, era_m, eta of the checkpoint, mode
+    #   "all":   the oracle advances the WHOLE lattice 20 steps from the GPU's snapshot: every site compared
+    #   "boxes": the oracle advances sub-lattices of the snapshot (sampled outputs: after k steps a site depends on
+    #            the sites within k links of it, so the inner (M-40)^d sites of a periodic M^d copy of a box see
+    #            exactly what they see in the whole lattice); boxes straddle the periodic seam, CTA tiles and z chunks
+    #   "+lit":  also the north_star tolerance against the oracle's LITERAL form
+    # Diagnostics and the weighted area of the checkpoint are compared on the whole lattice in every case.
+    (2, 4096, prs.F32, 1.0, 512.0, "all+lit"), (2, 4096, prs.F32, 2.0, 1843.0, "all"),
+    (2, 16384, prs.F32, 1.0, 7372.0, "all+lit"), (2, 16384, prs.F64, 1.0, 2048.0, "all+lit"),
+    (3, 512, prs.F32, 1.0, 230.0, "all+lit"),
+    (3, 1024, prs.F32, 2.0, 460.0, "all"), (3, 1024, prs.F64, 1.0, 128.0, "all"),
+    (3, 1024, prs.F32, 1.0, 128.0, "boxes+lit"), (3, 1024, prs.F64, 2.0, 460.0, "boxes+lit"),
+]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("dims,N,prec,era_m,eta,mode", LATE_CASES)
+def test_full_size_restart_parity_on_a_formed_network(dims, N, prec, era_m, eta, mode):
+    """SURVEY 8(c) T3/T4 at BASELINE.json's full sizes, every precision and era (the paper's own
+    validation compares sequential and parallel codes at LATE timesteps).  The GPU runs its default path to a
+    checkpoint where the wall network has formed (eta = N/8 or 0.45 N: a few per cent of the sites touch a wall,
+    which is where the diagnostics kernel's per-warp compaction and prs_weighted_area's link stack take their
+    data-dependent paths), then: snapshot -> oracle; diagnostics and Eq. 7's weighted area of that snapshot
+    against the oracle on the same bytes; 20 more steps on both sides; fields identical bit for bit against the
+    oracle's FMA form (and within the north_star bar of its LITERAL form), diagnostics again."""
+    adv = steps_to(eta)
+    g = prs.Simulation(dims, N, prec, era_m=era_m, seed=1)
+    g.init(1.0)
+    g.step(adv)
+    assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_TBS
+    d0 = g.diagnostics()
+    area0, _ = g.weighted_area()
+    sp, sv = g.copy_out()                                       # the checkpoint
+    o0 = ref.diagnostics_of(sp, sv)
+    assert d0["link_count"] == o0["link_count"] and d0["wall_sites"] == o0["wall_sites"]
+    assert abs(d0["sum_ratio"] - o0["sum_ratio"]) <= 1e-10 * o0["sum_ratio"]
+    assert 0 < d0["wall_sites"] < 0.25 * N ** dims              # a formed network, not the white-noise start
+    want = ref.weighted_area_of(sp)
+    assert abs(area0 - want) <= 1e-12 * want
+    assert d0["link_count"] / np.sqrt(dims) <= area0 <= d0["link_count"]
+    g.step(20)
+    d1 = g.diagnostics()
+    if mode.startswith("all"):
+        forms = [ref.ARITH_FMA] + ([ref.ARITH_LITERAL] if mode.endswith("+lit") else [])
+        for arith in forms:
+            r = ref.RefSim(dims, N, prec, era_m=era_m, arith=arith, threads=THREADS)
+            r.copy_in(sp, sv, eta0=1.0, step=adv)
+            if arith == forms[-1]:
+                del sp, sv                                      # 1024^3 FP64: keep the host footprint down
+            r.step(20)
+            o1 = r.diagnostics()
+            rp, rv = r.copy_out()
+            r.close()
+            gp, gv = g.copy_out()
+            if arith == ref.ARITH_FMA:
+                assert np.array_equal(gp, rp) and np.array_equal(gv, rv)
+                assert d1["link_count"] == o1["link_count"] and d1["wall_sites"] == o1["wall_sites"]
+                assert abs(d1["sum_ratio"] - o1["sum_ratio"]) <= 1e-10 * o1["sum_ratio"]
+                assert d1["eta"] == o1["eta"] and d1["step"] == o1["step"] == adv + 20
+            else:
+                assert chunked_maxdiff(gp, rp) <= TOL[prec] and chunked_maxdiff(gv, rv) <= TOL[prec]
+            del rp, rv, gp, gv
+    else:
+        M, R = 192, 20
+        gp, gv = g.copy_out()
+        o1 = ref.diagnostics_of(gp, gv)                         # the diagnostics of the advanced state, whole lattice
+        assert d1["link_count"] == o1["link_count"] and d1["wall_sites"] == o1["wall_sites"]
+        assert abs(d1["sum_ratio"] - o1["sum_ratio"]) <= 1e-10 * o1["sum_ratio"]
+        # corners (z, y, x): the periodic seam in all axes; the seam of the z chunks of 128 planes and of the
+        # 16-/20-row y tiles in mid-lattice; the x tiles (120 / 56 sites wide); one more in the bulk
+        for origin in ((N - 70, N - 90, N - 100), (128 - 96, 512 - 100, 300), (640 - 50, 37, N - 130), (300, 700, 450)):
+            bp, bv = wrapped_box(sp, origin, M), wrapped_box(sv, origin, M)
+            ap, av = wrapped_box(gp, origin, M), wrapped_box(gv, origin, M)
+            inner = (slice(R, M - R),) * dims
+            for arith in [ref.ARITH_FMA] + ([ref.ARITH_LITERAL] if mode.endswith("+lit") else []):
+                r = ref.RefSim(dims, M, prec, era_m=era_m, arith=arith, threads=THREADS)
+                r.copy_in(bp, bv, eta0=1.0, step=adv)
+                r.step(20)
+                rp, rv = r.copy_out()
+                r.close()
+                if arith == ref.ARITH_FMA:
+                    assert np.array_equal(ap[inner], rp[inner]) and np.array_equal(av[inner], rv[inner]), origin
+                else:
+                    assert maxdiff(ap[inner], rp[inner]) <= TOL[prec] and maxdiff(av[inner], rv[inner]) <= TOL[prec]
+    g.close()

@@ -277,3 +277,102 @@ def test_ranks_of_a_distributed_job_share_the_one_gpu(world, tmp_path):
         got = np.load(os.path.join(out, "diag%d.npy" % r))
         assert np.array_equal(got[:, :2], want[:, :2])
         assert np.allclose(got[:, 2], want[:, 2], rtol=1e-12, atol=0)
+
+
+@pytest.mark.parametrize("N,world", [(64, 1), (64, 4), (132, 3)])
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+def test_weighted_area_of_the_slabs_adds_up_to_the_lattice(N, world, prec):
+    """prs_weighted_area on a slab returns its partial sum of Eq. 7's weighted area (transverse neighbours of the
+    links of the outermost owned planes are halo planes); the parts add up to the unsharded lattice's and to the
+    oracle's value on the same bytes, on the initial field and on a formed network, with a fresh and a used halo."""
+    whole = prs.Simulation(3, N, prec, seed=4)
+    group = sharded.SlabGroup(N, [0] * world, prec, seed=4)
+    whole.init(1.0)
+    group.init(1.0)
+    for k in (0, 4, 3, 60, 1):
+        whole.step(k)
+        group.step(k)
+        a_w, r_w = whole.weighted_area()
+        a_g, r_g = group.weighted_area()
+        want = ref.weighted_area_of(whole.copy_out()[0])
+        assert abs(a_g - a_w) <= 1e-12 * max(a_w, 1.0) and abs(a_g - want) <= 1e-12 * max(want, 1.0)
+        assert abs(r_g - r_w) <= 1e-15
+    s = group.slabs[0]
+    s.step(s.halo_valid)                                      # use the halo up: the call must refuse, not misread
+    if world > 1:
+        with pytest.raises(prs.PrsError):
+            s.weighted_area()
+    group.close()
+    whole.close()
+
+
+def test_sharded_simulation_on_a_stream_of_its_own():
+    """The halo transport must run on the slab's stream: with a non-default, non-blocking stream the
+    copies would otherwise race with the step kernels.  world = 1: the slab is its own neighbour."""
+    import torch
+
+    N = 96
+    st = torch.cuda.Stream()
+    whole = prs.Simulation(3, N, prs.F32, seed=5)
+    one = sharded.ShardedSimulation(N, prs.F32, rank=0, world=1, seed=5, stream=st)
+    whole.init(1.0)
+    one.init(1.0)
+    for k in (4, 4, 4, 9, 2):
+        whole.step(k)
+        one.step(k)
+    one.slab.sync()
+    wp, wv = whole.copy_out()
+    gp, gv = one.copy_out()
+    assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes()
+    same_diag(one.diagnostics(), whole.diagnostics())
+    assert abs(one.weighted_area()[0] - whole.weighted_area()[0]) <= 1e-12 * whole.weighted_area()[0]
+    one.close()
+    whole.close()
+
+
+def test_handles_work_whatever_device_is_current():
+    """A handle belongs to the device that owns its workspace (include/prs.h "Devices"): every call switches to it
+    and restores the caller's device.  With one GPU this checks the restore; with two or more, that a handle on
+    device 1 can be driven while device 0 is current and that the > 48 KB shared-memory attribute is set per device."""
+    import torch
+    from paper_1710_10420_b200 import prs as binding
+
+    ndev = torch.cuda.device_count()
+    dev = ndev - 1
+    with torch.cuda.device(dev):
+        g = prs.Simulation(3, 128, prs.F32, seed=7)            # 128^3: the four-step kernel (172 KB of shared memory)
+    assert g.get_info(binding.INFO_DEVICE) == dev
+    torch.cuda.set_device(0)
+    g.init(1.0)
+    g.step(9)
+    d = g.diagnostics()
+    assert torch.cuda.current_device() == 0
+    assert g.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_TBS
+    ref_g = prs.Simulation(3, 128, prs.F32, seed=7)            # on device 0
+    ref_g.init(1.0)
+    ref_g.step(9)
+    same_diag(d, ref_g.diagnostics())
+    assert g.copy_out()[0].tobytes() == ref_g.copy_out()[0].tobytes()
+    g.close()
+    ref_g.close()
+
+
+def test_slab_group_over_two_devices():
+    import torch
+
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs in one process (the box has one); see test_handles_work_whatever_device_is_current")
+    N = 128
+    whole = prs.Simulation(3, N, prs.F32, seed=3)
+    group = sharded.SlabGroup(N, [0, 1], prs.F32, seed=3)
+    whole.init(1.0)
+    group.init(1.0)
+    for k in STEPS:
+        whole.step(k)
+        group.step(k)
+        wp, wv = whole.copy_out()
+        gp, gv = group.copy_out()
+        assert gp.tobytes() == wp.tobytes() and gv.tobytes() == wv.tobytes(), k
+        same_diag(group.diagnostics(), whole.diagnostics())
+    group.close()
+    whole.close()
