@@ -70,9 +70,13 @@ enum {
     PRS_OPT_TB2_TILE_Y  = 6,   /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
     PRS_OPT_TBS_STEPS   = 7,   /* steps per pass of the multi-step kernel: 3 or 4, in 2D also 6 or 8;
                                 * default 4 in 3D, in 2D 8 (FP32) or 6 (FP64)                       */
-    PRS_OPT_TBS_ROWS    = 8    /* tuning, 3D multi-step kernel: rows of the tile per thread, 1 (default) or
+    PRS_OPT_TBS_ROWS    = 8,   /* tuning, 3D multi-step kernel: rows of the tile per thread, 1 (default) or
                                 * 2 (step3d_tbr_kernel: half the shared-memory traffic, taller tiles;
                                 * bit-identical; about 3 % faster in FP32, slower in FP64)            */
+    PRS_OPT_TBS_LOADER  = 9    /* tuning, 3D multi-step kernel: how the shared-memory rings are filled: 0 (default)
+                                * = TMA bulk copies of whole tile rows completing on mbarriers where a lattice
+                                * row holds >= 32 16-byte vectors, else per-thread cp.async; 1 = always cp.async;
+                                * 2 = same as 0.  Bit-identical either way                              */
 };
 enum {
     PRS_KERNEL_AUTO    = 0,    /* fastest kernel that supports (dims, N, precision)                */
@@ -159,6 +163,16 @@ int prs_sync(prs_handle h);
 int prs_set_option(prs_handle h, int option, int64_t value);   /* PRS_ERR_UNSUPPORTED if the kernel  *
                                                                 * cannot take this (dims, N, T)      */
 int prs_get_info(prs_handle h, int info, int64_t* value);
+
+/* What the most recent prs_step call launched first -- its main kernel: the schedule goes from the deepest
+ * pipeline to single steps, e.g. prs_step(50) = 12 four-step launches, then one two-step launch.  name: the kernel
+ * with its template arguments as a profiler demangles it, minus "(int)", "(bool)" and blanks, e.g.
+ * "step3d_tbs_kernel<float,2,4,16,1>" (truncated to name_bytes); grid, block: its launch configuration; smem_bytes:
+ * dynamic shared memory; steps_per_launch: PRS steps one launch advances; launches: how many times that call launched
+ * it.  Any pointer may be NULL (HOST pointers).  PRS_ERR_STATE before the first step.  Lets a benchmark tie a
+ * profiler capture to the kernel that actually ran. */
+int prs_step_launch_info(prs_handle h, char* name, size_t name_bytes, int64_t grid[3], int64_t block[3],
+                         int64_t* smem_bytes, int64_t* steps_per_launch, int64_t* launches);
 
 /* DEVICE pointers to the current phi^n and phidot^{n-1/2} arrays (valid until the next prs_step /
  * prs_copy_in / prs_init): lets a caller (e.g. a torch tensor view) read the state without a copy. */

@@ -138,6 +138,9 @@ cudaError_t launch_generic(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     const unsigned blocks = (unsigned)((h->S + 255) / 256);
     step_generic_kernel<T, DIMS, ARITH><<<blocks, 256, 0, h->stream>>>(p, v, pn, vn, (long long)h->N,
                                                                          (long long)h->NZ, (long long)h->S, k);
+    char name[96];
+    snprintf(name, sizeof(name), "step_generic_kernel<%s,%d,%d>", type_name<T>(), DIMS, ARITH);
+    note_launch(h, name, dim3(blocks, 1, 1), dim3(256, 1, 1), 0, 1);
     return cudaGetLastError();
 }
 
@@ -171,6 +174,9 @@ cudaError_t launch_tiled3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     if (ty == 4) step3d_tiled_kernel<T, ARITH, 4><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k);
     else if (ty == 16) step3d_tiled_kernel<T, ARITH, 16><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k);
     else step3d_tiled_kernel<T, ARITH, 8><<<grid, block, 0, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k);
+    char name[96];
+    snprintf(name, sizeof(name), "step3d_tiled_kernel<%s,%d,%d>", type_name<T>(), ARITH, (ty == 4 || ty == 16) ? ty : 8);
+    note_launch(h, name, grid, block, 0, 1);
     return cudaGetLastError();
 }
 
@@ -183,6 +189,9 @@ cudaError_t launch_tiled2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, con
     const int YC = pick_chunk(h, gx, BX);
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
     step2d_tiled_kernel<T, ARITH><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k);
+    char name[96];
+    snprintf(name, sizeof(name), "step2d_tiled_kernel<%s,%d>", type_name<T>(), ARITH);
+    note_launch(h, name, grid, dim3(BX, 1, 1), 0, 1);
     return cudaGetLastError();
 }
 
@@ -240,6 +249,9 @@ cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int
         if (e != cudaSuccess) return e;
     }
     step2d_cluster_kernel<T, ARITH><<<CLUSTER_CTAS, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N, nsteps, ks);
+    char name[96];
+    snprintf(name, sizeof(name), "step2d_cluster_kernel<%s,%d>", type_name<T>(), ARITH);
+    note_launch(h, name, dim3(CLUSTER_CTAS, 1, 1), dim3(CLUSTER_THREADS, 1, 1), smem, nsteps);
     return cudaGetLastError();
 }
 
@@ -398,7 +410,9 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     // measured, 16384^2, site-updates/s: FP32 1.29e12 (S = 4), 1.76e12 (6), 1.95e12 (8); FP64 6.8e11 (4), 9.5e11 (6), 8.9e11 (8)
     h->opt_tbs_steps = (dims == 3) ? 4 : (precision == PRS_F32 ? 8 : 6);
     h->opt_tbs_rows = 1;
+    h->opt_tbs_loader = 0;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
+    memset(&h->main_launch, 0, sizeof(h->main_launch));
     h->h_result = nullptr;
     h->device = attr.device;                      // the device that owns the workspace: all launches go there
     DeviceGuard guard(h->device);
@@ -484,6 +498,7 @@ int prs_step(prs_handle h, int64_t nsteps) {
     PRS_ON_DEVICE(h);
     if (nsteps < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_step: nsteps must be >= 0");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
+    if (nsteps > 0) h->main_launch.open = true;
     if (h->slab) {
         // Each step uses up one halo plane per side (the halo sites are advanced redundantly from the
         // planes beyond them).  nsteps = 4 or 3 is one pass of the multi-step kernel, which writes the
@@ -742,6 +757,10 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
                 return fail(h, PRS_ERR_INVALID_ARG, "tbs_rows must be 1 or, in 3D, 2");
             h->opt_tbs_rows = (int)value;
             return PRS_OK;
+        case PRS_OPT_TBS_LOADER:
+            if (value != 0 && value != 1 && value != 2) return fail(h, PRS_ERR_INVALID_ARG, "tbs_loader must be 0 (auto), 1 (cp.async) or 2 (bulk)");
+            h->opt_tbs_loader = (int)value;
+            return PRS_OK;
         case PRS_OPT_TB2_TILE_Y:
             if (value != 4 && value != 8 && value != 12 && value != 28)
                 return fail(h, PRS_ERR_INVALID_ARG, "tb2_tile_y must be 4, 8, 12 or 28");
@@ -764,6 +783,22 @@ int prs_get_info(prs_handle h, int info, int64_t* value) {
         case PRS_INFO_DEVICE: *value = h->device; return PRS_OK;
         default: return fail(h, PRS_ERR_INVALID_ARG, "unknown info key");
     }
+}
+
+int prs_step_launch_info(prs_handle h, char* name, size_t name_bytes, int64_t grid[3], int64_t block[3],
+                         int64_t* smem_bytes, int64_t* steps_per_launch, int64_t* launches) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    const auto& m = h->main_launch;
+    if (m.count == 0 || m.open) return fail(h, PRS_ERR_STATE, "prs_step_launch_info: no step kernel launched yet");
+    if (name && name_bytes) snprintf(name, name_bytes, "%s", m.name);
+    for (int i = 0; i < 3; ++i) {
+        if (grid) grid[i] = m.grid[i];
+        if (block) block[i] = m.block[i];
+    }
+    if (smem_bytes) *smem_bytes = (int64_t)m.smem;
+    if (steps_per_launch) *steps_per_launch = m.steps;
+    if (launches) *launches = m.count;
+    return PRS_OK;
 }
 
 int prs_device_pointers(prs_handle h, void** phi, void** phidot) {

@@ -9,6 +9,8 @@
 #include <atomic>
 #include <cmath>
 #include <cstdint>
+#include <cstdio>
+#include <cstring>
 #include <string>
 
 #include <cuda_runtime.h>
@@ -32,7 +34,7 @@ struct prs_ctx {
     double eta0;
     int64_t step;
     bool inited;
-    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps, opt_tbs_rows;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps, opt_tbs_rows, opt_tbs_loader;
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;
@@ -41,6 +43,16 @@ struct prs_ctx {
     // z slab of a sharded 3D lattice (prs_create_slab): the arrays hold NZ = nz_own + 2*halo planes of
     // N x N sites, local plane l = global plane (z_begin - halo + l) mod N; S counts the local sites.
     // halo_valid = how many more steps the halo planes can feed before they must be exchanged again.
+    // the first kernel launched by the most recent prs_step call (its main kernel: the schedule goes from the
+    // deepest pipeline to single steps), as prs_step_launch_info reports it
+    struct {
+        char name[96];                        // e.g. "step3d_tbs_kernel<float,2,4,16,1>"
+        unsigned grid[3], block[3];
+        size_t smem;
+        int steps;                            // PRS steps one launch advances
+        int count;                            // launches of it in that prs_step call
+        bool open;                            // no launch recorded yet in the current prs_step call
+    } main_launch;
     bool slab;
     int64_t NZ, nz_own, halo, z_begin;
     int halo_valid;
@@ -68,6 +80,24 @@ struct DeviceGuard {
     DeviceGuard(const DeviceGuard&) = delete;
     DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
+
+template <typename T> inline const char* type_name();
+template <> inline const char* type_name<float>() { return "float"; }
+template <> inline const char* type_name<double>() { return "double"; }
+
+// Book-keeping for prs_step_launch_info: `name` is the kernel with its template arguments, written the way a
+// profiler's demangled name reads once "(int)", "(bool)" and blanks are stripped.
+inline void note_launch(prs_ctx* h, const char* name, dim3 grid, dim3 block, size_t smem, int steps) {
+    auto& m = h->main_launch;
+    if (m.open) {
+        snprintf(m.name, sizeof(m.name), "%s", name);
+        m.grid[0] = grid.x; m.grid[1] = grid.y; m.grid[2] = grid.z;
+        m.block[0] = block.x; m.block[1] = block.y; m.block[2] = block.z;
+        m.smem = smem; m.steps = steps; m.count = 1; m.open = false;
+    } else if (strncmp(m.name, name, sizeof(m.name)) == 0 && m.grid[0] == grid.x && m.grid[1] == grid.y && m.grid[2] == grid.z) {
+        m.count += 1;
+    }
+}
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: it is set once per
 // (kernel instantiation, device).  `done` is the instantiation's own bit mask of devices already configured

@@ -39,6 +39,43 @@ __device__ __forceinline__ void static_for(F&& f) {
     }
 }
 
+// ---- TMA bulk copies completing on an mbarrier (cp.async.bulk, SASS UBLKCP / SYNCS) ----------------------------
+// Addresses are 32-bit shared-window addresses of this CTA (a CTA is a cluster of one).
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+// true in exactly one lane of the (converged) warp, and known to the compiler as such
+__device__ __forceinline__ bool elect_one() {
+    unsigned pred;
+    asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}\n" : "=r"(pred));
+    return pred != 0u;
+}
+__device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+// blocks (hardware sleep, not a spin) until the phase of the given parity has completed
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// bytes: a multiple of 16; both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(unsigned smem_dst, const void* gmem_src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(smem_dst), "l"(gmem_src), "r"(bytes), "r"(bar) : "memory");
+}
+
 template <typename T, int S>
 struct StepCoefs {
     StepCoef<T> k[S];
@@ -56,10 +93,19 @@ template <typename T, int S> __host__ __device__ constexpr int tbs_xhalo() { ret
 template <typename T, int S> __host__ __device__ constexpr int tbs_xout() { return 32 - 2 * tbs_xhalo<T, S>(); }
 template <typename T, int S, int TY>
 constexpr size_t tbs_smem_bytes() {
-    return (size_t)(4 + 4 + 2 * (S - 1)) * (TY + 2 * S) * 32 * 16;
+    return (size_t)(4 + 4 + 2 * (S - 1)) * (TY + 2 * S) * 32 * 16 + 64;       // + four mbarriers (bulk loader)
 }
 
-template <typename T, int ARITH, int S, int TY>
+// BULK = false: every thread fetches its own 16-byte column of the two rings with cp.async (LDGSTS) and waits on
+// its own groups.  BULK = true (lattices with at least 32 vectors per row): the rings are filled by TMA bulk copies
+// -- one 512-byte row of the tile per copy, two where the row straddles the periodic seam in x, so the periodic
+// lattice needs no tensor map -- issued by one elected lane of each warp for the warp's own row (all operands of a
+// bulk copy are warp-uniform, so the cursor lives in uniform registers) and completing on one mbarrier per ring
+// slot; the tile's last warp (row ROWS-1, which computes nothing) sleeps on the slot's mbarrier before it joins the
+// CTA barrier, so the computing warps wait on nothing but the one barrier per plane.  Measured (ncu, 1024^3 FP32): an LDGSTS.128
+// costs 13.8 wavefronts of the l1tex data pipe against 4 for an LDS.128 -- the two per thread and plane were 30 %
+// of that pipe's load, the busiest unit of the kernel.
+template <typename T, int ARITH, int S, int TY, bool BULK>
 __global__ void __launch_bounds__(32 * (TY + 2 * S), 1)
 step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int ZC, StepCoefs<T, S> coefs, ZRange zr) {
@@ -70,6 +116,7 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     constexpr int XH = tbs_xhalo<T, S>(), XOUT = tbs_xout<T, S>();
     constexpr int ROWS = TY + 2 * S;
     constexpr int PLANE = ROWS * 32;                                 // vectors per shared plane
+    static_assert(ROWS <= 32, "the bulk loader feeds one row of the tile per lane of one warp");
     extern __shared__ __align__(16) unsigned char tbs_smem[];
     const int lane = threadIdx.x, row = threadIdx.y;
     const int me = row * 32 + lane;
@@ -78,13 +125,36 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     V* const sB = sP + 4 * PLANE;                                    // published planes [S-1][2][PLANE]
 
     const int NQ = N / W;
+    const int z0 = zr.lo + (int)blockIdx.z * ZC;
+    const int zend = min(z0 + ZC, zr.hi);
+    const int niter = (zend - z0) + 2 * S - 2;                       // >= 2S-1
+    const unsigned NNv = (unsigned)N * (unsigned)NQ;                 // vectors per plane
+    const V* const gA = reinterpret_cast<const V*>(phi);
+    const V* const gP = reinterpret_cast<const V*>(phidot);
+
+    // ---- bulk loader: four mbarriers, one per ring slot; each of the ROWS warps arrives once per issue ----------
+    const unsigned bars = smem_u32(tbs_smem + (size_t)(4 + 4 + 2 * (S - 1)) * PLANE * 16);       // full[4], 8 bytes each
+    if constexpr (BULK) {
+        if (me == 0) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) mbar_init(bars + 8 * u, ROWS);
+            mbar_init_fence();
+        }
+        __syncthreads();
+    }
+    // The warp's row as a value the compiler knows to be warp-uniform (a shuffle from lane 0), so that the row
+    // cursor, the mbarrier and ring addresses of the bulk copies live in uniform registers (UBLKCP takes only those).
+    const int row_u = BULK ? __shfl_sync(0xffffffffu, row, 0) : row;
+    const int q0 = wrap_mod(XOUT * (int)blockIdx.x - XH, NQ);       // first vector of the tile's rows (periodic)
+    const unsigned len0 = (unsigned)min(32, NQ - q0) * 16u, len1 = 512u - len0;   // bytes before / after the x seam
+    const unsigned rowA = smem_u32(tbs_smem) + (unsigned)row_u * 512u;             // this warp's row of ring A, slot 0
+    const unsigned rowP = rowA + 4u * PLANE * 16u;
+    const bool leader = BULK ? elect_one() : false;
+
     const int qraw = XOUT * (int)blockIdx.x - XH + lane;
     const int q = wrap_mod(qraw, NQ);
     const int yraw = TY * (int)blockIdx.y - S + row;
     const int y = wrap_mod(yraw, N);
-    const int z0 = zr.lo + (int)blockIdx.z * ZC;
-    const int zend = min(z0 + ZC, zr.hi);
-    const int niter = (zend - z0) + 2 * S - 2;                       // >= 2S-1
     const bool store_ok = (yraw < N) && (lane >= XH) && (lane < 32 - XH) && (qraw < NQ);
 
     PackCoef<T> pc[S];
@@ -93,14 +163,12 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 
     // Unsigned 32-bit indices of 16-byte vectors (the host checks N^3 / W <= 2^31, so that the cursor,
     // which runs one lattice length past the end before it wraps, stays below 2^32).
-    const V* const gA = reinterpret_cast<const V*>(phi);
-    const V* const gP = reinterpret_cast<const V*>(phidot);
     V* const oA = reinterpret_cast<V*>(phi_out);
     V* const oP = reinterpret_cast<V*>(phidot_out);
-    const unsigned NNv = (unsigned)N * (unsigned)NQ;                 // vectors per plane
     const unsigned colv = (unsigned)y * (unsigned)NQ + (unsigned)q;  // this thread's column within a plane
     int zl = wrap_mod(z0 - S, zr.nz);
-    unsigned il = (unsigned)zl * NNv + colv;                         // load cursor: issue i = plane a = i
+    // load cursor (issue i = plane a = i): of this thread's column (cp.async) or of the warp's row (bulk copies)
+    unsigned il = (unsigned)zl * NNv + (BULK ? (unsigned)wrap_mod(TY * (int)blockIdx.y - S + row_u, N) * (unsigned)NQ + (unsigned)q0 : colv);
     int left_to_wrap = zr.nz - zl;                                   // issues until z wraps to 0
     unsigned io = (unsigned)z0 * NNv + colv;                         // store cursor
 
@@ -108,17 +176,42 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
         constexpr int NS = decltype(ns_tag)::value;                  // stages this row runs
         int ni = 0;
         auto issue = [&](int slot_a, int slot_p) {
-            if (ni < niter + 2) cp_async16(sA + slot_a * PLANE, gA + il);
-            if (NS >= 1 && ni >= 1 && ni <= niter) cp_async16(sP + slot_p * PLANE, gP + il);
+            if constexpr (BULK) {
+                // Unconditional: the planes past the chunk's last (two of phi, four of phidot, and phidot plane 0) are
+                // fetched and never read -- 2 % of the L2 traffic -- so that every issue is the same few uniform
+                // instructions and every phase of a slot's mbarrier expects the same bytes.
+                if (leader) {                                        // one lane: the row of the warp, both rings
+                    const unsigned bar = bars + 8u * (unsigned)slot_a;
+                    mbar_arrive_expect_tx(bar, NS >= 1 ? 1024u : 512u);
+                    const unsigned d = rowA + (unsigned)slot_a * (PLANE * 16u);
+                    bulk_g2s(d, gA + il, len0, bar);
+                    if (len1) bulk_g2s(d + len0, gA + (il - (unsigned)q0), len1, bar);
+                    if constexpr (NS >= 1) {
+                        const unsigned e = rowP + (unsigned)slot_p * (PLANE * 16u);
+                        bulk_g2s(e, gP + il, len0, bar);
+                        if (len1) bulk_g2s(e + len0, gP + (il - (unsigned)q0), len1, bar);
+                    }
+                }
+            } else {
+                const bool la = ni < niter + 2, lp = NS >= 1 && ni >= 1 && ni <= niter;
+                if (la) cp_async16(sA + slot_a * PLANE, gA + il);
+                if (lp) cp_async16(sP + slot_p * PLANE, gP + il);
+            }
             ++ni; il += NNv;
             if (--left_to_wrap == 0) { il -= zr.wrap; left_to_wrap = zr.nz; }   // modulo 2^32, exact
         };
-        // prologue: group 0 = issues 0, 1, 2 (phi^n planes 0..2, phidot planes 0..1); group 1 = issue 3
+        // prologue: issues 0..3 (phi^n planes 0..3, phidot planes 1..3); planes 0 and 1 must have landed
         issue(0, 3); issue(1, 0); issue(2, 1);
-        cp_async_commit();
-        issue(3, 2);
-        cp_async_commit();
-        cp_async_wait<1>();
+        if constexpr (BULK) {
+            issue(3, 2);
+            if (row_u == ROWS - 1) { mbar_wait(bars + 0, 0u); mbar_wait(bars + 8, 0u); }       // the waiter warp, see below
+            __syncthreads();
+        } else {
+            cp_async_commit();                  // group 0 = issues 0, 1, 2; group 1 = issue 3
+            issue(3, 2);
+            cp_async_commit();
+            cp_async_wait<1>();
+        }
         // register windows: wprev[s], wcur[s] = input field of stage s at planes a_s-1, a_s (own column);
         // qcur[s] = phidot input of stage s at plane a_s (s >= 1)
         V wprev[S], wcur[S], qcur[S];
@@ -127,16 +220,28 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
         wprev[0] = sA[0 * PLANE];
         wcur[0] = sA[1 * PLANE];
 
+        // phase parity of the next issue to wait for on each slot's mbarrier: issues 0, 1 (slots 0, 1) were waited for
+        // in the prologue, so slots 0, 1 are at their second phase and slots 2, 3 at their first
+        unsigned ph[4] = {1u, 1u, 0u, 0u};
         // One iteration.  U = j mod 4 (ring slots) and PAR = j mod 2 (published plane) are compile-time
         // constants; ACTRAW = number of stages that have started (j/2 + 1, capped at S).
         auto iteration = [&](auto u_tag, auto act_tag) {
             constexpr int U = decltype(u_tag)::value, PAR = U & 1;
             constexpr int ACTRAW = decltype(act_tag)::value;
             constexpr int ACT = (NS > ACTRAW) ? ACTRAW : NS;
-            cp_async_wait<1>();                 // group j has landed for this thread
+            if constexpr (BULK) {
+                // The tile's last warp (which computes nothing) sleeps on the mbarrier of issue j+2 and then joins
+                // the CTA barrier: after it, the planes are there for everybody.  ph = phase parity of issue j+2.
+                if constexpr (NS == 0) {
+                    if (row_u == ROWS - 1) mbar_wait(bars + 8u * (unsigned)((U + 2) & 3), ph[(U + 2) & 3]);
+                    ph[(U + 2) & 3] ^= 1u;
+                }
+            } else {
+                cp_async_wait<1>();             // group j has landed for this thread
+            }
             __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
             issue(U, (U + 3) & 3);              // issue j+4: phi^n plane j+4 takes the slot of plane j
-            cp_async_commit();
+            if constexpr (!BULK) cp_async_commit();
             if constexpr (NS >= 1) {
                 V carry, qout[S];
                 {   // stage 0 on plane a = j+1
@@ -194,7 +299,7 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             if (j + 3 >= niter) break;
             iteration(integral_constant<int, (J0 + 3) & 3>{}, integral_constant<int, S>{});
         }
-        cp_async_wait<0>();
+        if constexpr (!BULK) cp_async_wait<0>();
     };
     // rows r from the tile edge run min(r, S) stages
     const int edge = min(row, ROWS - 1 - row);

@@ -26,6 +26,9 @@ cudaError_t launch_tb2_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, c
     const dim3 grid(gx, gy, (unsigned)((NZ + ZC - 1) / ZC));
     const dim3 block(32, TY + 4, 1);
     step3d_tb2_kernel<T, ARITH, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, NZ, ZC, k1, k2);
+    char name[96];
+    snprintf(name, sizeof(name), "step3d_tb2_kernel<%s,%d,%d>", type_name<T>(), ARITH, TY);
+    note_launch(h, name, grid, block, smem, 2);
     return cudaGetLastError();
 }
 
@@ -51,6 +54,9 @@ cudaError_t launch_tb2_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, cons
     int YC = h->opt_chunk > 0 ? (int)std::min<int64_t>(h->opt_chunk, N) : (int)std::min<int64_t>(64, N);
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
     step2d_tb2_kernel<T, ARITH><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, k1, k2);
+    char name[96];
+    snprintf(name, sizeof(name), "step2d_tb2_kernel<%s,%d>", type_name<T>(), ARITH);
+    note_launch(h, name, grid, dim3(BX, 1, 1), 0, 2);
     return cudaGetLastError();
 }
 

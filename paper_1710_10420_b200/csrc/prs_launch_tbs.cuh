@@ -49,12 +49,6 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     if (h->opt_tbs_rows == 2) return launch_tbr_3d<T, ARITH, S>(h, p, v, pn, vn);      // PRS_OPT_TBS_ROWS
     StepCoefs<T, S> ks;
     for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
-    const size_t smem = tbs_smem_bytes<T, S, TY>();
-    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
-    {
-        const cudaError_t e = ensure_dynamic_smem(step3d_tbs_kernel<T, ARITH, S, TY>, smem, h->device, configured);
-        if (e != cudaSuccess) return e;
-    }
     constexpr int XOUT = tbs_xout<T, S>();
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
     // z slab (prs_create_slab): the lattice is N x N x (owned + 2 halo) planes and only the owned planes
@@ -66,7 +60,27 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const int ZC = tbs_pick_zc(h, (long long)gx * gy, nzo, S);
     const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, TY + 2 * S, 1);
-    step3d_tbs_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+    const size_t smem = tbs_smem_bytes<T, S, TY>();
+    // the rings are filled by TMA bulk copies of whole tile rows (at most two runs per row) when a row of the
+    // lattice holds at least 32 vectors; smaller lattices, or PRS_OPT_TBS_LOADER = 1, keep the per-thread cp.async
+    const bool bulk = NQ >= 32 && h->opt_tbs_loader != 1;
+    if (bulk) {
+        static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
+        const cudaError_t e = ensure_dynamic_smem(step3d_tbs_kernel<T, ARITH, S, TY, true>, smem, h->device, configured);
+        if (e != cudaSuccess) return e;
+        step3d_tbs_kernel<T, ARITH, S, TY, true><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+        char name[96];
+        snprintf(name, sizeof(name), "step3d_tbs_kernel<%s,%d,%d,%d,1>", type_name<T>(), ARITH, S, TY);
+        note_launch(h, name, grid, block, smem, S);
+    } else {
+        static std::atomic<unsigned long long> configured{0};
+        const cudaError_t e = ensure_dynamic_smem(step3d_tbs_kernel<T, ARITH, S, TY, false>, smem, h->device, configured);
+        if (e != cudaSuccess) return e;
+        step3d_tbs_kernel<T, ARITH, S, TY, false><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+        char name[96];
+        snprintf(name, sizeof(name), "step3d_tbs_kernel<%s,%d,%d,%d,0>", type_name<T>(), ARITH, S, TY);
+        note_launch(h, name, grid, block, smem, S);
+    }
     return cudaGetLastError();
 }
 
@@ -93,6 +107,9 @@ cudaError_t launch_tbr_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, (TY + 2 * S) / 2, 1);
     step3d_tbr_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+    char name[96];
+    snprintf(name, sizeof(name), "step3d_tbr_kernel<%s,%d,%d,%d>", type_name<T>(), ARITH, S, TY);
+    note_launch(h, name, grid, block, smem, S);
     return cudaGetLastError();
 }
 
@@ -129,6 +146,9 @@ cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     // none 0.180, 4 rows 0.154, 8 rows 0.153, 16 rows 0.163, 32 rows 0.215
     const int l2_ahead = std::min(TBS2D_L2_AHEAD, N);
     step2d_tbs_kernel<T, ARITH, S><<<grid, BX, 0, h->stream>>>(p, v, pn, vn, N, YC, l2_ahead, ks);
+    char name[96];
+    snprintf(name, sizeof(name), "step2d_tbs_kernel<%s,%d,%d>", type_name<T>(), ARITH, S);
+    note_launch(h, name, grid, dim3(BX, 1, 1), 0, S);
     return cudaGetLastError();
 }
 

@@ -15,7 +15,7 @@ from . import build as _build
 F32, F64 = 0, 1
 ARITH_LITERAL, ARITH_COEF, ARITH_FMA = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_TB2, KERNEL_TBS, KERNEL_CLUSTER = 0, 1, 2, 3, 4, 5
-OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS, OPT_TBS_LOADER = 1, 2, 3, 4, 5, 6, 7, 8, 9
 INFO_KERNEL_LAUNCHES, INFO_STEP_KERNEL, INFO_STEP, INFO_DIAG_KERNEL = 1, 2, 3, 4
 INFO_HALO_VALID, INFO_HALO_PLANES, INFO_DEVICE = 5, 6, 7
 ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WORKSPACE",
@@ -23,7 +23,7 @@ ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WOR
 
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
            "prs_weighted_area", "prs_set_beta", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
-           "prs_device_pointers", "prs_last_error",
+           "prs_device_pointers", "prs_last_error", "prs_step_launch_info",
            "prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled", "prs_diag_combine"]
 
 
@@ -67,6 +67,8 @@ def lib():
         L.prs_set_option.argtypes = [vp, ci, i64]
         L.prs_get_info.argtypes = [vp, ci, C.POINTER(i64)]
         L.prs_device_pointers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+        L.prs_step_launch_info.argtypes = [vp, C.c_char_p, sz, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64),
+                                           C.POINTER(i64), C.POINTER(i64)]
         L.prs_diag_combine.argtypes = [C.POINTER(Diag), ci, ci, i64, C.POINTER(Diag)]
         L.prs_last_error.argtypes = [vp]
         L.prs_last_error.restype = C.c_char_p
@@ -215,6 +217,17 @@ class Simulation:
         p, v = C.c_void_p(), C.c_void_p()
         self._chk(lib().prs_device_pointers(self._h, C.byref(p), C.byref(v)), "prs_device_pointers")
         return p.value, v.value
+
+    def step_launch_info(self):
+        """prs_step_launch_info: the main kernel of the last step() call -- name with template arguments, grid,
+        block, dynamic shared memory, PRS steps per launch, launches in that call."""
+        name = C.create_string_buffer(96)
+        grid, block = (C.c_int64 * 3)(), (C.c_int64 * 3)()
+        smem, steps, count = C.c_int64(), C.c_int64(), C.c_int64()
+        self._chk(lib().prs_step_launch_info(self._h, name, 96, grid, block, C.byref(smem), C.byref(steps),
+                                             C.byref(count)), "prs_step_launch_info")
+        return {"kernel": name.value.decode(), "grid": [int(v) for v in grid], "block": [int(v) for v in block],
+                "smem_bytes": int(smem.value), "steps_per_launch": int(steps.value), "launches": int(count.value)}
 
     # -- conveniences over set_option / get_info
     def set_step_kernel(self, kernel):

@@ -150,8 +150,8 @@ def test_slab_error_paths():
         s.diagnostics()                                                 # stale halo
     assert e.value.code == 4
     with pytest.raises(prs.PrsError) as e:
-        s.weighted_area()
-    assert e.value.code == 2
+        s.weighted_area()                                               # stale halo as well
+    assert e.value.code == 4
     with pytest.raises(prs.PrsError) as e:
         s.set_step_kernel(prs.KERNEL_TB2)
     assert e.value.code == 2
