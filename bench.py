@@ -53,24 +53,23 @@ CONFIGS = {
 DEFAULT_CONFIG = "3d_1024_f32_rad"
 BYTES_PER_SITE_UPDATE = {0: 16, 1: 32}        # read phi, phidot; write phidot, phi
 
-# dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed
-# `ncu --set full` capture of the headline config (profiles/): filled in once measured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    # profiles/r01c_ncu_step3d_tbs4_f32_1024.md: 9.485 GB read + 8.558 GB written per four-step launch
-    ("3d_1024_f32_rad", "tbs"): 18_043_506_000,
-    # profiles/r01d_ncu_step3d_tbs4_f64_1024.md: 19.655 GB read + 17.151 GB written per four-step launch
-    ("3d_1024_f64_rad", "tbs"): 36_806_144_000,
-    # profiles/r01b_ncu_step3d_tb2_f32_1024.md: 9.136 GB read + 8.552 GB written per two-step launch
-    ("3d_1024_f32_rad", "tb2"): 17_687_191_000,
-    # profiles/r01b_ncu_step3d_tb2_f64_1024.md: 18.451 GB read + 17.144 GB written per two-step launch
-    ("3d_1024_f64_rad", "tb2"): 35_594_988_000,
-    # profiles/r01a_ncu_step3d_tiled_f32_1024.md: 8.867 GB read + 8.549 GB written per single-step launch
-    ("3d_1024_f32_rad", "tiled"): 17_415_889_000,
-    # profiles/r01e_ncu_step2d_tbs8_f32_16384.md: 2.572 GB read + 2.109 GB written per eight-step launch
-    ("2d_16384_f32_rad", "tbs"): 4_680_775_000,
-    # profiles/r01e_ncu_step2d_tbs6_f64_16384.md: 5.133 GB read + 4.260 GB written per six-step launch
-    ("2d_16384_f64_rad", "tbs"): 9_392_606_000,
-}
+NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+
+
+def ncu_traffic_for(launch):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel that was ACTUALLY launched, from
+    the committed record of `ncu --set full` captures (profiles/ncu_traffic.json: one entry per capture with the
+    kernel's name and template arguments, grid, block and bytes).  A capture counts only if kernel, grid and
+    block all equal what prs_step_launch_info reports for this run; otherwise (None, why)."""
+    try:
+        with open(NCU_TRAFFIC_FILE) as fh:
+            captures = json.load(fh)["captures"]
+    except Exception as exc:
+        return None, "no capture record (%s)" % exc
+    for c in captures:
+        if c["kernel"] == launch["kernel"] and c["grid"] == launch["grid"] and c["block"] == launch["block"]:
+            return int(c["dram_bytes_read"]) + int(c["dram_bytes_write"]), "ncu capture %s" % c["profile"]
+    return None, "no committed ncu capture of %s grid %s block %s" % (launch["kernel"], launch["grid"], launch["block"])
 
 
 def measured_peak_gbs():
@@ -138,24 +137,31 @@ def host_threads():
         return os.cpu_count() or 1
 
 
-def oracle_sample(dims, prec, era_m, nsteps, threads, N=None, seed=1, with_init=True):
-    """Times the oracle's step loop + one diagnostics pass on a bounded sample of the workload: same
-    dimensionality, precision, parameters and seeded field, smaller box.  Returns
-    (site_updates, seconds, description)."""
+def oracle_sample(dims, prec, era_m, nsteps, threads, N, seed=1):
+    """Times the oracle as it stands on `threads` host threads on the workload's own lattice: seeded init
+    (untimed), `nsteps` PRS steps, one diagnostics pass.  Returns a dict with the times and the metric at the
+    bench's cadence: SUBSTEPS steps + 1 diagnostics pass per cycle, i.e. value = SUBSTEPS N^d /
+    (SUBSTEPS t_step + t_diag) -- the same quantity the GPU arm reports, from a bounded sample of the cycle."""
     from oracle import binding as ref
 
-    if N is None:
-        N = 512 if dims == 3 else 8192
     sim = ref.RefSim(dims, N, prec, era_m=era_m, seed=seed, threads=threads)
-    sim.init(1.0)
     t0 = time.perf_counter()
+    sim.init(1.0)
+    t1 = time.perf_counter()
     sim.step(nsteps)
+    t2 = time.perf_counter()
     d = sim.diagnostics()
-    dt = time.perf_counter() - t0
+    t3 = time.perf_counter()
     sim.close()
-    desc = "%dD %d^%d %s, %d PRS steps + 1 diagnostics pass, %d thread(s); rho=%.5f" % (
-        dims, N, dims, "FP32" if prec == 0 else "FP64", nsteps, threads, d["rho"])
-    return N ** dims * nsteps, dt, desc
+    t_step, t_diag = (t2 - t1) / nsteps, t3 - t2
+    S = N ** dims
+    return {"N": N, "nsteps": nsteps, "t_init_s": t1 - t0, "t_step_s": t_step, "t_diag_s": t_diag,
+            "value": SUBSTEPS * S / (SUBSTEPS * t_step + t_diag), "steps_only_value": S / t_step,
+            "desc": "%dD %d^%d %s (the workload's own lattice), oracle as it stands on %d thread(s): %d PRS steps timed "
+                    "(%.2f s each) + 1 diagnostics pass (%.2f s, on the state after those steps); value = %d N^d / (%d t_step + t_diag), "
+                    "the bench cycle's cadence; seeded init %.1f s not timed; rho=%.5f"
+                    % (dims, N, dims, "FP32" if prec == 0 else "FP64", threads, nsteps, t_step, t_diag, SUBSTEPS, SUBSTEPS,
+                       t1 - t0, d["rho"])}
 
 
 def reduce_over_ranks(times_ms, counts, world, device="cpu"):
@@ -181,27 +187,49 @@ def aggregate_value(sites, substeps, steps, world, ms_total):
 
 
 def run_reference(args):
+    """--impl reference: the oracle on the host cores, on this arm's config, metric and unit.  One bench step = a
+    bounded sample of the cycle on the workload's own lattice: 2 PRS steps timed; the diagnostics pass is timed
+    once (in the warm-up) and enters every step's value at the cycle's cadence."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     dims, N, prec, era_m = CONFIGS[args.config]
     threads = host_threads()
-    nsub = 10
-    for _ in range(args.warmup if args.warmup < 2 else 1):       # one warm pass is enough for a CPU loop
-        oracle_sample(dims, prec, era_m, 2, threads, N=256 if dims == 3 else 4096)
-    total_updates, total_s, desc = 0, 0.0, ""
+    from oracle import binding as ref
+
+    S = N ** dims
+    nsub = 2
+    sim = ref.RefSim(dims, N, prec, era_m=era_m, seed=1, threads=threads)
+    t0 = time.perf_counter()
+    sim.init(1.0)
+    t_init = time.perf_counter() - t0
+    for _ in range(max(1, min(args.warmup, 1))):                 # one warm pass is enough for a CPU loop
+        sim.step(1)
+    t0 = time.perf_counter()
+    d = sim.diagnostics()
+    t_diag = time.perf_counter() - t0
+    t_steps = []
     for _ in range(args.steps):
-        u, s, desc = oracle_sample(dims, prec, era_m, nsub, threads)
-        total_updates += u
-        total_s += s
-    value = total_updates / total_s
+        t0 = time.perf_counter()
+        sim.step(nsub)
+        t_steps.append((time.perf_counter() - t0) / nsub)
+    sim.close()
+    t_step = sum(t_steps) / len(t_steps)
+    t_cycle = SUBSTEPS * t_step + t_diag
+    value = SUBSTEPS * S / t_cycle
+    desc = ("%dD %d^%d %s (the workload's own lattice), oracle as it stands on %d threads; per bench step %d PRS steps "
+            "timed (mean %.2f s per PRS step), diagnostics pass timed once (%.2f s); value = %d N^d / (%d t_step + t_diag) "
+            "(the cycle's cadence); seeded init %.1f s not timed; rho=%.5f"
+            % (dims, N, dims, "FP32" if prec == 0 else "FP64", threads, nsub, t_step, t_diag, SUBSTEPS, SUBSTEPS, t_init, d["rho"]))
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_cycle,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if prec == 0 else "f64", "data": "synthetic",
-        "config": {"workload": args.config, "dims": dims, "N": N, "era_m": era_m, "substeps": SUBSTEPS,
-                   "note": "oracle timed on a bounded sample of this workload (see cpu_baseline.sample)"},
+        "config": {"workload": args.config, "dims": dims, "N": N, "era_m": era_m, "alpha": 3.0, "deta": 0.1,
+                   "W0": 10.0, "substeps_per_step": SUBSTEPS, "diagnostics_per_step": 1,
+                   "note": "ms_per_step = one cycle of %d PRS steps + 1 diagnostics pass, extrapolated from the timed sample "
+                           "(cpu_baseline.sample)" % SUBSTEPS},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -287,125 +315,186 @@ def run_gpu(args):
         if world > 1:
             dist.destroy_process_group()
         return 0
+    leg = time_leg(args, args.config, args.steps, args.warmup, world, rank, local, barrier, with_e2e=True, sample_clocks=True)
+
+    # ---- the other precision of BASELINE.json's metric ("3D 1024^3 FP32/FP64"): a short FP64 leg of the same workload,
+    # its own events and roofline, outside the FP32 timed region
+    also = None
+    if args.config == DEFAULT_CONFIG and not args.no_also:
+        try:
+            other = time_leg(args, "3d_1024_f64_rad", max(2, min(args.steps, 3)), 3, world, rank, local, barrier,
+                             with_e2e=False, sample_clocks=False)
+            also = {"3d_1024_f64_rad": {k: other[k] for k in ("value", "unit", "dtype", "steps", "warmup", "ms_per_step",
+                                                                "roofline", "gpu_launches", "last_diag")}}
+        except Exception as exc:
+            also = {"3d_1024_f64_rad": {"error": str(exc)[:200]}}
+
+    # ---- oracle on the host cores, rank 0, N=1 only: the workload's own lattice, the cycle's cadence
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        threads = host_threads()
+        o = oracle_sample(dims, prec, era_m, 2, threads, N)
+        o1 = oracle_sample(dims, prec, era_m, 2, 1, 256 if dims == 3 else 4096)
+        cpu = {"value": o["value"], "unit": UNIT, "cores": threads, "kind": "oracle", "sample": o["desc"],
+               "steps_only_value": o["steps_only_value"],
+               "single_thread_value": o1["value"], "single_thread_sample": o1["desc"]}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": leg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": leg["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": leg["dtype"], "data": "synthetic",
+            "config": leg["config"], "roofline": leg["roofline"], "cpu_baseline": cpu, "e2e": leg["e2e"],
+            "gpu_launches": leg["gpu_launches"], "clocks": leg["clocks"], "last_diag": leg["last_diag"], "also": also,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def time_leg(args, config, steps, warmup, world, rank, local, barrier, with_e2e, sample_clocks):
+    """One workload: W untimed cycles, then exactly K timed ones (device clock, max over ranks), the step kernel's
+    own events, optionally the end-to-end cycle with host buffers.  One cycle = SUBSTEPS PRS steps + 1 diagnostics pass."""
+    import torch
+
+    import paper_1710_10420_b200 as prs
+    from paper_1710_10420_b200 import prs as binding
+
+    dims, N, prec, era_m = CONFIGS[config]
+    S = N ** dims
+    bpu = BYTES_PER_SITE_UPDATE[prec]
     sim = prs.Simulation(dims, N, prec, era_m=era_m, seed=rank + 1)
     if args.kernel:
         sim.set_step_kernel({"generic": prs.KERNEL_GENERIC, "tiled": prs.KERNEL_TILED, "tb2": prs.KERNEL_TB2,
                              "tbs": prs.KERNEL_TBS}[args.kernel])
-    if args.tbs_rows != 1:
+    if args.tbs_rows:
         sim.set_option(binding.OPT_TBS_ROWS, args.tbs_rows)
+    if args.tbs_loader:
+        sim.set_option(binding.OPT_TBS_LOADER, args.tbs_loader)
     sim.init(1.0)
     stream = torch.cuda.current_stream()
+    # what prs_step(SUBSTEPS) launches first is its main kernel; the cycle is issued as prs_step(main) + prs_step(rest)
+    # so that the main kernel's launches -- and nothing else -- sit between their own pair of events
+    sim.step(SUBSTEPS)
+    info = sim.step_launch_info()
+    spl = info["steps_per_launch"]
+    main_steps = (SUBSTEPS // spl) * spl
+    main_launches = main_steps // spl
 
     def hot_path(ev=None):
         if ev:
             ev[0].record(stream)
-        sim.step(SUBSTEPS)
+        sim.step(main_steps)
         if ev:
             ev[1].record(stream)
+        if SUBSTEPS > main_steps:
+            sim.step(SUBSTEPS - main_steps)
         return sim.diagnostics()
 
-    for _ in range(args.warmup):
+    sim.diagnostics()
+    for _ in range(max(0, warmup - 1)):
         hot_path()
-    # ---- timed region: exactly K steps, device clock, max over ranks
+    sim.step(main_steps)
+    launch = sim.step_launch_info()                              # the kernel the timed region launches
+    sim.step(SUBSTEPS - main_steps)
+    sim.diagnostics()
+    # ---- timed region: exactly K cycles, device clock, max over ranks
     sampler = ClockSampler(local)
-    if rank == 0:
+    if rank == 0 and sample_clocks:
         sampler.start()
-    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = sim.kernel_launches
     barrier()
     t0.record(stream)
     diag = None
-    for i in range(args.steps):
+    for i in range(steps):
         diag = hot_path(kev[i])
     t1.record(stream)
     barrier()
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop() if (rank == 0 and sample_clocks) else None
     launches = sim.kernel_launches - l0
     ms_total = t0.elapsed_time(t1)
     ms_kernels = sum(a.elapsed_time(b) for a, b in kev)
     (ms_total, ms_kernels), (launches,) = reduce_over_ranks([ms_total, ms_kernels], [launches], world, "cuda")
-    value = aggregate_value(S, SUBSTEPS, args.steps, world, ms_total)
-    step_kernel_launches = SUBSTEPS * args.steps
-    step_kernel = sim.get_info(binding.INFO_STEP_KERNEL)
-    # PRS steps the dominant kernel advances per launch; a prs_step(50) of the four-step kernel is 12
-    # four-step launches and one two-step launch, so launch_ms is the time per steps_per_launch steps
-    tbs_steps = 4 if dims == 3 else (8 if prec == 0 else 6)          # the library's defaults (prs.h, PRS_OPT_TBS_STEPS)
-    steps_per_launch = {prs.KERNEL_TB2: 2, prs.KERNEL_TBS: tbs_steps}.get(step_kernel, 1)
-    launch_ms = ms_kernels / (step_kernel_launches / steps_per_launch)
-    achieved = S * steps_per_launch * bpu / (launch_ms * 1e-3) / 1e9
+    value = aggregate_value(S, SUBSTEPS, steps, world, ms_total)
+    launch_ms = ms_kernels / (steps * main_launches)
+    algorithmic = S * spl * bpu                                  # north_star: 16 B (32 B) per site-update, single-step roofline
+    achieved = algorithmic / (launch_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak_gbs()
-    kernel_name = {1: "generic", 2: "tiled", 3: "tb2", 4: "tbs"}.get(step_kernel, str(step_kernel))
+    traffic, traffic_src = ncu_traffic_for(launch)
+    compulsory = S * bpu                                         # one read + one write of both fields per LAUNCH (SURVEY 8(d): 16/s B per site-update)
+    own = {"compulsory_bytes_per_launch": compulsory,
+           "frac_of_compulsory_traffic": compulsory / (launch_ms * 1e-3) / 1e9 / peak}
+    if traffic:
+        own["frac_of_own_traffic"] = traffic / (launch_ms * 1e-3) / 1e9 / peak
+    else:
+        own["frac_of_own_traffic"] = None
+    kernel_name = {1: "generic", 2: "tiled", 3: "tb2", 4: "tbs", 5: "cluster"}.get(sim.get_info(binding.INFO_STEP_KERNEL), "?")
+    fbytes = S * (4 if prec == 0 else 8)
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
     e2e = None
-    fbytes = S * (4 if prec == 0 else 8)
-    try:
-        dt = torch.float32 if prec == 0 else torch.float64
-        hphi = torch.empty(S, dtype=dt, pin_memory=True)
-        hpd = torch.empty(S, dtype=dt, pin_memory=True)
-        sim.copy_out_to(hphi, hpd)
-        n_e2e = max(1, min(args.steps, 2))
-        step0 = sim.get_info(binding.INFO_STEP)
-
-        def e2e_step(k):
-            sim.copy_in(hphi, hpd, eta0=1.0, step=step0 + k * SUBSTEPS)
-            sim.step(SUBSTEPS)
-            d = sim.diagnostics()
+    if with_e2e:
+        try:
+            dt = torch.float32 if prec == 0 else torch.float64
+            hphi = torch.empty(S, dtype=dt, pin_memory=True)
+            hpd = torch.empty(S, dtype=dt, pin_memory=True)
             sim.copy_out_to(hphi, hpd)
-            return d
+            n_e2e = max(1, min(steps, 2))
+            step0 = sim.get_info(binding.INFO_STEP)
 
-        e2e_step(0)                                            # warm the copy path once
-        barrier()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        for k in range(n_e2e):
-            e2e_step(k + 1)
-        b.record(stream)
-        barrier()
-        ms_e2e = a.elapsed_time(b)
-        (ms_e2e,), _ = reduce_over_ranks([ms_e2e], [], world, "cuda")
-        e2e = {"value": aggregate_value(S, SUBSTEPS, n_e2e, world, ms_e2e), "unit": UNIT,
-               "h2d_bytes_per_step": 2 * fbytes, "d2h_bytes_per_step": 2 * fbytes + 24,
-               "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e,
-               "what": "prs_copy_in(pinned host) + %d prs_step + prs_diagnostics + prs_copy_out(pinned host)" % SUBSTEPS}
-        del hphi, hpd
-    except Exception as exc:                                   # e.g. not enough pinned host memory
-        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 2 * fbytes, "d2h_bytes_per_step": 2 * fbytes + 24,
-               "error": str(exc)[:200]}
+            def e2e_step(k):
+                sim.copy_in(hphi, hpd, eta0=1.0, step=step0 + k * SUBSTEPS)
+                sim.step(SUBSTEPS)
+                d = sim.diagnostics()
+                sim.copy_out_to(hphi, hpd)
+                return d
 
-    # ---- oracle on the host cores, rank 0, N=1 only
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        threads = host_threads()
-        u, s, desc = oracle_sample(dims, prec, era_m, 10, threads)
-        u1, s1, desc1 = oracle_sample(dims, prec, era_m, 4, 1, N=256 if dims == 3 else 4096)
-        cpu = {"value": u / s, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
-               "single_thread_value": u1 / s1, "single_thread_sample": desc1}
-
-    if rank == 0:
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if prec == 0 else "f64", "data": "synthetic",
-            "config": {"workload": args.config, "dims": dims, "N": N, "era_m": era_m, "alpha": 3.0, "deta": 0.1,
-                       "W0": 10.0, "substeps_per_step": SUBSTEPS, "diagnostics_per_step": 1,
-                       "parallelism": "replicas x%d (no sharding, no collective)" % world,
-                       "l2": "state (%.1f GiB) exceeds L2; no flush needed" % (4 * fbytes / 2 ** 30),
-                       "step_kernel": kernel_name, "tbs_rows_per_thread": args.tbs_rows},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((args.config, kernel_name)),
-                         "kernel": "step kernel", "launch_ms": launch_ms, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": S * steps_per_launch * bpu,
-                         "step_kernel_share_of_step": ms_kernels / ms_total},
-            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-            "last_diag": {k: diag[k] for k in ("step", "eta", "link_count", "wall_sites", "rho", "gv2")},
-        }
-        print(json.dumps(line))
+            e2e_step(0)                                            # warm the copy path once
+            barrier()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for k in range(n_e2e):
+                e2e_step(k + 1)
+            b.record(stream)
+            barrier()
+            ms_e2e = a.elapsed_time(b)
+            (ms_e2e,), _ = reduce_over_ranks([ms_e2e], [], world, "cuda")
+            e2e = {"value": aggregate_value(S, SUBSTEPS, n_e2e, world, ms_e2e), "unit": UNIT,
+                   "h2d_bytes_per_step": 2 * fbytes, "d2h_bytes_per_step": 2 * fbytes + 24,
+                   "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e,
+                   "what": "prs_copy_in(pinned host) + %d prs_step + prs_diagnostics + prs_copy_out(pinned host)" % SUBSTEPS}
+            del hphi, hpd
+        except Exception as exc:                                   # e.g. not enough pinned host memory
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 2 * fbytes, "d2h_bytes_per_step": 2 * fbytes + 24,
+                   "error": str(exc)[:200]}
+    out = {
+        "value": value, "unit": UNIT, "dtype": "f32" if prec == 0 else "f64", "steps": steps, "warmup": warmup,
+        "ms_per_step": ms_total / steps, "gpu_launches": launches, "clocks": clocks, "e2e": e2e,
+        "config": {"workload": config, "dims": dims, "N": N, "era_m": era_m, "alpha": 3.0, "deta": 0.1,
+                   "W0": 10.0, "substeps_per_step": SUBSTEPS, "diagnostics_per_step": 1,
+                   "parallelism": "replicas x%d (no sharding, no collective)" % world,
+                   "l2": "state (%.1f GiB) exceeds L2; no flush needed" % (4 * fbytes / 2 ** 30) if 4 * fbytes > (1 << 28)
+                         else "state (%.1f MiB) fits in L2: HBM fractions are not meaningful for this workload" % (4 * fbytes / 2 ** 20),
+                   "step_kernel": kernel_name},
+        "roofline": dict({"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                          "traffic": traffic, "traffic_source": traffic_src,
+                          "what": "achieved / frac: the north_star single-step roofline (16 B FP32 / 32 B FP64 per site-update x "
+                                  "site-updates per launch / launch time): above 1 because one launch advances several steps per "
+                                  "pass over HBM; frac_of_own_traffic: measured DRAM bytes per launch / launch time / peak, i.e. "
+                                  "how close the kernel is to being HBM-bound on the bytes it really moves",
+                          "kernel": launch["kernel"], "grid": launch["grid"], "block": launch["block"],
+                          "steps_per_launch": spl, "launches_timed": steps * main_launches, "launch_ms": launch_ms,
+                          "peak_source": peak_src, "algorithmic_bytes_per_launch": algorithmic,
+                          "step_kernel_share_of_step": ms_kernels / ms_total}, **own),
+        "last_diag": {k: diag[k] for k in ("step", "eta", "link_count", "wall_sites", "rho", "gv2")},
+    }
     sim.close()
-    if world > 1:
-        dist.destroy_process_group()
-    return 0
+    del sim
+    torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -417,8 +506,11 @@ def main():
     ap.add_argument("--config", default=DEFAULT_CONFIG, choices=sorted(CONFIGS))
     ap.add_argument("--kernel", default=None, choices=["generic", "tiled", "tb2", "tbs"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--tbs-rows", type=int, default=1, choices=[1, 2],
-                    help="3D multi-step kernel: rows per thread (PRS_OPT_TBS_ROWS; 2 = step3d_tbr_kernel)")
+    ap.add_argument("--tbs-rows", type=int, default=0, choices=[0, 1, 2],
+                    help="3D multi-step kernel: rows per thread (PRS_OPT_TBS_ROWS; 0 = the library's choice)")
+    ap.add_argument("--tbs-loader", type=int, default=0, choices=[0, 1, 2],
+                    help="3D multi-step kernel: ring loader (PRS_OPT_TBS_LOADER; 1 = cp.async, 0 / 2 = TMA bulk copies)")
+    ap.add_argument("--no-also", action="store_true", help="skip the FP64 leg that follows the default workload")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slabs"],
                     help="replicas (default; the contract's line) or one lattice as z slabs (opt-in)")
     ap.add_argument("--slabs", type=int, default=8, help="single process, --decomposition slabs: slabs on this GPU")

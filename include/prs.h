@@ -70,9 +70,10 @@ enum {
     PRS_OPT_TB2_TILE_Y  = 6,   /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
     PRS_OPT_TBS_STEPS   = 7,   /* steps per pass of the multi-step kernel: 3 or 4, in 2D also 6 or 8;
                                 * default 4 in 3D, in 2D 8 (FP32) or 6 (FP64)                       */
-    PRS_OPT_TBS_ROWS    = 8,   /* tuning, 3D multi-step kernel: rows of the tile per thread, 1 (default) or
+    PRS_OPT_TBS_ROWS    = 8,   /* tuning, 3D multi-step kernel: rows of the tile per thread: 1 (step3d_tbs_kernel),
                                 * 2 (step3d_tbr_kernel: half the shared-memory traffic, taller tiles;
-                                * bit-identical; about 3 % faster in FP32, slower in FP64)            */
+                                * bit-identical) or 0 = auto (default): 2 in FP32 where the bulk loader
+                                * applies (1024^3: 17 % faster), else 1                                */
     PRS_OPT_TBS_LOADER  = 9    /* tuning, 3D multi-step kernel: how the shared-memory rings are filled: 0 (default)
                                 * = TMA bulk copies of whole tile rows completing on mbarriers where a lattice
                                 * row holds >= 32 16-byte vectors, else per-thread cp.async; 1 = always cp.async;

@@ -409,7 +409,7 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
     // measured, 16384^2, site-updates/s: FP32 1.29e12 (S = 4), 1.76e12 (6), 1.95e12 (8); FP64 6.8e11 (4), 9.5e11 (6), 8.9e11 (8)
     h->opt_tbs_steps = (dims == 3) ? 4 : (precision == PRS_F32 ? 8 : 6);
-    h->opt_tbs_rows = 1;
+    h->opt_tbs_rows = 0;                          // auto (prs_launch_tbs.cuh)
     h->opt_tbs_loader = 0;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     memset(&h->main_launch, 0, sizeof(h->main_launch));
@@ -753,8 +753,8 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             h->opt_tbs_steps = (int)value;
             return PRS_OK;
         case PRS_OPT_TBS_ROWS:
-            if (value != 1 && !(value == 2 && h->dims == 3))
-                return fail(h, PRS_ERR_INVALID_ARG, "tbs_rows must be 1 or, in 3D, 2");
+            if (value != 0 && value != 1 && !(value == 2 && h->dims == 3))
+                return fail(h, PRS_ERR_INVALID_ARG, "tbs_rows must be 0 (auto), 1 or, in 3D, 2");
             h->opt_tbs_rows = (int)value;
             return PRS_OK;
         case PRS_OPT_TBS_LOADER:

@@ -29,10 +29,13 @@ namespace prs {
 
 template <typename T, int S, int TY>
 constexpr size_t tbr_smem_bytes() {
-    return (size_t)(4 + 4 + 2 * (S - 1)) * (TY + 2 * S) * 32 * 16;
+    return (size_t)(4 + 4 + 2 * (S - 1)) * (TY + 2 * S) * 32 * 16 + 64;       // + four mbarriers (bulk loader)
 }
 
-template <typename T, int ARITH, int S, int TY>
+// BULK: the rings are filled by TMA bulk copies (see step3d_tbs_kernel): one elected lane per warp copies the
+// warp's two rows of both rings, 512 bytes each (two runs where the row straddles the periodic seam in x); the
+// first warp, which runs a single stage, waits on the slot's mbarrier before it joins the CTA barrier.
+template <typename T, int ARITH, int S, int TY, bool BULK>
 __global__ void __launch_bounds__(16 * (TY + 2 * S), (TY + 2 * S <= 16) ? 2 : 1)
 step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                   T* __restrict__ phidot_out, int N, int ZC, StepCoefs<T, S> coefs, ZRange zr) {
@@ -70,7 +73,11 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 
     PackCoef<T> pc[S];
 #pragma unroll
-    for (int s = 0; s < S; ++s) pc[s].template set<3>(coefs.k[s]);
+    for (int s = 0; s < S; ++s) {
+        pc[s].template set<3>(coefs.k[s]);
+        // 1/phi0^2 and deta do not depend on the step (prs_host.cuh, coef_at): one register serves all stages
+        pc[s].I = pc[0].I; pc[s].deta = pc[0].deta;
+    }
 
     // unsigned 32-bit indices of 16-byte vectors, as in step3d_tbs_kernel
     const V* const gA = reinterpret_cast<const V*>(phi);
@@ -81,7 +88,28 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
     const unsigned colv = (unsigned)y0 * (unsigned)NQ + (unsigned)q; // the lower row's column within a plane
     const unsigned dhi = ((unsigned)y1 - (unsigned)y0) * (unsigned)NQ;   // to the upper row's (modulo 2^32)
     int zl = wrap_mod(z0 - S, zr.nz);
-    unsigned il = (unsigned)zl * NNv + colv;                         // load cursor: issue i = plane a = i
+    // bulk loader: mbarriers, and the pair's rows as warp-uniform values (a shuffle from lane 0: UBLKCP takes
+    // uniform registers only)
+    const unsigned bars = smem_u32(tbr_smem + (size_t)(4 + 4 + 2 * (S - 1)) * PLANE * 16);       // full[4], 8 bytes each
+    if constexpr (BULK) {
+        if (me == 0) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) mbar_init(bars + 8 * u, RP);                               // one arrival per warp
+            mbar_init_fence();
+        }
+        __syncthreads();
+    }
+    const int pr_u = BULK ? __shfl_sync(0xffffffffu, pr, 0) : pr;
+    const int q0 = wrap_mod(XOUT * (int)blockIdx.x - XH, NQ);       // first vector of the tile's rows (periodic)
+    const unsigned len0 = (unsigned)min(32, NQ - q0) * 16u, len1 = 512u - len0;   // bytes before / after the x seam
+    const unsigned rowA = smem_u32(tbr_smem) + (unsigned)pr_u * 1024u;             // the pair's lower row of ring A, slot 0
+    const unsigned rowP = rowA + 4u * PLANE * 16u;
+    const bool leader = BULK ? elect_one() : false;
+    const int yu = TY * (int)blockIdx.y - S + 2 * pr_u;
+    const unsigned rowv = (unsigned)wrap_mod(yu, N) * (unsigned)NQ + (unsigned)q0;                // lower row, first run
+    const unsigned dhu = ((unsigned)wrap_mod(yu + 1, N) - (unsigned)wrap_mod(yu, N)) * (unsigned)NQ;
+    // load cursor (issue i = plane a = i): of this thread's column (cp.async) or of the warp's lower row (bulk)
+    unsigned il = (unsigned)zl * NNv + (BULK ? rowv : colv);
     int left_to_wrap = zr.nz - zl;                                   // issues until z wraps to 0
     unsigned io = (unsigned)z0 * NNv + colv;                         // store cursor
 
@@ -89,22 +117,47 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
         constexpr int NS = decltype(ns_tag)::value;                  // stages this pair runs (>= 1)
         int ni = 0;
         auto issue = [&](int slot_a, int slot_p) {
-            if (ni < niter + 2) {
-                cp_async16(sA + slot_a * PLANE, gA + il);
-                cp_async16(sA + slot_a * PLANE + 32, gA + (il + dhi));
-            }
-            if (ni >= 1 && ni <= niter) {
-                cp_async16(sP + slot_p * PLANE, gP + il);
-                cp_async16(sP + slot_p * PLANE + 32, gP + (il + dhi));
+            if constexpr (BULK) {
+                if (leader) {          // unconditional, as in step3d_tbs_kernel: every issue is the same four copies
+                    const unsigned bar = bars + 8u * (unsigned)slot_a;
+                    mbar_arrive_expect_tx(bar, 2048u);
+                    const unsigned d = rowA + (unsigned)slot_a * (PLANE * 16u), e = rowP + (unsigned)slot_p * (PLANE * 16u);
+                    bulk_g2s(d, gA + il, len0, bar);
+                    bulk_g2s(d + 512u, gA + (il + dhu), len0, bar);
+                    bulk_g2s(e, gP + il, len0, bar);
+                    bulk_g2s(e + 512u, gP + (il + dhu), len0, bar);
+                    if (len1) {
+                        bulk_g2s(d + len0, gA + (il - (unsigned)q0), len1, bar);
+                        bulk_g2s(d + 512u + len0, gA + (il + dhu - (unsigned)q0), len1, bar);
+                        bulk_g2s(e + len0, gP + (il - (unsigned)q0), len1, bar);
+                        bulk_g2s(e + 512u + len0, gP + (il + dhu - (unsigned)q0), len1, bar);
+                    }
+                }
+            } else {
+                if (ni < niter + 2) {
+                    cp_async16(sA + slot_a * PLANE, gA + il);
+                    cp_async16(sA + slot_a * PLANE + 32, gA + (il + dhi));
+                }
+                if (ni >= 1 && ni <= niter) {
+                    cp_async16(sP + slot_p * PLANE, gP + il);
+                    cp_async16(sP + slot_p * PLANE + 32, gP + (il + dhi));
+                }
             }
             ++ni; il += NNv;
             if (--left_to_wrap == 0) { il -= zr.wrap; left_to_wrap = zr.nz; }   // modulo 2^32, exact
         };
         issue(0, 3); issue(1, 0); issue(2, 1);
-        cp_async_commit();
-        issue(3, 2);
-        cp_async_commit();
-        cp_async_wait<1>();
+        unsigned ph[4] = {1u, 1u, 0u, 0u};      // parity of the next phase to wait for on each slot's mbarrier
+        if constexpr (BULK) {
+            issue(3, 2);
+            if (pr_u == 0) { mbar_wait(bars + 0, 0u); mbar_wait(bars + 8, 0u); }       // planes 0 and 1 have landed
+            __syncthreads();
+        } else {
+            cp_async_commit();
+            issue(3, 2);
+            cp_async_commit();
+            cp_async_wait<1>();
+        }
         // register windows per stage and row: input field at planes a_s-1, a_s; phidot input at a_s
         V wprev[S][2], wcur[S][2], qcur[S][2];
 #pragma unroll
@@ -118,10 +171,17 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             constexpr int U = decltype(u_tag)::value, PAR = U & 1;
             constexpr int ACTRAW = decltype(act_tag)::value;
             constexpr int ACT = (NS > ACTRAW) ? ACTRAW : NS;
-            cp_async_wait<1>();                 // group j has landed for this thread
+            if constexpr (BULK) {
+                if constexpr (NS == 1) {        // the first warp runs one stage: it has the time to wait for issue j+2
+                    if (pr_u == 0) mbar_wait(bars + 8u * (unsigned)((U + 2) & 3), ph[(U + 2) & 3]);
+                    ph[(U + 2) & 3] ^= 1u;
+                }
+            } else {
+                cp_async_wait<1>();             // group j has landed for this thread
+            }
             __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
             issue(U, (U + 3) & 3);              // issue j+4: plane j+4 takes the slot of plane j
-            cp_async_commit();
+            if constexpr (!BULK) cp_async_commit();
             V carry[2], qout[S][2];
             {   // stage 0 on plane a = j+1
                 const V zp0 = sA[((U + 2) & 3) * PLANE], zp1 = sA[((U + 2) & 3) * PLANE + 32];
@@ -186,7 +246,7 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             if (j + 3 >= niter) break;
             iteration(integral_constant<int, (J0 + 3) & 3>{}, integral_constant<int, S>{});
         }
-        cp_async_wait<0>();
+        if constexpr (!BULK) cp_async_wait<0>();
     };
     const int nsp = 2 * min(pr, RP - 1 - pr) + 1;                    // stages the pair's better row is good for
     if (nsp >= S) march(integral_constant<int, S>{});

@@ -159,7 +159,11 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 
     PackCoef<T> pc[S];
 #pragma unroll
-    for (int s = 0; s < S; ++s) pc[s].template set<3>(coefs.k[s]);
+    for (int s = 0; s < S; ++s) {
+        pc[s].template set<3>(coefs.k[s]);
+        // 1/phi0^2 and deta do not depend on the step (prs_host.cuh, coef_at): one register serves all stages
+        pc[s].I = pc[0].I; pc[s].deta = pc[0].deta;
+    }
 
     // Unsigned 32-bit indices of 16-byte vectors (the host checks N^3 / W <= 2^31, so that the cursor,
     // which runs one lattice length past the end before it wraps, stays below 2^32).
@@ -342,7 +346,11 @@ step2d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
 
     PackCoef<T> pc[S];
 #pragma unroll
-    for (int s = 0; s < S; ++s) pc[s].template set<2>(coefs.k[s]);
+    for (int s = 0; s < S; ++s) {
+        pc[s].template set<2>(coefs.k[s]);
+        // 1/phi0^2 and deta do not depend on the step (prs_host.cuh, coef_at): one register serves all stages
+        pc[s].I = pc[0].I; pc[s].deta = pc[0].deta;
+    }
 
     // 32-bit indices of 16-byte vectors (the host checks N^2 / W < 2^30); one load cursor for both fields
     const V* const gA = reinterpret_cast<const V*>(phi);

@@ -46,7 +46,13 @@ cudaError_t launch_tbs_3d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     constexpr int TY = (sizeof(T) == 8) ? 20 : 16;
     constexpr int W = Pk<T>::W;
     const int N = (int)h->N, NQ = N / W;
-    if (h->opt_tbs_rows == 2) return launch_tbr_3d<T, ARITH, S>(h, p, v, pn, vn);      // PRS_OPT_TBS_ROWS
+    // Rows of the tile per thread (PRS_OPT_TBS_ROWS; 0 = auto).  Measured on B200, 1024^3, us per step at S = 4
+    // (cp.async | bulk loader): FP32 one row 1216 | 1157, two rows 1300 | 1034; FP64 one row 2556 | 2487, two rows
+    // 2618 | 2737 -- the two-row kernel pays off once the bulk loader has taken the LDGSTS out of the l1tex pipe, and
+    // only in FP32 (FP64 at two rows per thread runs 16 warps at the 128-register cap with spills).
+    const bool bulk_ok = NQ >= 32 && h->opt_tbs_loader != 1;
+    const int rows = h->opt_tbs_rows ? h->opt_tbs_rows : ((sizeof(T) == 4 && bulk_ok) ? 2 : 1);
+    if (rows == 2) return launch_tbr_3d<T, ARITH, S>(h, p, v, pn, vn);
     StepCoefs<T, S> ks;
     for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     constexpr int XOUT = tbs_xout<T, S>();
@@ -92,11 +98,6 @@ cudaError_t launch_tbr_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     StepCoefs<T, S> ks;
     for (int s = 0; s < S; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     const size_t smem = tbr_smem_bytes<T, S, TY>();
-    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
-    {
-        const cudaError_t e = ensure_dynamic_smem(step3d_tbr_kernel<T, ARITH, S, TY>, smem, h->device, configured);
-        if (e != cudaSuccess) return e;
-    }
     constexpr int XOUT = tbs_xout<T, S>();
     const unsigned gx = (unsigned)((NQ + XOUT - 1) / XOUT), gy = (unsigned)((N + TY - 1) / TY);
     ZRange zr = {N, 0, N, 0u};
@@ -106,9 +107,20 @@ cudaError_t launch_tbr_3d_ty(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     const int ZC = tbs_pick_zc(h, (long long)gx * gy, nzo, S);
     const dim3 grid(gx, gy, (unsigned)((nzo + ZC - 1) / ZC));
     const dim3 block(32, (TY + 2 * S) / 2, 1);
-    step3d_tbr_kernel<T, ARITH, S, TY><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+    const bool bulk = NQ >= 32 && h->opt_tbs_loader != 1;          // as in launch_tbs_3d
     char name[96];
-    snprintf(name, sizeof(name), "step3d_tbr_kernel<%s,%d,%d,%d>", type_name<T>(), ARITH, S, TY);
+    snprintf(name, sizeof(name), "step3d_tbr_kernel<%s,%d,%d,%d,%d>", type_name<T>(), ARITH, S, TY, bulk ? 1 : 0);
+    if (bulk) {
+        static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
+        const cudaError_t e = ensure_dynamic_smem(step3d_tbr_kernel<T, ARITH, S, TY, true>, smem, h->device, configured);
+        if (e != cudaSuccess) return e;
+        step3d_tbr_kernel<T, ARITH, S, TY, true><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+    } else {
+        static std::atomic<unsigned long long> configured{0};
+        const cudaError_t e = ensure_dynamic_smem(step3d_tbr_kernel<T, ARITH, S, TY, false>, smem, h->device, configured);
+        if (e != cudaSuccess) return e;
+        step3d_tbr_kernel<T, ARITH, S, TY, false><<<grid, block, smem, h->stream>>>(p, v, pn, vn, N, ZC, ks, zr);
+    }
     note_launch(h, name, grid, block, smem, S);
     return cudaGetLastError();
 }

@@ -61,3 +61,38 @@ def test_reference_arm_prints_on_rank_zero_only():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                           "--steps", "1", "--warmup", "0"], env=env, stdout=subprocess.PIPE, text=True, timeout=300)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_reference_arm_line_on_a_small_config():
+    """--impl reference times the oracle on the workload's own lattice and prints the contract's keys."""
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "2d_256_f32_rad",
+                          "--steps", "2", "--warmup", "1"], stdout=subprocess.PIPE, text=True, timeout=300)
+    assert out.returncode == 0
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["metric"] == "site_updates_per_sec" and line["value"] > 0
+    assert line["config"]["workload"] == "2d_256_f32_rad" and line["config"]["N"] == 256
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] == line["value"]
+    assert line["e2e"] == {"value": line["value"], "unit": line["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "256^2" in line["cpu_baseline"]["sample"]
+
+
+def test_ncu_traffic_is_reported_only_for_the_kernel_that_was_launched(tmp_path, monkeypatch):
+    sys.path.insert(0, ROOT)
+    import bench
+
+    rec = {"captures": [{"profile": "x.md", "kernel": "step3d_tbr_kernel<float,2,4,24,1>", "grid": [9, 43, 8],
+                         "block": [32, 16, 1], "dram_bytes_read": 10, "dram_bytes_write": 5}]}
+    f = tmp_path / "ncu_traffic.json"
+    f.write_text(json.dumps(rec))
+    monkeypatch.setattr(bench, "NCU_TRAFFIC_FILE", str(f))
+    hit = {"kernel": "step3d_tbr_kernel<float,2,4,24,1>", "grid": [9, 43, 8], "block": [32, 16, 1]}
+    assert bench.ncu_traffic_for(hit)[0] == 15
+    for miss in (dict(hit, kernel="step3d_tbr_kernel<float,2,4,24,0>"), dict(hit, grid=[9, 43, 4]), dict(hit, block=[32, 24, 1])):
+        got, why = bench.ncu_traffic_for(miss)
+        assert got is None and "no committed ncu capture" in why
+    # the committed record parses and every entry names its profile summary, which exists
+    monkeypatch.undo()
+    if os.path.exists(bench.NCU_TRAFFIC_FILE):
+        for c in json.load(open(bench.NCU_TRAFFIC_FILE))["captures"]:
+            assert os.path.exists(os.path.join(ROOT, "profiles", c["profile"])), c["profile"]
+            assert len(c["grid"]) == 3 and len(c["block"]) == 3 and c["dram_bytes_read"] > 0
