@@ -61,31 +61,64 @@ def source_hash():
     return h.hexdigest()
 
 
-def is_current():
-    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
+# Build variants: "" = the product; "jitter" = the same sources with -DPRS_RACE_JITTER=1 (csrc/prs_arith.cuh: random
+# warp-uniform delays around every barrier and publication), used by tests/sanitize_kernels.py to look for races.
+VARIANTS = {"": [], "jitter": ["-DPRS_RACE_JITTER=1"]}
+
+
+def lib_path(variant=""):
+    return LIB if not variant else os.path.join(HERE, "libprs_%s.so" % variant)
+
+
+def is_current(variant=""):
+    lib, stamp = lib_path(variant), lib_path(variant) + ".srchash"
+    if not (os.path.exists(lib) and os.path.exists(stamp)):
         return False
-    with open(STAMP) as fh:
+    with open(stamp) as fh:
         return fh.read().strip() == source_hash()
 
 
-def _compile(unit):
-    name, src, flags = unit
-    obj = os.path.join(OBJDIR, name + ".o")
-    cmd = [_nvcc()] + NVCC_FLAGS + flags + ["-c", "-o", obj, os.path.join(CSRC, src)]
+def _compile(job):
+    (name, src, flags), objdir, extra = job
+    obj = os.path.join(objdir, name + ".o")
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + flags + ["-c", "-o", obj, os.path.join(CSRC, src)]
     res = subprocess.run(cmd, cwd=HERE, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     return name, obj, cmd, res
 
 
-def build(force=False, verbose=False, jobs=None):
-    """Compiles the translation units of csrc/ in parallel and links libprs.so; returns the library
-    path.  Raises on compiler failure."""
-    if not force and is_current():
-        return LIB
-    os.makedirs(OBJDIR, exist_ok=True)
+def build(force=False, verbose=False, jobs=None, variant=""):
+    """Compiles the translation units of csrc/ in parallel and links libprs.so (or libprs_<variant>.so); returns
+    the library path.  Raises on compiler failure.  Safe under concurrent callers (the ranks of a torchrun job):
+    the whole build runs under an exclusive lock on a file beside the library, into a per-process object
+    directory, and whoever gets the lock second finds the library current."""
+    import fcntl
+    import shutil
+
+    if variant not in VARIANTS:
+        raise ValueError("unknown build variant %r" % variant)
+    LIBV, STAMPV = lib_path(variant), lib_path(variant) + ".srchash"
+    if not force and is_current(variant):
+        return LIBV
+    with open(LIBV + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and is_current(variant):               # another process built it while we waited
+                return LIBV
+            return _build_locked(verbose, jobs, variant, LIBV, STAMPV)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose, jobs, variant, LIBV, STAMPV):
+    import shutil
+
+    objdir = os.path.join(OBJDIR, "%s.%d" % (variant or "product", os.getpid()))
+    shutil.rmtree(objdir, ignore_errors=True)
+    os.makedirs(objdir, exist_ok=True)
     jobs = jobs or int(os.environ.get("PRS_BUILD_JOBS", "0")) or min(len(units()), os.cpu_count() or 1)
     with ThreadPoolExecutor(max_workers=jobs) as pool:
-        results = list(pool.map(_compile, units()))
-    log = os.path.join(HERE, "build.log")
+        results = list(pool.map(_compile, [(u, objdir, VARIANTS[variant]) for u in units()]))
+    log = os.path.join(HERE, "build%s.log" % ("_" + variant if variant else ""))
     with open(log, "w") as fh:
         for name, obj, cmd, res in results:
             fh.write("### %s\n%s\n%s\n" % (name, " ".join(cmd), res.stdout))
@@ -94,7 +127,7 @@ def build(force=False, verbose=False, jobs=None):
     failed = [(name, res) for name, obj, cmd, res in results if res.returncode != 0]
     if failed:
         raise RuntimeError("nvcc failed on %s (see %s):\n%s" % (failed[0][0], log, failed[0][1].stdout[-4000:]))
-    tmp = LIB + ".tmp.%d" % os.getpid()
+    tmp = LIBV + ".tmp.%d" % os.getpid()
     cmd = [_nvcc(), "--shared", "-o", tmp] + [obj for name, obj, cmd, res in results]
     res = subprocess.run(cmd, cwd=HERE, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     with open(log, "a") as fh:
@@ -103,11 +136,14 @@ def build(force=False, verbose=False, jobs=None):
         if os.path.exists(tmp):
             os.remove(tmp)
         raise RuntimeError("link failed (see %s):\n%s" % (log, res.stdout[-4000:]))
-    os.replace(tmp, LIB)
-    with open(STAMP, "w") as fh:
+    os.replace(tmp, LIBV)
+    with open(STAMPV, "w") as fh:
         fh.write(source_hash() + "\n")
-    return LIB
+    if not verbose:
+        shutil.rmtree(objdir, ignore_errors=True)
+    return LIBV
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                variant="jitter" if "--jitter" in sys.argv else ""))

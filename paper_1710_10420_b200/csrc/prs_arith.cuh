@@ -13,6 +13,24 @@
 
 namespace prs {
 
+// Race hunting without a race checker (compute-sanitizer is closed on this pool's GPUs): a second build of the library
+// with -DPRS_RACE_JITTER=1 puts random, warp-uniform delays of up to a few microseconds at the points below -- before
+// and after every barrier, between a row's fetch and its publication, between the two halves of a stack push -- so that
+// an ordering that holds only because the warps of a CTA happen to run in step shows up as a wrong bit in
+// tests/sanitize_kernels.py (every result is compared with the one-thread-per-site kernel).  The delays change no value.
+#ifdef PRS_RACE_JITTER
+__device__ __forceinline__ void prs_jitter(unsigned salt) {
+    unsigned h = (blockIdx.x * 73856093u) ^ (blockIdx.y * 19349663u) ^ ((threadIdx.y + (threadIdx.x >> 5)) * 83492791u) ^
+                 (salt * 2654435761u) ^ (unsigned)clock();
+    h ^= h >> 13; h *= 0x5bd1e995u; h ^= h >> 15;
+    h = __shfl_sync(0xffffffffu, h, 0);                  // one decision per warp: the warp stays converged
+    if ((h & 3u) == 0u) __nanosleep(h >> 20);            // one warp in four sleeps up to 4 us
+}
+#define PRS_JITTER(salt) ::prs::prs_jitter(salt)
+#else
+#define PRS_JITTER(salt) ((void)0)
+#endif
+
 template <typename T> struct Ar;
 
 template <> struct Ar<float> {

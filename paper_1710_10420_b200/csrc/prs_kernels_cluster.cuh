@@ -90,7 +90,9 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
             *reinterpret_cast<V*>(pd + o) = vn;
         }
         // everyone has written phi^{n+1} and is done reading phi^n, which is overwritten next step
+        PRS_JITTER(1u + s);
         cluster.sync();
+        PRS_JITTER(40u + s);
     }
     const T* const fin = (nsteps & 1) ? bufB : bufA;
     for (int i = t; i < RNQ; i += CLUSTER_THREADS) {

@@ -140,9 +140,12 @@ step3d_tb2_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             constexpr int U = decltype(u_tag)::value;
             constexpr bool STAGE2 = decltype(s2_tag)::value && ROLE == 2;
             cp_async_wait<TB2_PF - 1>();        // group j has landed for this thread
+            PRS_JITTER(1u);
             __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
+            PRS_JITTER(2u);
             issue(U, (U + 3) & 3);              // issue j+4: phi^n plane j+4 takes the slot of plane j
             cp_async_commit();
+            PRS_JITTER(3u);
             if (ROLE == 0) return;
 
             // stage 1 on plane a = j+1

@@ -179,9 +179,12 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             } else {
                 cp_async_wait<1>();             // group j has landed for this thread
             }
+            PRS_JITTER(1u);
             __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
+            PRS_JITTER(2u);
             issue(U, (U + 3) & 3);              // issue j+4: plane j+4 takes the slot of plane j
             if constexpr (!BULK) cp_async_commit();
+            PRS_JITTER(3u);
             V carry[2], qout[S][2];
             {   // stage 0 on plane a = j+1
                 const V zp0 = sA[((U + 2) & 3) * PLANE], zp1 = sA[((U + 2) & 3) * PLANE + 32];
@@ -194,6 +197,7 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
                 V out0, out1;
                 packed_vector_update<T, 3, ARITH>(pc[0], wcur[0][0], l0, r0, ym, wcur[0][1], wprev[0][0], zp0, pd0, out0, qout[0][0]);
                 packed_vector_update<T, 3, ARITH>(pc[0], wcur[0][1], l1, r1, wcur[0][0], yp, wprev[0][1], zp1, pd1, out1, qout[0][1]);
+                PRS_JITTER(4u);
                 if (S > 1) { sB[(0 * 2 + PAR) * PLANE] = out0; sB[(0 * 2 + PAR) * PLANE + 32] = out1; }
                 wprev[0][0] = wcur[0][0]; wprev[0][1] = wcur[0][1];
                 wcur[0][0] = zp0; wcur[0][1] = zp1;
@@ -211,6 +215,7 @@ step3d_tbr_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
                 packed_vector_update<T, 3, ARITH>(pc[s], wcur[s][0], l0, r0, ym, wcur[s][1], wprev[s][0], carry[0], qcur[s][0], out0, qout[s][0]);
                 packed_vector_update<T, 3, ARITH>(pc[s], wcur[s][1], l1, r1, wcur[s][0], yp, wprev[s][1], carry[1], qcur[s][1], out1, qout[s][1]);
                 if constexpr (s < S - 1) {
+                    PRS_JITTER(5u + s);
                     sB[(s * 2 + PAR) * PLANE] = out0; sB[(s * 2 + PAR) * PLANE + 32] = out1;
                 } else {
                     if (st0) { oP[io] = qout[s][0]; oA[io] = out0; }

@@ -243,9 +243,12 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
             } else {
                 cp_async_wait<1>();             // group j has landed for this thread
             }
+            PRS_JITTER(1u);
             __syncthreads();                    // ... and for every thread; retires iteration j-1's reads
+            PRS_JITTER(2u);
             issue(U, (U + 3) & 3);              // issue j+4: phi^n plane j+4 takes the slot of plane j
             if constexpr (!BULK) cp_async_commit();
+            PRS_JITTER(3u);
             if constexpr (NS >= 1) {
                 V carry, qout[S];
                 {   // stage 0 on plane a = j+1
@@ -256,6 +259,7 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
                     const T right = __shfl_down_sync(0xffffffffu, K::first(wcur[0]), 1);
                     V out;
                     packed_vector_update<T, 3, ARITH>(pc[0], wcur[0], left, right, ym, yp, wprev[0], zp, pd, out, qout[0]);
+                    PRS_JITTER(4u);
                     if (S > 1) sB[(0 * 2 + PAR) * PLANE] = out;
                     wprev[0] = wcur[0]; wcur[0] = zp; carry = out;
                 }
@@ -268,6 +272,7 @@ step3d_tbs_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __
                     V out;
                     packed_vector_update<T, 3, ARITH>(pc[s], wcur[s], left, right, ym, yp, wprev[s], carry, qcur[s], out, qout[s]);
                     if constexpr (s < S - 1) {
+                        PRS_JITTER(5u + s);
                         sB[(s * 2 + PAR) * PLANE] = out;
                     } else {
                         if (store_ok) {

@@ -256,6 +256,7 @@ struct WallQueue {
         using O = VecOps<T>;
         if (__ballot_sync(0xffffffffu, wallmask != 0u) == 0u) return;
         acc.walls += __popc(wallmask);
+        PRS_JITTER(1u);
         __syncwarp();                           // pops of the previous call are done before slots are reused
 #pragma unroll
         for (int i = 0; i < O::W; ++i) {

@@ -49,7 +49,10 @@ def lib():
     """Loads (building first if the sources changed) paper_1710_10420_b200/libprs.so."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        # PRS_LIBRARY_VARIANT=jitter loads the race-hunting build (build.py VARIANTS; tests/sanitize_kernels.py)
+        import os
+
+        path = _build.build(variant=os.environ.get("PRS_LIBRARY_VARIANT", ""))
         L = C.CDLL(path)
         vp, i64, dbl, u64, ci, sz = C.c_void_p, C.c_int64, C.c_double, C.c_uint64, C.c_int, C.c_size_t
         L.prs_workspace_bytes.argtypes = [ci, i64, ci]

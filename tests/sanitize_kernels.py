@@ -1,6 +1,13 @@
-"""Drives every kernel of libprs on small ragged lattices, for runs under compute-sanitizer.
+"""Drives every kernel of libprs on small ragged lattices: for runs under compute-sanitizer where that tool is
+available, and -- since it is closed on this pool's GPUs -- with the library's race-hunting build:
 
     compute-sanitizer --tool racecheck|memcheck|initcheck|synccheck python -m tests.sanitize_kernels
+    PRS_LIBRARY_VARIANT=jitter python -m tests.sanitize_kernels          # libprs_jitter.so: -DPRS_RACE_JITTER=1
+
+The jitter build (csrc/prs_arith.cuh, build.py VARIANTS) puts random warp-uniform delays of up to 4 us before and after
+every barrier, before every publication of a row to shared memory and inside the wall-site stack, so that an ordering
+that holds only because the warps of a CTA run in step turns into a wrong bit here: every result is compared bit
+for bit with the one-thread-per-site kernel, which has no shared memory and no barrier.
 
 ("Race detection / sanitizers".)  The default step kernels are shared-memory pipelines whose
 correctness rests on one CTA barrier per plane and on cp.async group accounting; the sizes below make every
@@ -8,6 +15,7 @@ kind of tile appear: several tiles and z chunks, ragged last tiles in x and y, t
 lattices smaller than one tile.  Each result is also compared bit for bit with the generic one-thread-per-site
 kernel, so a run is a (small) parity test as well.  The summaries of the last run are in profiles/.
 """
+import os
 import sys
 
 import numpy as np
@@ -98,7 +106,10 @@ def main():
             group.close()
             whole.close()
             print("ok slabs N=%d x%d %s" % (N, world, "f32" if prec == prs.F32 else "f64"), flush=True)
-    print("sanitize_kernels: all kernels ran, %d launches, results identical to the generic kernel" % launches)
+    from paper_1710_10420_b200 import build as prs_build
+
+    print("sanitize_kernels: all kernels of %s ran, %d launches, results identical to the generic kernel"
+          % (os.path.basename(prs_build.lib_path(os.environ.get("PRS_LIBRARY_VARIANT", ""))), launches))
     return 0
 
 

@@ -794,3 +794,20 @@ def test_full_size_restart_parity_on_a_formed_network(dims, N, prec, era_m, eta,
                 else:
                     assert maxdiff(ap[inner], rp[inner]) <= TOL[prec] and maxdiff(av[inner], rv[inner]) <= TOL[prec]
     g.close()
+
+
+def test_race_hunting_build_gives_the_same_bits():
+    """compute-sanitizer is closed on this pool's GPUs, so races are hunted with a second build of the same sources
+    (-DPRS_RACE_JITTER=1: random warp-uniform delays of up to 4 us around every barrier, publication and stack push).
+    tests/sanitize_kernels.py drives every kernel with it on ragged lattices and compares each result bit for bit with
+    the generic kernel; an ordering that holds only because the warps run in step would fail there."""
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, PRS_LIBRARY_VARIANT="jitter")
+    out = subprocess.run([sys.executable, "-m", "tests.sanitize_kernels"], cwd=root, env=env, stdout=subprocess.PIPE,
+                         stderr=subprocess.STDOUT, text=True, timeout=900)
+    assert out.returncode == 0, out.stdout[-3000:]
+    assert "results identical to the generic kernel" in out.stdout
+    assert "libprs_jitter.so" in out.stdout
