@@ -64,7 +64,7 @@ typedef struct {
 enum {
     PRS_OPT_STEP_KERNEL = 1,   /* PRS_KERNEL_*                                   default AUTO     */
     PRS_OPT_ARITH       = 2,   /* PRS_ARITH_*                                    default FMA      */
-    PRS_OPT_DIAG_KERNEL = 3,   /* PRS_KERNEL_AUTO / GENERIC / TILED              default AUTO     */
+    PRS_OPT_DIAG_KERNEL = 3,   /* PRS_KERNEL_AUTO / GENERIC / TILED / BITS       default AUTO     */
     PRS_OPT_CHUNK       = 4,   /* tuning: planes (3D) / rows (2D) one CTA marches; 0 = auto        */
     PRS_OPT_TILE_Y      = 5,   /* tuning: rows per CTA of the 3D tiled kernel, 4 / 8 / 16          */
     PRS_OPT_TB2_TILE_Y  = 6,   /* tuning: output rows per CTA of the 3D two-step kernel, 4 / 8 / 12 / 28 */
@@ -88,6 +88,10 @@ enum {
     PRS_KERNEL_CLUSTER = 5,    /* small 2D boxes (N = 64, 128, 256): the state stays in the shared   *
                                 * memory of one 8-CTA thread-block cluster for up to 32 steps per    *
                                 * launch; bit-identical to single steps                              */
+    PRS_KERNEL_BITS    = 6,    /* PRS_OPT_DIAG_KERNEL only: diagnostics on packed sign bits -- one pass reads phi   *
+                                * and packs a bit per site, a second counts links and wall sites on the bit words *
+                                * and fetches phidot at wall sites only; N a multiple of 32 16-byte vectors; what *
+                                * AUTO takes from 2^26 sites up                                                   */
     PRS_KERNEL_TBS     = 4     /* PRS_OPT_TBS_STEPS steps per pass over HBM (2D and 3D), bit-identical *
                                 * to single steps; leftovers of a prs_step call go through TB2 and  *
                                 * TILED                                                             */

@@ -13,6 +13,7 @@
 #include "prs_kernels_generic.cuh"
 #include "prs_kernels_tiled.cuh"
 #include "prs_kernels_cluster.cuh"
+#include "prs_kernels_bits.cuh"
 
 using namespace prs;
 
@@ -34,7 +35,7 @@ inline bool args_ok(int dims, int64_t N, int precision) {
 inline size_t sites_of(int dims, int64_t N) { return dims == 3 ? (size_t)N * N * N : (size_t)N * N; }
 
 struct Layout {
-    size_t field_bytes, off_phi[2], off_pd[2], off_partials, off_result, total;
+    size_t field_bytes, off_phi[2], off_pd[2], off_partials, off_result, off_bits, total;
 };
 
 constexpr int SLAB_HALO = 4;                 // halo planes per side = the most steps one 3D launch takes
@@ -49,6 +50,7 @@ Layout layout_of_sites(size_t sites, int precision) {
     L.off_pd[1] = o; o += L.field_bytes;
     L.off_partials = o; o += align_up(sizeof(DiagPartial) * MAX_PARTIALS);
     L.off_result = o; o += align_up(sizeof(DiagPartial));
+    L.off_bits = o; o += align_up((sites + 7) / 8);             // one sign bit per site (prs_kernels_bits.cuh)
     L.total = o;
     return L;
 }
@@ -300,9 +302,19 @@ bool diag_tiled_supported(const prs_ctx* h) {
     return tiles <= MAX_PARTIALS;
 }
 
+// The packed-sign-bit pass (prs_kernels_bits.cuh): whole groups of 32 vectors per row.
+bool diag_bits_supported(const prs_ctx* h) {
+    const int W = vec_width(h->precision);
+    return h->N % (32 * W) == 0 && h->N <= (1 << 30);
+}
+
 int resolve_diag_kernel(const prs_ctx* h) {
     int want = h->opt_diag_kernel;
-    if (want == PRS_KERNEL_AUTO) want = diag_tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
+    if (want == PRS_KERNEL_AUTO) {
+        // the three launches of the bit pass pay off once reading phi dominates (measured)
+        if (diag_bits_supported(h) && h->S >= ((size_t)1 << 26)) want = PRS_KERNEL_BITS;
+        else want = diag_tiled_supported(h) ? PRS_KERNEL_TILED : PRS_KERNEL_GENERIC;
+    }
     return want;
 }
 
@@ -326,7 +338,28 @@ int diag_launch(prs_ctx* h) {
     const T* v = (const T*)h->pd[h->cur];
     const int kernel = resolve_diag_kernel(h);
     long long blocks;
-    if (kernel == PRS_KERNEL_TILED) {
+    if (kernel == PRS_KERNEL_BITS) {
+        constexpr int W = VecOps<T>::W;
+        const int N = (int)h->N, NG = N / (32 * W);
+        const long long rows_per_plane = (h->dims == 3) ? N : 1;
+        const long long nplanes = (h->dims == 3) ? h->NZ : N;            // 2D: a "plane" is a row
+        // rows to measure, and the rows whose signs they need (a slab: one halo plane on either side)
+        const long long p0 = h->slab ? h->halo : 0, p1 = h->slab ? h->halo + h->nz_own : nplanes;
+        const long long b0 = h->slab ? p0 - 1 : 0, b1 = h->slab ? p1 + 1 : nplanes;
+        const long long cap = (long long)h->sm_count * 16;
+        const long long sgroups = (b1 - b0) * rows_per_plane * NG;       // one warp each
+        const long long sblocks = std::min<long long>((sgroups + 7) / 8, cap);
+        sign_bits_kernel<T><<<(unsigned)sblocks, 256, 0, h->stream>>>(p, h->bits, N, b0 * rows_per_plane, b1 * rows_per_plane);
+        cudaError_t e0 = cudaGetLastError();
+        if (e0 != cudaSuccess) return cuda_fail(h, e0, "sign-bit kernel launch");
+        const long long lgroups = (p1 - p0) * rows_per_plane * NG;       // one thread each
+        blocks = std::min<long long>((lgroups + BITS_THREADS - 1) / BITS_THREADS, std::min<long long>(MAX_PARTIALS, cap));
+        if (h->dims == 3)
+            bit_links_kernel<T, 3><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, (int)h->NZ, p0 * rows_per_plane, p1 * rows_per_plane, V0, I, h->partials);
+        else
+            bit_links_kernel<T, 2><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, 1, p0, p1, V0, I, h->partials);
+        h->launches += 1;
+    } else if (kernel == PRS_KERNEL_TILED) {
         constexpr int W = VecOps<T>::W;
         const int N = (int)h->N;
         if (h->dims == 3) {
@@ -404,6 +437,7 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->pd[0] = h->ws + L.off_pd[0]; h->pd[1] = h->ws + L.off_pd[1];
     h->partials = (DiagPartial*)(h->ws + L.off_partials);
     h->d_result = (DiagPartial*)(h->ws + L.off_result);
+    h->bits = (unsigned*)(h->ws + L.off_bits);
     h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
     h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_FMA; h->opt_diag_kernel = PRS_KERNEL_AUTO;
     h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
@@ -705,7 +739,8 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
     if (!h) return PRS_ERR_INVALID_ARG;
     if (h->slab && option == PRS_OPT_STEP_KERNEL && value != PRS_KERNEL_AUTO && value != PRS_KERNEL_GENERIC && value != PRS_KERNEL_TBS)
         return fail(h, PRS_ERR_UNSUPPORTED, "a slab steps with the generic or the four-step kernel");
-    if (h->slab && (option == PRS_OPT_DIAG_KERNEL || option == PRS_OPT_TBS_STEPS) && value != PRS_KERNEL_AUTO && !(option == PRS_OPT_TBS_STEPS && value == SLAB_HALO))
+    if (h->slab && (option == PRS_OPT_DIAG_KERNEL || option == PRS_OPT_TBS_STEPS) && value != PRS_KERNEL_AUTO && !(option == PRS_OPT_TBS_STEPS && value == SLAB_HALO) &&
+        !(option == PRS_OPT_DIAG_KERNEL && value == PRS_KERNEL_BITS))
         return fail(h, PRS_ERR_UNSUPPORTED, "not configurable on a slab");
     switch (option) {
         case PRS_OPT_STEP_KERNEL:
@@ -733,6 +768,11 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             return PRS_OK;
         case PRS_OPT_DIAG_KERNEL:
             if (value == PRS_KERNEL_AUTO || value == PRS_KERNEL_GENERIC) { h->opt_diag_kernel = (int)value; return PRS_OK; }
+            if (value == PRS_KERNEL_BITS) {
+                if (!diag_bits_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "the sign-bit diagnostics pass needs N to be a multiple of 32 16-byte vectors");
+                h->opt_diag_kernel = (int)value;
+                return PRS_OK;
+            }
             if (value == PRS_KERNEL_TILED) {
                 if (!diag_tiled_supported(h)) return fail(h, PRS_ERR_UNSUPPORTED, "tiled diagnostics kernel cannot take this lattice");
                 h->opt_diag_kernel = (int)value;

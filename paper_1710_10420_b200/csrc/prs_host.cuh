@@ -30,6 +30,7 @@ struct prs_ctx {
     int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
     prs::DiagPartial* partials;
     prs::DiagPartial* d_result;
+    unsigned* bits;                           // one sign bit per site: scratch of the sign-bit diagnostics pass
     prs::DiagPartial* h_result;               // pinned host, 24 bytes
     double eta0;
     int64_t step;

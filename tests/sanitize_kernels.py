@@ -72,9 +72,10 @@ def main():
             assert run(2, N, prec, prs.KERNEL_CLUSTER, 35) == want
             print("ok step cluster            2D N=%-4d %s" % (N, "f32" if prec == prs.F32 else "f64"), flush=True)
         # diagnostics (tiled and generic) and the weighted area, early and on a forming network
-        for dims, N in ((3, 68), (3, 132), (2, 260)):
+        for dims, N in ((3, 68), (3, 132), (2, 260), (3, 128), (2, 256)):
             res = []
-            for dk in (prs.KERNEL_GENERIC, prs.KERNEL_TILED):
+            W = 4 if prec == prs.F32 else 2
+            for dk in (prs.KERNEL_GENERIC, prs.KERNEL_TILED) + ((prs.KERNEL_BITS,) if N % (32 * W) == 0 else ()):
                 g = prs.Simulation(dims, N, prec, seed=4)
                 g.set_option(binding.OPT_DIAG_KERNEL, dk)
                 g.init(1.0)
@@ -86,7 +87,7 @@ def main():
                 res.append(row)
                 launches += g.kernel_launches
                 g.close()
-            assert [(a, b) for a, b, _ in res[0]] == [(a, b) for a, b, _ in res[1]]
+            assert all([(a, b) for a, b, _ in res[0]] == [(a, b) for a, b, _ in r] for r in res[1:])
             print("ok diagnostics + weighted area %dD N=%-4d %s" % (dims, N, "f32" if prec == prs.F32 else "f64"), flush=True)
         # a lattice as two and three z slabs (init_slab_kernel, plane-range launches, halo copies)
         for N, world in ((68, 2), (132, 3)):

@@ -301,6 +301,58 @@ def test_diagnostics_match_on_snapshots(diag_kernel, prec, dims, N):
 
 
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 128), (2, 256), (2, 1152), (3, 64), (3, 128), (3, 192), (3, 256)])
+def test_sign_bit_diagnostics_match_on_snapshots(prec, dims, N):
+    """PRS_KERNEL_BITS (prs_kernels_bits.cuh: a pass that packs one sign bit per site, a pass that counts links and
+    wall sites on the bit words and fetches phidot at wall sites only) against the oracle on the GPU's exact bytes
+    and against the one-pass tiled kernel: on the white-noise start (every site a wall site: the stack path at full
+    load), while the network forms, and on a formed network (a few wall sites per warp)."""
+    W = 4 if prec == prs.F32 else 2
+    g = prs.Simulation(dims, N, prec, seed=4)
+    if N % (32 * W):
+        with pytest.raises(prs.PrsError) as e:
+            g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_BITS)
+        assert e.value.code == 2
+        return
+    g.init(1.0)
+    for nsteps in (0, 20, 60, 300):
+        g.step(nsteps)
+        g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_BITS)
+        db = g.diagnostics()
+        assert g.get_info(binding.INFO_DIAG_KERNEL) == prs.KERNEL_BITS
+        g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_TILED)
+        dt = g.diagnostics()
+        gp, gv = g.copy_out()
+        do = ref.diagnostics_of(gp, gv)                          # oracle on the GPU's exact bytes
+        for d in (dt, do):
+            assert db["link_count"] == d["link_count"] and db["wall_sites"] == d["wall_sites"]
+            assert abs(db["sum_ratio"] - d["sum_ratio"]) <= 1e-10 * max(d["sum_ratio"], 1e-300)
+        assert db["rho"] == dt["rho"] and db["step"] == dt["step"] and db["eta"] == dt["eta"]
+    # twice the same bits (the order of the double additions is fixed by the launch configuration)
+    g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_BITS)
+    assert g.diagnostics()["sum_ratio"] == g.diagnostics()["sum_ratio"]
+    # special fields: the vacuum, a signed zero, a planar kink pair
+    dt_np = NP[prec]
+    vac = np.full((N,) * dims, -1.0, dt_np)
+    g.copy_in(vac, np.zeros_like(vac))
+    d = g.diagnostics()
+    assert d["link_count"] == 0 and d["wall_sites"] == 0 and d["gv2"] == 0.0
+    z = np.ones((N,) * dims, dt_np)
+    z[(3,) * dims] = -0.0                                        # -0 is negative (sign bit), also at a group edge below
+    z[(0,) * dims] = -0.5
+    z[(N - 1,) * dims] = -0.25                                   # the periodic neighbour of site 0 in every direction
+    g.copy_in(z, np.ones_like(z))
+    d, do = g.diagnostics(), ref.diagnostics_of(z, np.ones_like(z))
+    assert d["link_count"] == do["link_count"] and d["wall_sites"] == do["wall_sites"]
+    assert abs(d["sum_ratio"] - do["sum_ratio"]) <= 1e-12 * do["sum_ratio"]
+    phi = fg.kink_pair(dims, N, np.pi / 10.0, dtype=dt_np)
+    g.copy_in(phi, np.zeros_like(phi))
+    d = g.diagnostics()
+    assert d["link_count"] == 2 * N ** (dims - 1) and d["wall_sites"] == 4 * N ** (dims - 1)
+    g.close()
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 def test_diagnostics_of_special_fields(prec):
     dt = NP[prec]
     N = 64

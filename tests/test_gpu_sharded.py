@@ -376,3 +376,26 @@ def test_slab_group_over_two_devices():
         same_diag(group.diagnostics(), whole.diagnostics())
     group.close()
     whole.close()
+
+
+@pytest.mark.parametrize("N,world", [(128, 1), (128, 4), (256, 8)])
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+def test_sign_bit_diagnostics_on_slabs(N, world, prec):
+    """The packed-sign-bit diagnostics pass (PRS_KERNEL_BITS) on z slabs: a slab packs the signs of its owned planes and
+    of one halo plane on either side and measures the owned planes; the parts add up to the unsharded lattice's."""
+    from paper_1710_10420_b200 import prs as binding
+
+    whole = prs.Simulation(3, N, prec, seed=6)
+    group = sharded.SlabGroup(N, [0] * world, prec, seed=6)
+    for s in group.slabs:
+        s.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_BITS)
+    whole.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_TILED)
+    whole.init(1.0)
+    group.init(1.0)
+    for k in (0, 4, 3, 120, 1):
+        whole.step(k)
+        group.step(k)
+        same_diag(group.diagnostics(), whole.diagnostics())
+        assert all(s.get_info(4) == prs.KERNEL_BITS for s in group.slabs)
+    group.close()
+    whole.close()

@@ -30,7 +30,7 @@ def test_library_exports_every_declared_symbol():
 def test_workspace_bytes():
     S = 1024 ** 3
     w = prs.prs_workspace_bytes(3, 1024, prs.F32)
-    assert 4 * 4 * S <= w < 4 * 4 * S + (1 << 21)          # phi x2, phidot x2 + small scratch
+    assert 4 * 4 * S + S // 8 <= w < 4 * 4 * S + S // 8 + (1 << 21)      # phi x2, phidot x2, one sign bit per site + small scratch
     assert prs.prs_workspace_bytes(3, 1024, prs.F64) >= 4 * 8 * S
     assert prs.prs_workspace_bytes(2, 16384, prs.F32) >= 4 * 4 * 16384 ** 2
     for bad in [(1, 8, 0), (4, 8, 0), (2, 0, 0), (2, -3, 0), (2, 8, 2), (3, 100000, 0)]:
