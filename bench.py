@@ -50,6 +50,8 @@ CONFIGS = {
     "2d_4096_f32_mat": (2, 4096, 0, 2.0),
     "2d_256_f32_rad": (2, 256, 0, 1.0),        # configs[0]
 }
+# diagnostics cadence BASELINE.json states for the small config ("wall link-count every 10 steps")
+OWN_CADENCE = {"2d_256_f32_rad": 10}
 DEFAULT_CONFIG = "3d_1024_f32_rad"
 BYTES_PER_SITE_UPDATE = {0: 16, 1: 32}        # read phi, phidot; write phidot, phi
 
@@ -346,6 +348,7 @@ def run_gpu(args):
             "scaling": "weak", "vs_baseline": None, "dtype": leg["dtype"], "data": "synthetic",
             "config": leg["config"], "roofline": leg["roofline"], "cpu_baseline": cpu, "e2e": leg["e2e"],
             "gpu_launches": leg["gpu_launches"], "clocks": leg["clocks"], "last_diag": leg["last_diag"], "also": also,
+            "small_lattice": leg["small_lattice"],
         }
         print(json.dumps(line))
     if world > 1:
@@ -470,6 +473,36 @@ def time_leg(args, config, steps, warmup, world, rank, local, barrier, with_e2e,
         except Exception as exc:                                   # e.g. not enough pinned host memory
             e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 2 * fbytes, "d2h_bytes_per_step": 2 * fbytes + 24,
                    "error": str(exc)[:200]}
+    # ---- lattices that fit in L2 are bound by launches and host round trips, not by HBM: report the cycle at the
+    # config's own cadence three ways -- one prs_step + prs_diagnostics call per cycle, prs_run (all cycles queued,
+    # records read back once), and the step kernels alone
+    small = None
+    if 4 * fbytes <= (64 << 20):
+        cad = OWN_CADENCE.get(config, SUBSTEPS)
+        ncyc = max(20, 2000 // cad)
+
+        def timed(fn):
+            fn()
+            barrier()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            barrier()
+            return a.elapsed_time(b) * 1e3 / (ncyc * cad)           # us per PRS step
+
+        def per_call():
+            for _ in range(ncyc):
+                sim.step(cad)
+                sim.diagnostics()
+
+        small = {"cycle": "%d PRS steps + 1 diagnostics pass, %d cycles" % (cad, ncyc),
+                 "us_per_step_one_call_per_cycle": timed(per_call),
+                 "us_per_step_prs_run": timed(lambda: sim.run(ncyc, cad)),
+                 "us_per_step_step_kernels_only": timed(lambda: sim.step(ncyc * cad)),
+                 "steps_per_s_prs_run": None,
+                 "note": "state fits in L2: HBM fractions are meaningless here; the figures are launch- and latency-bound"}
+        small["steps_per_s_prs_run"] = 1e6 / small["us_per_step_prs_run"]
     out = {
         "value": value, "unit": UNIT, "dtype": "f32" if prec == 0 else "f64", "steps": steps, "warmup": warmup,
         "ms_per_step": ms_total / steps, "gpu_launches": launches, "clocks": clocks, "e2e": e2e,
@@ -490,6 +523,7 @@ def time_leg(args, config, steps, warmup, world, rank, local, barrier, with_e2e,
                           "peak_source": peak_src, "algorithmic_bytes_per_launch": algorithmic,
                           "step_kernel_share_of_step": ms_kernels / ms_total}, **own),
         "last_diag": {k: diag[k] for k in ("step", "eta", "link_count", "wall_sites", "rho", "gv2")},
+        "small_lattice": small,
     }
     sim.close()
     del sim

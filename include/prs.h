@@ -74,6 +74,8 @@ enum {
                                 * 2 (step3d_tbr_kernel: half the shared-memory traffic, taller tiles;
                                 * bit-identical) or 0 = auto (default): 2 in FP32 where the bulk loader
                                 * applies (1024^3: 17 % faster), else 1                                */
+    PRS_OPT_DIAG_CHUNK  = 10,  /* tuning: planes (3D) / rows (2D) one CTA of the one-pass diagnostics kernel marches;
+                                * 0 = auto                                                               */
     PRS_OPT_TBS_LOADER  = 9    /* tuning, 3D multi-step kernel: how the shared-memory rings are filled: 0 (default)
                                 * = TMA bulk copies of whole tile rows completing on mbarriers where a lattice
                                 * row holds >= 32 16-byte vectors, else per-thread cp.async; 1 = always cp.async;
@@ -141,6 +143,15 @@ int prs_step(prs_handle h, int64_t nsteps);
 
 /* Measures Eqs. 7-8 on the current state; synchronises the stream; fills *out (HOST pointer). */
 int prs_diagnostics(prs_handle h, prs_diag* out);
+
+/* ncycles times: steps_per_cycle steps of Eqs. 3-6, then Eqs. 7-8 on the state reached -- the loop every config of
+ * BASELINE.json runs ("diagnostics every 10 / 50 / 100 steps"), as ONE call: all launches are queued back to back, every
+ * cycle's reduced record stays on the device (a ring of 4096 records in the workspace) and the records cross to the host
+ * once per 4096 cycles, so a cycle costs its kernels and nothing else (the per-step transfer of the
+ * partial sums is what hurts small boxes).  out: HOST array of ncycles records, out[i] = what prs_diagnostics would
+ * have returned after (i + 1) * steps_per_cycle further steps -- identical bits: the same kernels in the same launch
+ * configuration.  Synchronises the stream before it returns.  Not on a slab (PRS_ERR_UNSUPPORTED). */
+int prs_run(prs_handle h, int64_t ncycles, int64_t steps_per_cycle, prs_diag* out);
 
 /* Orientation-weighted wall area of the current phi^n: PAPER.md Eq. 7 as printed (:59-62), the sum over
  * crossing forward links of |grad phi| / (|phi,x| + |phi,y| + |phi,z|) with the gradient on a link taken as

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "prs_kernels_generic.cuh"
 #include "prs_kernels_tiled.cuh"
@@ -21,6 +22,7 @@ namespace {
 
 constexpr size_t ALIGN = 256;
 constexpr int MAX_PARTIALS = 1 << 16;        // upper bound on diagnostics blocks (1.5 MiB of scratch)
+constexpr int RESULTS_CAP = 4096;            // diagnostics records prs_run keeps on the device between readbacks (96 KiB)
 
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
@@ -35,7 +37,7 @@ inline bool args_ok(int dims, int64_t N, int precision) {
 inline size_t sites_of(int dims, int64_t N) { return dims == 3 ? (size_t)N * N * N : (size_t)N * N; }
 
 struct Layout {
-    size_t field_bytes, off_phi[2], off_pd[2], off_partials, off_result, off_bits, total;
+    size_t field_bytes, off_phi[2], off_pd[2], off_partials, off_result, off_results, off_bits, total;
 };
 
 constexpr int SLAB_HALO = 4;                 // halo planes per side = the most steps one 3D launch takes
@@ -50,6 +52,7 @@ Layout layout_of_sites(size_t sites, int precision) {
     L.off_pd[1] = o; o += L.field_bytes;
     L.off_partials = o; o += align_up(sizeof(DiagPartial) * MAX_PARTIALS);
     L.off_result = o; o += align_up(sizeof(DiagPartial));
+    L.off_results = o; o += align_up(sizeof(DiagPartial) * RESULTS_CAP);
     L.off_bits = o; o += align_up((sites + 7) / 8);             // one sign bit per site (prs_kernels_bits.cuh)
     L.total = o;
     return L;
@@ -318,25 +321,32 @@ int resolve_diag_kernel(const prs_ctx* h) {
     return want;
 }
 
-// Chunk length of the diagnostics march: as short as the partials scratch allows, but no shorter
-// than 16 (the first plane / row of a chunk costs three loads instead of one).
-int diag_chunk(const prs_ctx* h, long long tiles_per_slab) {
+// Chunk length of the diagnostics march (planes in 3D, rows in 2D; PRS_OPT_DIAG_CHUNK overrides).  Large lattices: as
+// short as the partials scratch allows but no shorter than 16 (the first plane / row of a chunk costs three loads
+// instead of one).  Small lattices are bound by the latency of the march, not by its loads: there the chunks are cut
+// down (to no less than 2) until the grid holds about four CTAs per SM.
+int diag_chunk(const prs_ctx* h, long long tiles_per_slab, int span) {
+    if (h->opt_diag_chunk > 0) return std::max(1, std::min(h->opt_diag_chunk, span));
     long long max_chunks = MAX_PARTIALS / tiles_per_slab;
     if (max_chunks < 1) max_chunks = 1;
-    long long len = (h->N + max_chunks - 1) / max_chunks;
+    long long len = (span + max_chunks - 1) / max_chunks;
     if (len < 16) len = 16;
-    if (len > h->N) len = h->N;
+    const long long want = 4LL * std::max(1, h->sm_count);
+    while (len > 2 && tiles_per_slab * ((span + len - 1) / len) < want) len /= 2;
+    if (len > span) len = span;
     return (int)len;
 }
 
+// Launches the diagnostics pass on the current state; the reduced record goes to `dst` (device).
 template <typename T>
-int diag_launch(prs_ctx* h) {
+int diag_launch(prs_ctx* h, DiagPartial* dst) {
     const double pi = 3.14159265358979323846;
     const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0);
     const double I = 1.0 / (h->phi0 * h->phi0);
     const T* p = (const T*)h->phi[h->cur];
     const T* v = (const T*)h->pd[h->cur];
     const int kernel = resolve_diag_kernel(h);
+    const DiagFinish fin = {h->partials, dst, h->d_ticket};   // the last block to finish reduces the partials into dst
     long long blocks;
     if (kernel == PRS_KERNEL_BITS) {
         constexpr int W = VecOps<T>::W;
@@ -355,9 +365,9 @@ int diag_launch(prs_ctx* h) {
         const long long lgroups = (p1 - p0) * rows_per_plane * NG;       // one thread each
         blocks = std::min<long long>((lgroups + BITS_THREADS - 1) / BITS_THREADS, std::min<long long>(MAX_PARTIALS, cap));
         if (h->dims == 3)
-            bit_links_kernel<T, 3><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, (int)h->NZ, p0 * rows_per_plane, p1 * rows_per_plane, V0, I, h->partials);
+            bit_links_kernel<T, 3><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, (int)h->NZ, p0 * rows_per_plane, p1 * rows_per_plane, V0, I, fin);
         else
-            bit_links_kernel<T, 2><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, 1, p0, p1, V0, I, h->partials);
+            bit_links_kernel<T, 2><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, 1, p0, p1, V0, I, fin);
         h->launches += 1;
     } else if (kernel == PRS_KERNEL_TILED) {
         constexpr int W = VecOps<T>::W;
@@ -367,16 +377,16 @@ int diag_launch(prs_ctx* h) {
             const unsigned gx = (unsigned)((N + 32 * W - 1) / (32 * W)), gy = (unsigned)((N + TY - 1) / TY);
             // a z slab measures its owned planes only (their z neighbours are halo planes, never the wrap)
             const int NZ = (int)h->NZ, zlo = h->slab ? (int)h->halo : 0, zhi = h->slab ? (int)(h->halo + h->nz_own) : N;
-            const int ZC = std::min(diag_chunk(h, (long long)gx * gy), zhi - zlo);
+            const int ZC = diag_chunk(h, (long long)gx * gy, zhi - zlo);
             const dim3 grid(gx, gy, (unsigned)((zhi - zlo + ZC - 1) / ZC));
             blocks = (long long)grid.x * grid.y * grid.z;
-            diag3d_tiled_kernel<T, TY><<<grid, dim3(32, TY, 1), 0, h->stream>>>(p, v, N, NZ, zlo, zhi, ZC, V0, I, h->partials);
+            diag3d_tiled_kernel<T, TY><<<grid, dim3(32, TY, 1), 0, h->stream>>>(p, v, N, NZ, zlo, zhi, ZC, V0, I, fin);
         } else {
             const unsigned gx = (unsigned)((N + 128 * W - 1) / (128 * W));
-            const int YC = diag_chunk(h, gx);
+            const int YC = diag_chunk(h, gx, N);
             const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
             blocks = (long long)grid.x * grid.y;
-            diag2d_tiled_kernel<T><<<grid, 128, 0, h->stream>>>(p, v, N, YC, V0, I, h->partials);
+            diag2d_tiled_kernel<T><<<grid, 128, 0, h->stream>>>(p, v, N, YC, V0, I, fin);
         }
     } else {
         // a z slab measures its owned planes only (their z neighbours are halo planes, never the wrap)
@@ -386,16 +396,14 @@ int diag_launch(prs_ctx* h) {
         const long long cap = std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 8);
         if (blocks > cap) blocks = cap;
         if (h->dims == 3)
-            diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->NZ, s0, s1, V0, I, h->partials);
+            diag_generic_kernel<T, 3><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->NZ, s0, s1, V0, I, fin);
         else
-            diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->NZ, s0, s1, V0, I, h->partials);
+            diag_generic_kernel<T, 2><<<(unsigned)blocks, 256, 0, h->stream>>>(p, v, (long long)h->N, (long long)h->NZ, s0, s1, V0, I, fin);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics kernel launch");
-    diag_finalize_kernel<<<1, 1024, 0, h->stream>>>(h->partials, (int)blocks, h->d_result);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(h, e, "diagnostics finalize launch");
-    h->launches += 2;
+    (void)blocks;
+    h->launches += 1;
     h->last_diag_kernel = kernel;
     return PRS_OK;
 }
@@ -437,7 +445,9 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->pd[0] = h->ws + L.off_pd[0]; h->pd[1] = h->ws + L.off_pd[1];
     h->partials = (DiagPartial*)(h->ws + L.off_partials);
     h->d_result = (DiagPartial*)(h->ws + L.off_result);
+    h->d_ticket = (unsigned*)(h->ws + L.off_result + 64);         // in the record's 256-byte slot
     h->bits = (unsigned*)(h->ws + L.off_bits);
+    h->d_results = (DiagPartial*)(h->ws + L.off_results);
     h->cur = 0; h->eta0 = 1.0; h->step = 0; h->inited = false;
     h->opt_step_kernel = PRS_KERNEL_AUTO; h->opt_arith = PRS_ARITH_FMA; h->opt_diag_kernel = PRS_KERNEL_AUTO;
     h->opt_chunk = 0; h->opt_tile_y = 4; h->opt_tb2_tile_y = 12;
@@ -445,6 +455,7 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->opt_tbs_steps = (dims == 3) ? 4 : (precision == PRS_F32 ? 8 : 6);
     h->opt_tbs_rows = 0;                          // auto (prs_launch_tbs.cuh)
     h->opt_tbs_loader = 0;
+    h->opt_diag_chunk = 0;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     memset(&h->main_launch, 0, sizeof(h->main_launch));
     h->h_result = nullptr;
@@ -456,6 +467,11 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
         return PRS_ERR_CUDA;
     }
     if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) h->sm_count = 148;
+    if (cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned), h->stream) != cudaSuccess) {     // the caller's workspace is uninitialised
+        cudaGetLastError();
+        delete h;
+        return PRS_ERR_CUDA;
+    }
     if (cudaHostAlloc((void**)&h->h_result, sizeof(DiagPartial), cudaHostAllocDefault) != cudaSuccess) {
         cudaGetLastError();
         delete h;
@@ -527,9 +543,16 @@ int prs_init(prs_handle h, double eta0) {
     return PRS_OK;
 }
 
+static int step_impl(prs_handle h, int64_t nsteps);
+
 int prs_step(prs_handle h, int64_t nsteps) {
     if (!h) return PRS_ERR_INVALID_ARG;
     PRS_ON_DEVICE(h);
+    return step_impl(h, nsteps);
+}
+
+// the launches of prs_step; the handle's device is current
+static int step_impl(prs_handle h, int64_t nsteps) {
     if (nsteps < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_step: nsteps must be >= 0");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_step: call prs_init or prs_copy_in first");
     if (nsteps > 0) h->main_launch.open = true;
@@ -609,7 +632,7 @@ int prs_diagnostics(prs_handle h, prs_diag* out) {
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_diagnostics: call prs_init or prs_copy_in first");
     if (h->slab && h->halo_valid < 1)
         return fail(h, PRS_ERR_STATE, "prs_diagnostics: the slab's halo planes are stale; exchange them first");
-    const int rc = (h->precision == PRS_F32) ? diag_launch<float>(h) : diag_launch<double>(h);
+    const int rc = (h->precision == PRS_F32) ? diag_launch<float>(h, h->d_result) : diag_launch<double>(h, h->d_result);
     if (rc != PRS_OK) return rc;
     PRS_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -623,6 +646,44 @@ int prs_diagnostics(prs_handle h, prs_diag* out) {
     d.rho = (double)d.link_count / (h->slab ? (double)h->N * (double)h->N * (double)h->N : (double)h->S);
     d.gv2 = d.wall_sites ? d.sum_ratio / (2.0 * (double)d.wall_sites) : 0.0;
     *out = d;
+    return PRS_OK;
+}
+
+static void fill_diag(const prs_ctx* h, const DiagPartial& r, int64_t step, prs_diag* d) {
+    d->step = step;
+    d->eta = h->eta0 + (double)step * h->deta;
+    d->link_count = r.links;
+    d->wall_sites = r.walls;
+    d->sum_ratio = r.sum;
+    d->rho = (double)r.links / (h->slab ? (double)h->N * (double)h->N * (double)h->N : (double)h->S);
+    d->gv2 = r.walls ? r.sum / (2.0 * (double)r.walls) : 0.0;
+}
+
+int prs_run(prs_handle h, int64_t ncycles, int64_t steps_per_cycle, prs_diag* out) {
+    if (!h) return PRS_ERR_INVALID_ARG;
+    PRS_ON_DEVICE(h);
+    if (ncycles < 0 || steps_per_cycle < 0) return fail(h, PRS_ERR_INVALID_ARG, "prs_run: ncycles and steps_per_cycle must be >= 0");
+    if (ncycles > 0 && !out) return fail(h, PRS_ERR_INVALID_ARG, "prs_run: out is NULL");
+    if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_run: call prs_init or prs_copy_in first");
+    if (h->slab) return fail(h, PRS_ERR_UNSUPPORTED, "prs_run: a slab needs its halo planes exchanged between passes; use prs_step / prs_diagnostics");
+    std::vector<DiagPartial> host;
+    std::vector<int64_t> steps;
+    for (int64_t done = 0; done < ncycles;) {
+        const int64_t batch = std::min<int64_t>(ncycles - done, RESULTS_CAP);
+        host.resize((size_t)batch);
+        steps.resize((size_t)batch);
+        for (int64_t i = 0; i < batch; ++i) {                         // queued back to back: no sync, no transfer
+            int rc = step_impl(h, steps_per_cycle);
+            if (rc != PRS_OK) return rc;
+            rc = (h->precision == PRS_F32) ? diag_launch<float>(h, h->d_results + i) : diag_launch<double>(h, h->d_results + i);
+            if (rc != PRS_OK) return rc;
+            steps[(size_t)i] = h->step;
+        }
+        PRS_CUDA(h, cudaMemcpyAsync(host.data(), h->d_results, sizeof(DiagPartial) * (size_t)batch, cudaMemcpyDeviceToHost, h->stream));
+        PRS_CUDA(h, cudaStreamSynchronize(h->stream));
+        for (int64_t i = 0; i < batch; ++i) fill_diag(h, host[(size_t)i], steps[(size_t)i], out + done + i);
+        done += batch;
+    }
     return PRS_OK;
 }
 
@@ -650,17 +711,16 @@ int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
     const long long blocks = (long long)grid.x * grid.y * grid.z;
     if (blocks > MAX_PARTIALS) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: lattice too large for the reduction scratch");
     const void* p = h->phi[h->cur];
+    const DiagFinish fin = {h->partials, h->d_result, h->d_ticket};
     if (h->precision == PRS_F32) {
-        if (h->dims == 3) weighted_area_kernel<float, 3><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, h->partials);
-        else weighted_area_kernel<float, 2><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, h->partials);
+        if (h->dims == 3) weighted_area_kernel<float, 3><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, fin);
+        else weighted_area_kernel<float, 2><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, fin);
     } else {
-        if (h->dims == 3) weighted_area_kernel<double, 3><<<grid, 256, 0, h->stream>>>((const double*)p, N, NM, mlo, mhi, L, h->partials);
-        else weighted_area_kernel<double, 2><<<grid, 256, 0, h->stream>>>((const double*)p, N, NM, mlo, mhi, L, h->partials);
+        if (h->dims == 3) weighted_area_kernel<double, 3><<<grid, 256, 0, h->stream>>>((const double*)p, N, NM, mlo, mhi, L, fin);
+        else weighted_area_kernel<double, 2><<<grid, 256, 0, h->stream>>>((const double*)p, N, NM, mlo, mhi, L, fin);
     }
     PRS_CUDA(h, cudaGetLastError());
-    diag_finalize_kernel<<<1, 1024, 0, h->stream>>>(h->partials, (int)blocks, h->d_result);
-    PRS_CUDA(h, cudaGetLastError());
-    h->launches += 2;
+    h->launches += 1;
     PRS_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     if (area) *area = h->h_result->sum;
@@ -796,6 +856,10 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             if (value != 0 && value != 1 && !(value == 2 && h->dims == 3))
                 return fail(h, PRS_ERR_INVALID_ARG, "tbs_rows must be 0 (auto), 1 or, in 3D, 2");
             h->opt_tbs_rows = (int)value;
+            return PRS_OK;
+        case PRS_OPT_DIAG_CHUNK:
+            if (value < 0 || value > (1 << 20)) return fail(h, PRS_ERR_INVALID_ARG, "diag_chunk must be >= 0");
+            h->opt_diag_chunk = (int)value;
             return PRS_OK;
         case PRS_OPT_TBS_LOADER:
             if (value != 0 && value != 1 && value != 2) return fail(h, PRS_ERR_INVALID_ARG, "tbs_loader must be 0 (auto), 1 (cp.async) or 2 (bulk)");

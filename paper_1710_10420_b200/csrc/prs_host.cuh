@@ -30,12 +30,14 @@ struct prs_ctx {
     int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
     prs::DiagPartial* partials;
     prs::DiagPartial* d_result;
+    unsigned* d_ticket;                       // ticket counter of the diagnostics kernels' last-block reduction
+    prs::DiagPartial* d_results;              // ring of reduced records for prs_run (RESULTS_CAP entries)
     unsigned* bits;                           // one sign bit per site: scratch of the sign-bit diagnostics pass
     prs::DiagPartial* h_result;               // pinned host, 24 bytes
     double eta0;
     int64_t step;
     bool inited;
-    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps, opt_tbs_rows, opt_tbs_loader;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps, opt_tbs_rows, opt_tbs_loader, opt_diag_chunk;
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;

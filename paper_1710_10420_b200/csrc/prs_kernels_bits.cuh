@@ -83,7 +83,7 @@ constexpr int BITS_STACK = 64;                   // entries per warp: < 32 left 
 template <typename T, int DIMS>
 __global__ void __launch_bounds__(BITS_THREADS)
 bit_links_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, const unsigned* __restrict__ bits, int N, int NZ,
-                 long long R0, long long R1, double V0, double I, DiagPartial* __restrict__ partials) {
+                 long long R0, long long R1, double V0, double I, DiagFinish fin) {
     constexpr int W = VecOps<T>::W;
     __shared__ unsigned short stack_all[BITS_THREADS / 32][BITS_STACK];
     unsigned short* const stack = stack_all[threadIdx.x >> 5];
@@ -173,7 +173,7 @@ bit_links_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, const 
         if (held) work_off(held);                                    // the bases belong to this batch of groups
     }
     acc = block_reduce(acc);
-    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+    finish_partials(fin, acc);
 }
 
 }  // namespace prs

@@ -160,12 +160,52 @@ __device__ __forceinline__ DiagPartial block_reduce(DiagPartial p) {
     return p;
 }
 
+// Final reduction without a second launch.  Every block stores its partial and draws a ticket; the block that draws
+// the last one adds all partials in index order -- thread-strided, then the block reduction: an order fixed by the
+// launch configuration alone, whichever block happens to be last, so the double sum is reproducible -- writes the record
+// and puts the ticket counter back to zero for the next pass.  (A launch costs 4-5 us of host time on this box: on a
+// 256^2 lattice the separate one-block reduction kernel was a fifth of a 10-step cycle.)
+struct DiagFinish {
+    DiagPartial* partials;      // one per block
+    DiagPartial* out;           // the reduced record
+    unsigned* ticket;           // zero between passes
+};
+
+// All threads of the block must call; acc is the block's partial, valid in thread 0 (what block_reduce returns).
+__device__ __forceinline__ void finish_partials(const DiagFinish& f, DiagPartial acc) {
+    __shared__ bool is_last;
+    const unsigned tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const unsigned nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const unsigned nblocks = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned block = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    if (tid == 0) {
+        f.partials[block] = acc;
+        __threadfence();                                   // the partial is visible before the ticket is drawn
+        is_last = (atomicAdd(f.ticket, 1u) == nblocks - 1u);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    DiagPartial sum = {0ull, 0ull, 0.0};
+    for (unsigned i = tid; i < nblocks; i += nthreads) {
+        const DiagPartial* q = f.partials + i;             // written by other SMs: read past L1
+        sum.links += __ldcg(&q->links);
+        sum.walls += __ldcg(&q->walls);
+        sum.sum = __dadd_rn(sum.sum, __ldcg(&q->sum));
+    }
+    sum = block_reduce(sum);
+    if (tid == 0) {
+        *f.out = sum;
+        *f.ticket = 0u;
+    }
+}
+
 // Generic diagnostics: grid-stride over sites; each site owns its d forward links (Eq. 7) and tests
 // all 2d links for the wall-site predicate (Eq. 8's N).
 template <typename T, int DIMS>
 __global__ void __launch_bounds__(256)
 diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, long long N, long long NZ,
-                    long long s0, long long S, double V0, double I, DiagPartial* __restrict__ partials) {
+                    long long s0, long long S, double V0, double I, DiagFinish fin) {
     using A = Ar<T>;
     DiagPartial acc = {0ull, 0ull, 0.0};
     // sites s0 <= s < S of an N x N x NZ lattice (cubic: NZ = N, s0 = 0; z slab: the owned planes)
@@ -195,7 +235,7 @@ diag_generic_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, lon
         }
     }
     acc = block_reduce(acc);
-    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+    finish_partials(fin, acc);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -260,7 +300,7 @@ __device__ __forceinline__ double link_weight(const T* __restrict__ phi, int N, 
 
 template <typename T, int DIMS>
 __global__ void __launch_bounds__(WAREA_THREADS)
-weighted_area_kernel(const T* __restrict__ phi, int N, int NM, int mlo, int mhi, int L, DiagPartial* __restrict__ partials) {
+weighted_area_kernel(const T* __restrict__ phi, int N, int NM, int mlo, int mhi, int L, DiagFinish fin) {
     // the slowest (march) axis holds NM sites, of which mlo <= m < mhi are measured: N, 0, N on a whole lattice; on a
     // z slab (prs_create_slab) its NZ planes and the owned range, whose z neighbours are halo planes (never the wrap)
     using A = Ar<T>;
@@ -327,22 +367,7 @@ weighted_area_kernel(const T* __restrict__ phi, int N, int NM, int mlo, int mhi,
     }
     work_off(held);
     acc = block_reduce(acc);
-    if (threadIdx.x == 0)
-        partials[blockIdx.x + gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z)] = acc;
-}
-
-// Final reduction of the per-block partials by one block, in a fixed order.
-__global__ void __launch_bounds__(1024)
-diag_finalize_kernel(const DiagPartial* __restrict__ partials, int npartials, DiagPartial* __restrict__ out) {
-    DiagPartial acc = {0ull, 0ull, 0.0};
-    for (int i = threadIdx.x; i < npartials; i += blockDim.x) {
-        const DiagPartial p = partials[i];
-        acc.links += p.links;
-        acc.walls += p.walls;
-        acc.sum = __dadd_rn(acc.sum, p.sum);
-    }
-    acc = block_reduce(acc);
-    if (threadIdx.x == 0) *out = acc;
+    finish_partials(fin, acc);
 }
 
 }  // namespace prs

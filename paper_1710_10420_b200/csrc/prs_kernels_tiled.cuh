@@ -290,7 +290,7 @@ struct WallQueue {
 template <typename T, int TYB>
 __global__ void __launch_bounds__(32 * TYB)
 diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int N, int NZ, int zlo, int zhi, int ZC, double V0, double I,
-                    DiagPartial* __restrict__ partials) {
+                    DiagFinish fin) {
     using O = VecOps<T>;
     using V = typename O::V;
     constexpr int W = O::W;
@@ -360,14 +360,13 @@ diag3d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
         wq.drain(V0, I, acc);
     }
     acc = block_reduce(acc);
-    if (threadIdx.x == 0 && threadIdx.y == 0)
-        partials[blockIdx.x + gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z)] = acc;
+    finish_partials(fin, acc);
 }
 
 template <typename T>
 __global__ void __launch_bounds__(128)
 diag2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int N, int YC, double V0, double I,
-                    DiagPartial* __restrict__ partials) {
+                    DiagFinish fin) {
     using O = VecOps<T>;
     using V = typename O::V;
     constexpr int W = O::W;
@@ -427,7 +426,7 @@ diag2d_tiled_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, int
         wq.drain(V0, I, acc);
     }
     acc = block_reduce(acc);
-    if (threadIdx.x == 0) partials[blockIdx.x + (size_t)gridDim.x * blockIdx.y] = acc;
+    finish_partials(fin, acc);
 }
 
 }  // namespace prs

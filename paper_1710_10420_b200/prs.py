@@ -15,7 +15,7 @@ from . import build as _build
 F32, F64 = 0, 1
 ARITH_LITERAL, ARITH_COEF, ARITH_FMA = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_TB2, KERNEL_TBS, KERNEL_CLUSTER, KERNEL_BITS = 0, 1, 2, 3, 4, 5, 6
-OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS, OPT_TBS_LOADER = 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS, OPT_TBS_LOADER, OPT_DIAG_CHUNK = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 INFO_KERNEL_LAUNCHES, INFO_STEP_KERNEL, INFO_STEP, INFO_DIAG_KERNEL = 1, 2, 3, 4
 INFO_HALO_VALID, INFO_HALO_PLANES, INFO_DEVICE = 5, 6, 7
 ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WORKSPACE",
@@ -23,7 +23,7 @@ ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WOR
 
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
            "prs_weighted_area", "prs_set_beta", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
-           "prs_device_pointers", "prs_last_error", "prs_step_launch_info",
+           "prs_device_pointers", "prs_last_error", "prs_step_launch_info", "prs_run",
            "prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled", "prs_diag_combine"]
 
 
@@ -62,6 +62,7 @@ def lib():
         L.prs_init.argtypes = [vp, dbl]
         L.prs_step.argtypes = [vp, i64]
         L.prs_diagnostics.argtypes = [vp, C.POINTER(Diag)]
+        L.prs_run.argtypes = [vp, i64, i64, C.POINTER(Diag)]
         L.prs_weighted_area.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
         L.prs_set_beta.argtypes = [vp, dbl]
         L.prs_copy_out.argtypes = [vp, vp, vp]
@@ -165,6 +166,12 @@ class Simulation:
         d = Diag()
         self._chk(lib().prs_diagnostics(self._h, C.byref(d)), "prs_diagnostics")
         return d.as_dict()
+
+    def run(self, ncycles, steps_per_cycle):
+        """prs_run: ncycles x (steps_per_cycle steps + diagnostics) in one call; a list of ncycles dicts."""
+        arr = (Diag * max(1, ncycles))()
+        self._chk(lib().prs_run(self._h, ncycles, steps_per_cycle, arr), "prs_run")
+        return [arr[i].as_dict() for i in range(ncycles)]
 
     def set_beta(self, beta):
         self._chk(lib().prs_set_beta(self._h, beta), "prs_set_beta")

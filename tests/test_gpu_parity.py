@@ -863,3 +863,48 @@ def test_race_hunting_build_gives_the_same_bits():
     assert out.returncode == 0, out.stdout[-3000:]
     assert "results identical to the generic kernel" in out.stdout
     assert "libprs_jitter.so" in out.stdout
+
+
+@pytest.mark.parametrize("dims,N,prec,every,ncyc", [(2, 256, prs.F32, 10, 127), (2, 64, prs.F64, 1, 4100), (3, 64, prs.F32, 7, 9),
+                                                   (3, 128, prs.F64, 50, 3), (2, 1000, prs.F32, 3, 5)])
+def test_batched_cycles_equal_the_step_and_diagnostics_loop(dims, N, prec, every, ncyc):
+    """prs_run(ncycles, steps_per_cycle) = the loop every BASELINE.json config runs, queued without a host round trip
+    per cycle: every record must equal what prs_step + prs_diagnostics return, bit for bit (same kernels, same launch
+    configuration), across the 4096-record ring on the device as well; the state afterwards is the same."""
+    a = prs.Simulation(dims, N, prec, seed=3)
+    b = prs.Simulation(dims, N, prec, seed=3)
+    a.init(1.0)
+    b.init(1.0)
+    got = a.run(ncyc, every)
+    assert len(got) == ncyc
+    for i in range(ncyc):
+        b.step(every)
+        want = b.diagnostics()
+        if i < 40 or i % 97 == 0 or i >= ncyc - 5:
+            assert got[i] == want, i
+    assert got[-1]["step"] == ncyc * every and a.get_info(binding.INFO_STEP) == ncyc * every
+    pa, pb = a.copy_out(), b.copy_out()
+    assert pa[0].tobytes() == pb[0].tobytes() and pa[1].tobytes() == pb[1].tobytes()
+    assert a.run(0, 5) == [] and a.get_info(binding.INFO_STEP) == ncyc * every
+    zero = a.run(2, 0)                                          # no steps: the same state measured twice
+    assert zero[0] == zero[1] and zero[0]["step"] == ncyc * every
+    a.close()
+    b.close()
+
+
+def test_batched_cycles_error_paths():
+    from paper_1710_10420_b200 import sharded
+
+    g = prs.Simulation(2, 64, prs.F32)
+    with pytest.raises(prs.PrsError) as e:
+        g.run(1, 1)                                             # no state yet
+    assert e.value.code == 4
+    g.init(1.0)
+    with pytest.raises(prs.PrsError) as e:
+        g.run(-1, 1)
+    assert e.value.code == 1
+    s = sharded.SlabSimulation(64, 0, 16, prs.F32)
+    s.init(1.0)
+    with pytest.raises(prs.PrsError) as e:
+        s.run(1, 4)                                             # a slab's halo must be exchanged between passes
+    assert e.value.code == 2
