@@ -337,6 +337,36 @@ int diag_chunk(const prs_ctx* h, long long tiles_per_slab, int span) {
     return (int)len;
 }
 
+// The rows the sign-bit passes measure [m0, m1) and the rows whose signs they need [b0, b1) (a slab: its owned planes,
+// and one halo plane on either side), in units of lattice rows (row = y + N z; 2D: y).
+struct BitRows { long long m0, m1, b0, b1; };
+BitRows bit_rows(const prs_ctx* h) {
+    const long long rows_per_plane = (h->dims == 3) ? h->N : 1;
+    const long long nplanes = (h->dims == 3) ? h->NZ : h->N;     // 2D: a "plane" is a row
+    const long long p0 = h->slab ? h->halo : 0, p1 = h->slab ? h->halo + h->nz_own : nplanes;
+    const long long b0 = h->slab ? p0 - 1 : 0, b1 = h->slab ? p1 + 1 : nplanes;
+    return {p0 * rows_per_plane, p1 * rows_per_plane, b0 * rows_per_plane, b1 * rows_per_plane};
+}
+
+// Packs the sign bits of the current phi unless the bit array already holds them (prs_weighted_area right after
+// prs_diagnostics: the state has not moved).  The tag is the step counter, the ping-pong index and a generation number
+// that prs_init, prs_copy_in and prs_slab_halo_filled advance.
+template <typename T>
+int ensure_bits(prs_ctx* h) {
+    if (h->bits_valid && h->bits_step == h->step && h->bits_cur == h->cur && h->bits_gen == h->state_gen) return PRS_OK;
+    constexpr int W = VecOps<T>::W;
+    const int N = (int)h->N, NG = N / (32 * W);
+    const BitRows br = bit_rows(h);
+    const long long sgroups = (br.b1 - br.b0) * NG;                  // one warp each
+    const long long sblocks = std::min<long long>((sgroups + 7) / 8, (long long)h->sm_count * 16);
+    sign_bits_kernel<T><<<(unsigned)sblocks, 256, 0, h->stream>>>((const T*)h->phi[h->cur], h->bits, N, br.b0, br.b1);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(h, e, "sign-bit kernel launch");
+    h->launches += 1;
+    h->bits_valid = true; h->bits_step = h->step; h->bits_cur = h->cur; h->bits_gen = h->state_gen;
+    return PRS_OK;
+}
+
 // Launches the diagnostics pass on the current state; the reduced record goes to `dst` (device).
 template <typename T>
 int diag_launch(prs_ctx* h, DiagPartial* dst) {
@@ -351,24 +381,15 @@ int diag_launch(prs_ctx* h, DiagPartial* dst) {
     if (kernel == PRS_KERNEL_BITS) {
         constexpr int W = VecOps<T>::W;
         const int N = (int)h->N, NG = N / (32 * W);
-        const long long rows_per_plane = (h->dims == 3) ? N : 1;
-        const long long nplanes = (h->dims == 3) ? h->NZ : N;            // 2D: a "plane" is a row
-        // rows to measure, and the rows whose signs they need (a slab: one halo plane on either side)
-        const long long p0 = h->slab ? h->halo : 0, p1 = h->slab ? h->halo + h->nz_own : nplanes;
-        const long long b0 = h->slab ? p0 - 1 : 0, b1 = h->slab ? p1 + 1 : nplanes;
-        const long long cap = (long long)h->sm_count * 16;
-        const long long sgroups = (b1 - b0) * rows_per_plane * NG;       // one warp each
-        const long long sblocks = std::min<long long>((sgroups + 7) / 8, cap);
-        sign_bits_kernel<T><<<(unsigned)sblocks, 256, 0, h->stream>>>(p, h->bits, N, b0 * rows_per_plane, b1 * rows_per_plane);
-        cudaError_t e0 = cudaGetLastError();
-        if (e0 != cudaSuccess) return cuda_fail(h, e0, "sign-bit kernel launch");
-        const long long lgroups = (p1 - p0) * rows_per_plane * NG;       // one thread each
-        blocks = std::min<long long>((lgroups + BITS_THREADS - 1) / BITS_THREADS, std::min<long long>(MAX_PARTIALS, cap));
+        const int rc = ensure_bits<T>(h);
+        if (rc != PRS_OK) return rc;
+        const BitRows br = bit_rows(h);
+        const long long lgroups = (br.m1 - br.m0) * NG;                  // one thread each
+        blocks = std::min<long long>((lgroups + BITS_THREADS - 1) / BITS_THREADS, std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 16));
         if (h->dims == 3)
-            bit_links_kernel<T, 3><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, (int)h->NZ, p0 * rows_per_plane, p1 * rows_per_plane, V0, I, fin);
+            bit_links_kernel<T, 3><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, (int)h->NZ, br.m0, br.m1, V0, I, fin);
         else
-            bit_links_kernel<T, 2><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, 1, p0, p1, V0, I, fin);
-        h->launches += 1;
+            bit_links_kernel<T, 2><<<(unsigned)blocks, BITS_THREADS, 0, h->stream>>>(p, v, h->bits, N, 1, br.m0, br.m1, V0, I, fin);
     } else if (kernel == PRS_KERNEL_TILED) {
         constexpr int W = VecOps<T>::W;
         const int N = (int)h->N;
@@ -456,6 +477,7 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->opt_tbs_rows = 0;                          // auto (prs_launch_tbs.cuh)
     h->opt_tbs_loader = 0;
     h->opt_diag_chunk = 0;
+    h->bits_valid = false; h->bits_step = 0; h->bits_cur = 0; h->bits_gen = 0; h->state_gen = 0;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
     memset(&h->main_launch, 0, sizeof(h->main_launch));
     h->h_result = nullptr;
@@ -540,6 +562,7 @@ int prs_init(prs_handle h, double eta0) {
     PRS_CUDA(h, cudaGetLastError());
     h->launches += 1;
     h->eta0 = eta0; h->step = 0; h->inited = true;
+    h->state_gen += 1;
     return PRS_OK;
 }
 
@@ -709,10 +732,29 @@ int prs_weighted_area(prs_handle h, double* area, double* rho_weighted) {
     const unsigned nch = (unsigned)((span + L - 1) / L);
     const dim3 grid = (h->dims == 3) ? dim3(gx, (unsigned)N, nch) : dim3(gx, nch, 1);
     const long long blocks = (long long)grid.x * grid.y * grid.z;
-    if (blocks > MAX_PARTIALS) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: lattice too large for the reduction scratch");
+    const bool on_bits = diag_bits_supported(h) && h->S >= ((size_t)1 << 22) && h->opt_diag_kernel != PRS_KERNEL_TILED &&
+                         h->opt_diag_kernel != PRS_KERNEL_GENERIC;
+    if (!on_bits && blocks > MAX_PARTIALS) return fail(h, PRS_ERR_UNSUPPORTED, "prs_weighted_area: lattice too large for the reduction scratch");
     const void* p = h->phi[h->cur];
     const DiagFinish fin = {h->partials, h->d_result, h->d_ticket};
-    if (h->precision == PRS_F32) {
+    // from 2^22 sites up on lattices of whole 32-vector groups: on the packed sign bits (prs_kernels_bits.cuh), which
+    // the preceding prs_diagnostics may have left behind
+    if (on_bits) {
+        const int rc = (h->precision == PRS_F32) ? ensure_bits<float>(h) : ensure_bits<double>(h);
+        if (rc != PRS_OK) return rc;
+        const int NG = N / (32 * vec_width(h->precision));
+        const BitRows br = bit_rows(h);
+        const long long lgroups = (br.m1 - br.m0) * NG;
+        const unsigned bl = (unsigned)std::min<long long>((lgroups + BITS_THREADS - 1) / BITS_THREADS, std::min<long long>(MAX_PARTIALS, (long long)h->sm_count * 16));
+        const int NZ = (int)h->NZ;
+        if (h->precision == PRS_F32) {
+            if (h->dims == 3) bit_area_kernel<float, 3><<<bl, BITS_THREADS, 0, h->stream>>>((const float*)p, h->bits, N, NZ, br.m0, br.m1, fin);
+            else bit_area_kernel<float, 2><<<bl, BITS_THREADS, 0, h->stream>>>((const float*)p, h->bits, N, 1, br.m0, br.m1, fin);
+        } else {
+            if (h->dims == 3) bit_area_kernel<double, 3><<<bl, BITS_THREADS, 0, h->stream>>>((const double*)p, h->bits, N, NZ, br.m0, br.m1, fin);
+            else bit_area_kernel<double, 2><<<bl, BITS_THREADS, 0, h->stream>>>((const double*)p, h->bits, N, 1, br.m0, br.m1, fin);
+        }
+    } else if (h->precision == PRS_F32) {
         if (h->dims == 3) weighted_area_kernel<float, 3><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, fin);
         else weighted_area_kernel<float, 2><<<grid, 256, 0, h->stream>>>((const float*)p, N, NM, mlo, mhi, L, fin);
     } else {
@@ -777,6 +819,7 @@ int prs_copy_in(prs_handle h, const void* phi_src, const void* phidot_src, doubl
     PRS_CUDA(h, cudaMemcpyAsync((char*)h->pd[h->cur] + off, phidot_src, bytes, cudaMemcpyDefault, h->stream));
     PRS_CUDA(h, cudaStreamSynchronize(h->stream));
     h->eta0 = eta0; h->step = step; h->inited = true;
+    h->state_gen += 1;
     h->halo_valid = 0;                            // a slab's halo planes now belong to the old state
     return PRS_OK;
 }
@@ -935,6 +978,7 @@ int prs_slab_halo_filled(prs_handle h) {
     if (!h->slab) return fail(h, PRS_ERR_STATE, "prs_slab_halo_filled: not a slab");
     if (!h->inited) return fail(h, PRS_ERR_STATE, "prs_slab_halo_filled: no state yet");
     h->halo_valid = (int)h->halo;
+    h->state_gen += 1;                            // the halo planes' signs changed
     return PRS_OK;
 }
 

@@ -30,6 +30,10 @@ struct prs_ctx {
     int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
     prs::DiagPartial* partials;
     prs::DiagPartial* d_result;
+    bool bits_valid;                          // the bit array holds the signs of the state (bits_step, bits_cur, bits_gen)
+    int64_t bits_step;
+    int bits_cur;
+    uint64_t bits_gen, state_gen;             // state_gen: advanced by prs_init, prs_copy_in, prs_slab_halo_filled
     unsigned* d_ticket;                       // ticket counter of the diagnostics kernels' last-block reduction
     prs::DiagPartial* d_results;              // ring of reduced records for prs_run (RESULTS_CAP entries)
     unsigned* bits;                           // one sign bit per site: scratch of the sign-bit diagnostics pass

@@ -176,4 +176,103 @@ bit_links_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, const 
     finish_partials(fin, acc);
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Eq. 7 with the PRS orientation weight (R15) on the same bit words: the crossing forward
+// links ARE the set bits of c ^ right, c ^ up, c ^ above, so only they -- 2 % of the links of a formed network -- cost
+// anything beyond the words: their entries (owner group, axis, word, bit) go onto the warp's stack group by group and
+// are worked off 32 at a time by link_weight() (prs_kernels_generic.cuh: the gathers of the transverse neighbours, the
+// square root and the division in double), every lane busy.  partials[].links counts the crossing links again as a
+// cross-check against Eq. 7's unweighted count.  Rows and planes as in bit_links_kernel.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename T, int DIMS>
+__global__ void __launch_bounds__(BITS_THREADS)
+bit_area_kernel(const T* __restrict__ phi, const unsigned* __restrict__ bits, int N, int NZ, long long R0, long long R1,
+                DiagFinish fin) {
+    constexpr int W = VecOps<T>::W;
+    __shared__ unsigned short stack_all[BITS_THREADS / 32][BITS_STACK];
+    unsigned short* const stack = stack_all[threadIdx.x >> 5];
+    const unsigned lane = threadIdx.x & 31, lt = (1u << lane) - 1u;
+    const int NG = N / (32 * W);
+    const int NM = (DIMS == 3) ? NZ : N;                             // extent of the slowest axis (a slab: its planes)
+    const long long ngroups = (R1 - R0) * NG;
+    const long long wstep = (long long)gridDim.x * (BITS_THREADS / 32) * 32;
+    DiagPartial acc = {0ull, 0ull, 0.0};
+    int held = 0;
+    for (long long g0 = ((long long)blockIdx.x * (BITS_THREADS / 32) + (threadIdx.x >> 5)) * 32; g0 < ngroups; g0 += wstep) {
+        const long long gi = g0 + lane;
+        const bool live = gi < ngroups;
+        unsigned f[DIMS][W];                                         // crossing forward links per axis and word
+#pragma unroll
+        for (int k = 0; k < DIMS; ++k)
+#pragma unroll
+            for (int i = 0; i < W; ++i) f[k][i] = 0u;
+        int row = 0, grp = 0;                                        // this thread's row (y + N z) and group: < 2^31
+        if (live) {
+            const long long r = R0 + gi / NG;
+            const int g = (int)(gi % NG);
+            row = (int)r; grp = g;
+            const int y = (int)(r % N);
+            const long long ryp = (y == N - 1) ? r - (N - 1) : r + 1;
+            const int gxp = (g == NG - 1) ? 0 : g + 1;
+            BitWords<W> c, yp, zp;
+            c.load(bits + (r * NG + g) * W);
+            yp.load(bits + (ryp * NG + g) * W);
+            if (DIMS == 3) {
+                const long long z = r / N;
+                const long long rzp = (z == NZ - 1) ? r - (long long)(NZ - 1) * N : r + N;
+                zp.load(bits + (rzp * NG + g) * W);
+            }
+            const unsigned next0 = __ldg(bits + (r * NG + gxp) * W);
+#pragma unroll
+            for (int i = 0; i < W; ++i) {
+                const unsigned right = (i < W - 1) ? c.w[i + 1] : ((c.w[0] >> 1) | (next0 << 31));
+                f[0][i] = c.w[i] ^ right;
+                f[1][i] = c.w[i] ^ yp.w[i];
+                if (DIMS == 3) f[2][i] = c.w[i] ^ zp.w[i];
+#pragma unroll
+                for (int k = 0; k < DIMS; ++k) acc.links += __popc(f[k][i]);
+            }
+        }
+        auto work_off = [&](int n) {                                 // the top n <= 32 entries
+            PRS_JITTER(1u);
+            __syncwarp();
+            const unsigned e = ((int)lane < n) ? stack[held - n + (int)lane] : 0u;
+            const unsigned owner = e >> 9;
+            const int orow = __shfl_sync(0xffffffffu, row, owner), ogrp = __shfl_sync(0xffffffffu, grp, owner);
+            if ((int)lane < n) {
+                const unsigned long long x = (unsigned long long)(W * (32 * ogrp + (int)(e & 31u)) + (int)((e >> 5) & 3u));
+                const unsigned long long yy = (unsigned long long)(orow % N), zz = (unsigned long long)(orow / N);
+                const unsigned long long k = (e >> 7) & 3u;
+                // link_weight's entry: x | y << 20 | z << 40 | axis << 60 (2D: the row is y)
+                const unsigned long long entry = x | (yy << 20) | (zz << 40) | (k << 60);
+                acc.sum = __dadd_rn(acc.sum, link_weight<T, DIMS>(phi, N, NM, entry));
+            }
+            held -= n;
+            __syncwarp();
+        };
+        unsigned any = 0u;
+#pragma unroll
+        for (int k = 0; k < DIMS; ++k)
+#pragma unroll
+            for (int i = 0; i < W; ++i) any |= f[k][i];
+        for (unsigned owners = __ballot_sync(0xffffffffu, any != 0u); owners; owners &= owners - 1u) {
+            const unsigned owner = (unsigned)__ffs(owners) - 1u;
+#pragma unroll
+            for (int k = 0; k < DIMS; ++k)
+#pragma unroll
+                for (int i = 0; i < W; ++i) {
+                    const unsigned m = __shfl_sync(0xffffffffu, f[k][i], owner);
+                    if (m == 0u) continue;
+                    if ((m >> lane) & 1u)
+                        stack[held + __popc(m & lt)] = (unsigned short)((owner << 9) | ((unsigned)k << 7) | ((unsigned)i << 5) | lane);
+                    held += __popc(m);
+                    if (held >= 32) work_off(32);
+                }
+        }
+        if (held) work_off(held);
+    }
+    acc = block_reduce(acc);
+    finish_partials(fin, acc);
+}
+
 }  // namespace prs

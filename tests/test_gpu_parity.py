@@ -421,6 +421,47 @@ def test_weighted_area_matches_the_oracle_on_snapshots(prec, dims, N):
         assert C / np.sqrt(dims) - 1e-9 <= area <= C + 1e-9
 
 
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("dims,N", [(2, 2048), (3, 256)])
+def test_weighted_area_on_the_packed_sign_bits(prec, dims, N):
+    """From 2^22 sites up prs_weighted_area finds the crossing links as the set bits of the XOR words of the packed sign
+    bits (bit_area_kernel) instead of marching the lattice: against the oracle on the GPU's exact bytes and against the
+    marching kernel (forced through PRS_OPT_DIAG_KERNEL = TILED), early and on a formed network; the bit array left by
+    prs_diagnostics is reused (one launch instead of two) and a step invalidates it."""
+    g = prs.Simulation(dims, N, prec, seed=4)
+    g.init(1.0)
+    for nsteps in (0, 40, 300):
+        g.step(nsteps)
+        g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_AUTO)
+        l0 = g.kernel_launches
+        a_bits, rho_bits = g.weighted_area()
+        assert g.kernel_launches - l0 == 2                       # sign bits + links
+        l0 = g.kernel_launches
+        assert g.weighted_area() == (a_bits, rho_bits)           # same bits, and the bit array was reused
+        assert g.kernel_launches - l0 == 1
+        g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_TILED)
+        a_old, _ = g.weighted_area()
+        want = ref.weighted_area_of(g.copy_out()[0])
+        assert abs(a_bits - want) <= 1e-12 * want and abs(a_old - want) <= 1e-12 * want
+        assert rho_bits == a_bits / N ** dims
+    # prs_diagnostics (sign-bit pass) leaves the bits behind; a step invalidates them
+    g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_BITS)
+    d = g.diagnostics()
+    l0 = g.kernel_launches
+    a1, _ = g.weighted_area()
+    assert g.kernel_launches - l0 == 1 and d["link_count"] / np.sqrt(dims) <= a1 <= d["link_count"]
+    g.step(1)
+    l0 = g.kernel_launches
+    a2, _ = g.weighted_area()
+    assert g.kernel_launches - l0 == 2 and a2 != a1
+    assert abs(a2 - ref.weighted_area_of(g.copy_out()[0])) <= 1e-12 * a2
+    # copy_in invalidates them as well
+    phi = fg.kink_pair(dims, N, np.pi / 10.0, dtype=NP[prec])
+    g.copy_in(phi, np.zeros_like(phi))
+    assert g.weighted_area()[0] == 2.0 * N ** (dims - 1)           # walls normal to x: weight exactly 1
+    g.close()
+
+
 def test_weighted_area_of_special_fields():
     N = 64
     g = prs.Simulation(3, N, prs.F64)

@@ -279,7 +279,7 @@ def test_ranks_of_a_distributed_job_share_the_one_gpu(world, tmp_path):
         assert np.allclose(got[:, 2], want[:, 2], rtol=1e-12, atol=0)
 
 
-@pytest.mark.parametrize("N,world", [(64, 1), (64, 4), (132, 3)])
+@pytest.mark.parametrize("N,world", [(64, 1), (64, 4), (132, 3), (256, 2)])        # 256^3 in two slabs: the sign-bit path
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 def test_weighted_area_of_the_slabs_adds_up_to_the_lattice(N, world, prec):
     """prs_weighted_area on a slab returns its partial sum of Eq. 7's weighted area (transverse neighbours of the
