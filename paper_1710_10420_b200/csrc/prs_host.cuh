@@ -30,6 +30,10 @@ struct prs_ctx {
     int cur;                                  // index of the arrays holding phi^n, phidot^{n-1/2}
     prs::DiagPartial* partials;
     prs::DiagPartial* d_result;
+    bool seen_valid;                          // link count of the last prs_diagnostics and the state it belongs to
+    uint64_t seen_links, seen_gen;
+    int64_t seen_step;
+    int seen_cur;
     bool bits_valid;                          // the bit array holds the signs of the state (bits_step, bits_cur, bits_gen)
     int64_t bits_step;
     int bits_cur;

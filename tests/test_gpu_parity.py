@@ -444,6 +444,17 @@ def test_weighted_area_on_the_packed_sign_bits(prec, dims, N):
         want = ref.weighted_area_of(g.copy_out()[0])
         assert abs(a_bits - want) <= 1e-12 * want and abs(a_old - want) <= 1e-12 * want
         assert rho_bits == a_bits / N ** dims
+    # a state that prs_diagnostics has just found dense in crossing links (the white-noise start) goes through the
+    # marching kernel (one launch, no sign bits), a formed network through the bits; same value either way
+    h2 = prs.Simulation(dims, N, prec, seed=4)
+    h2.init(1.0)
+    a_unknown, _ = h2.weighted_area()                           # nothing known about the state: the bits
+    d = h2.diagnostics()
+    assert d["link_count"] > 0.25 * dims * N ** dims
+    l0 = h2.kernel_launches
+    a_dense, _ = h2.weighted_area()
+    assert h2.kernel_launches - l0 == 1 and abs(a_dense - a_unknown) <= 1e-12 * a_unknown
+    h2.close()
     # prs_diagnostics (sign-bit pass) leaves the bits behind; a step invalidates them
     g.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_BITS)
     d = g.diagnostics()
