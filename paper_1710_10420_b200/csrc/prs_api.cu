@@ -128,7 +128,7 @@ int resolve_step_kernel(const prs_ctx* h) {
         // 128^3 up -- on small lattices because it needs a quarter of the launches, on large ones
         // because it moves a quarter of the bytes; below that the single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        else if (h->N == 64 && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;   // 0.8 vs 1.1 us per step
+        else if ((h->N == 64 || h->N == 128) && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;   // us per step, FP32: 64^2 0.64 vs 1.10, 128^2 0.80 vs 1.14 (256^2: 1.92 vs 1.05)
         else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
         else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = PRS_KERNEL_TB2;
         else want = PRS_KERNEL_TILED;

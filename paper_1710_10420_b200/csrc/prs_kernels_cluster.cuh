@@ -58,6 +58,7 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
     constexpr int W = K::W;
     const int t = threadIdx.x;
     const int NQ = N / W, RNQ = R * NQ;
+    const int lgNQ = 31 - __clz(NQ);
     const size_t base = (size_t)rank * RN;                           // first site of this CTA's rows
 
     for (int i = t; i < RNQ; i += CLUSTER_THREADS) {
@@ -74,7 +75,7 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
         const T* const src_below = (s & 1) ? belowB : belowA;
         const T* const src_above = (s & 1) ? aboveB : aboveA;
         for (int v = t; v < RNQ; v += CLUSTER_THREADS) {
-            const int r = v / NQ, x = (v - r * NQ) * W;
+            const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;          // NQ is a power of two (N = 64, 128, 256)
             const int o = r * N + x;
             const V c = *reinterpret_cast<const V*>(src + o);
             const V ym = (r > 0) ? *reinterpret_cast<const V*>(src + o - N)

@@ -725,7 +725,7 @@ def test_copy_in_out_roundtrip_device_and_host_and_step_split():
     # device_pointers view equals copy_out
     pp, pv = g.device_pointers()
     assert pp and pv and pp != pv
-    assert g.kernel_launches >= 3              # 3 steps = a two-step launch + a single step, 4 steps = one four-step launch
+    assert g.kernel_launches >= 2              # 128^2: the cluster-resident kernel, one launch per prs_step call
 
 
 def test_error_paths_on_device():
