@@ -229,6 +229,36 @@ int prs_slab_halo_regions(prs_handle h, void* send[4], void* recv[4], size_t* by
 int prs_diag_combine(const prs_diag* parts, int n, int dims, int64_t N, prs_diag* out);
 int prs_slab_halo_filled(prs_handle h);
 
+/* ---- for callers that must not allocate ------------------------------------------------------------------------
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  prs_diagnostics_static
+ * measures PAPER.md Eqs. 7-8 (:57-66; the readings of DESIGN.md section 3, as prs_diagnostics) on fields the CALLER
+ * holds, with no handle and no workspace, and calls no cudaMalloc / cudaFree / cudaHostAlloc or any allocating routine:
+ * the scratch of the pass (one partial sum per block of 4096 sites, and a ticket counter) is a file-scope
+ * static __device__ array of prs_diagnostics_static_scratch_bytes() = 786 688 bytes, which every GPU that loads the
+ * library holds until the process exits.
+ *   phi, phidot   DEVICE pointers, inputs: dense T[N^dims], x fastest, T = float (PRS_F32) / double (PRS_F64);
+ *                 the call runs on the device that owns phi (made current for the call, restored after)
+ *   sums_device   DEVICE pointer, output: the three sums, written by the pass's last block; form rho and gv2 from them
+ *                 with prs_diag_combine (a prs_diag with these three fields set is one "part")
+ *   cuda_stream   cudaStream_t; the call queues one 256-byte memset and one kernel there and does NOT synchronise
+ *   err           optional HOST buffer of err_bytes for the reason of a failure (there is no handle to ask)
+ * Limit: N^dims <= prs_diagnostics_static_max_sites() = 2^27 = 134 217 728 sites (512^3, 11585^2): a larger lattice is
+ * refused with PRS_ERR_UNSUPPORTED and a message, never truncated; use prs_diagnostics on a handle for those.
+ * The array is shared by every call on a GPU and keeps the last call's contents; the ticket counter is cleared on the
+ * stream before each pass.  Calls that OVERLAP on one GPU (two streams, two threads) race on it: serialise them.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress, which may load the module): make
+ * that first call outside any stream capture.  Counts are bit-exact; sum_ratio differs from prs_diagnostics' by the
+ * order of its double additions only (about 1e-15 relative). */
+typedef struct {
+    uint64_t link_count;   /* C   (Eq. 7's sum of delta_pm)                   */
+    uint64_t wall_sites;   /* N_w (Eq. 8's N)                                 */
+    double   sum_ratio;    /* sum over wall sites of phidot^2 / V(phi)        */
+} prs_diag_sums;
+int prs_diagnostics_static(int dims, int64_t N, int precision, double W0, double phi0, const void* phi, const void* phidot,
+                           prs_diag_sums* sums_device, void* cuda_stream, char* err, size_t err_bytes);
+size_t  prs_diagnostics_static_scratch_bytes(void);
+int64_t prs_diagnostics_static_max_sites(void);
+
 const char* prs_last_error(prs_handle h);
 
 #ifdef __cplusplus

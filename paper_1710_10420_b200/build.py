@@ -28,7 +28,7 @@ OBJDIR = os.path.join(HERE, "_build")
 def units():
     """(object name, source file, extra flags): prs_api.cu plus prs_instances.cu once per kernel family,
     precision and arithmetic form (csrc/prs_instances.cu says which is which)."""
-    out = [("prs_api", "prs_api.cu", [])]
+    out = [("prs_api", "prs_api.cu", []), ("prs_static", "prs_static.cu", [])]
     for unit, family in ((3, "tbs2d"), (2, "tbs3d"), (1, "tb2")):       # longest first
         for T in ("float", "double"):
             for arith in (0, 1, 2):

@@ -24,6 +24,7 @@ ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WOR
 EXPORTS = ["prs_workspace_bytes", "prs_create", "prs_destroy", "prs_init", "prs_step", "prs_diagnostics",
            "prs_weighted_area", "prs_set_beta", "prs_copy_out", "prs_copy_in", "prs_sync", "prs_set_option", "prs_get_info",
            "prs_device_pointers", "prs_last_error", "prs_step_launch_info", "prs_run",
+           "prs_diagnostics_static", "prs_diagnostics_static_scratch_bytes", "prs_diagnostics_static_max_sites",
            "prs_slab_workspace_bytes", "prs_create_slab", "prs_slab_halo_regions", "prs_slab_halo_filled", "prs_diag_combine"]
 
 
@@ -74,6 +75,11 @@ def lib():
         L.prs_step_launch_info.argtypes = [vp, C.c_char_p, sz, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64),
                                            C.POINTER(i64), C.POINTER(i64)]
         L.prs_diag_combine.argtypes = [C.POINTER(Diag), ci, ci, i64, C.POINTER(Diag)]
+        L.prs_diagnostics_static.argtypes = [ci, i64, ci, dbl, dbl, vp, vp, vp, vp, C.c_char_p, sz]
+        L.prs_diagnostics_static_scratch_bytes.argtypes = []
+        L.prs_diagnostics_static_scratch_bytes.restype = sz
+        L.prs_diagnostics_static_max_sites.argtypes = []
+        L.prs_diagnostics_static_max_sites.restype = i64
         L.prs_last_error.argtypes = [vp]
         L.prs_last_error.restype = C.c_char_p
         _lib = L
@@ -95,6 +101,18 @@ def diag_combine(parts, dims, N):
     if rc != 0:
         raise PrsError(rc, "prs_diag_combine")
     return out.as_dict()
+
+
+def diagnostics_static(dims, N, precision, phi, phidot, sums_out, stream=None, W0=10.0, phi0=1.0):
+    """prs_diagnostics_static: Eqs. 7-8 on caller-held DEVICE fields with no handle, no workspace and no allocation
+    (the scratch is a static device array inside the library; at most 2^27 sites).  phi, phidot: device tensors or
+    addresses; sums_out: 24 bytes of device memory (e.g. a torch int64[3] tensor) that receive link_count, wall_sites
+    (uint64) and sum_ratio (double); stream: a torch stream or None for the legacy default stream.  Does not synchronise."""
+    err = C.create_string_buffer(400)
+    rc = lib().prs_diagnostics_static(dims, N, precision, W0, phi0, _raw_pointer(phi), _raw_pointer(phidot),
+                                      _raw_pointer(sums_out), None if stream is None else stream.cuda_stream, err, 400)
+    if rc != 0:
+        raise PrsError(rc, "prs_diagnostics_static", err.value.decode())
 
 
 def _raw_pointer(obj):
