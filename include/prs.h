@@ -88,7 +88,7 @@ enum {
     PRS_KERNEL_TB2     = 3,    /* temporally blocked: two steps per pass over HBM (same per-site   *
                                 * arithmetic, bit-identical to two single steps)                   */
     PRS_KERNEL_CLUSTER = 5,    /* small 2D boxes (N = 64, 128, 256): the state stays in the shared   *
-                                * memory of one 8-CTA thread-block cluster for up to 32 steps per    *
+                                * memory and registers of one 8-CTA thread-block cluster for up to 64 steps per    *
                                 * launch; bit-identical to single steps                              */
     PRS_KERNEL_BITS    = 6,    /* PRS_OPT_DIAG_KERNEL only: diagnostics on packed sign bits -- one pass reads phi   *
                                 * and packs a bit per site, a second counts links and wall sites on the bit words *
@@ -149,8 +149,12 @@ int prs_diagnostics(prs_handle h, prs_diag* out);
  * cycle's reduced record stays on the device (a ring of 4096 records in the workspace) and the records cross to the host
  * once per 4096 cycles, so a cycle costs its kernels and nothing else (the per-step transfer of the
  * partial sums is what hurts small boxes).  out: HOST array of ncycles records, out[i] = what prs_diagnostics would
- * have returned after (i + 1) * steps_per_cycle further steps -- identical bits: the same kernels in the same launch
- * configuration.  Synchronises the stream before it returns.  Not on a slab (PRS_ERR_UNSUPPORTED). */
+ * have returned after (i + 1) * steps_per_cycle further steps: the fields and the integer counts identical, and
+ * sum_ratio identical too (the same kernels in the same launch configuration) except where the cluster-resident
+ * small-box kernel is the step kernel (2D, N = 64 or 128 by default): there the diagnostics passes run INSIDE the step
+ * launches, up to 64 steps and all their passes per launch with the state on chip throughout, and sum_ratio differs
+ * from prs_diagnostics' by the order of its double additions (about 1e-15 relative).  Synchronises the stream before
+ * it returns.  Not on a slab (PRS_ERR_UNSUPPORTED). */
 int prs_run(prs_handle h, int64_t ncycles, int64_t steps_per_cycle, prs_diag* out);
 
 /* Orientation-weighted wall area of the current phi^n: PAPER.md Eq. 7 as printed (:59-62), the sum over

@@ -241,34 +241,43 @@ int step_many(prs_ctx* h, int S) {
     return PRS_OK;
 }
 
-// Up to CLUSTER_MAX_STEPS steps inside one cluster-resident launch (2D small boxes).
+// Up to CLUSTER_MAX_STEPS steps inside one cluster-resident launch (2D small boxes), with the diagnostics passes `dg`
+// schedules inside it (dg.every = 0: none).
 template <typename T, int ARITH>
-cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int nsteps) {
+cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int nsteps, const ClusterDiag& dg) {
     ClusterCoefs<T> ks;
     for (int s = 0; s < nsteps; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     for (int s = nsteps; s < CLUSTER_MAX_STEPS; ++s) ks.k[s] = ks.k[0];
     const size_t smem = cluster_smem_bytes<T>((int)h->N);
-    static std::atomic<unsigned long long> configured{0};      // per instantiation: devices already set up
-    {
-        const cudaError_t e = ensure_dynamic_smem(step2d_cluster_kernel<T, ARITH>, 227 * 1024, h->device, configured);
-        if (e != cudaSuccess) return e;
-    }
-    step2d_cluster_kernel<T, ARITH><<<CLUSTER_CTAS, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N, nsteps, ks);
+    const int vpt = cluster_vpt<T>((int)h->N);                 // vectors per thread: 1, 2 or 4 (cluster_supported)
+#define PRS_CLUSTER_LAUNCH(VPT)                                                                                              \
+    do {                                                                                                                     \
+        static std::atomic<unsigned long long> configured{0};  /* per instantiation: devices already set up */               \
+        /* the most any supported lattice needs (256^2 FP64: 128 KiB); 227 KB would exceed the limit with the static part */ \
+        const cudaError_t e = ensure_dynamic_smem(step2d_cluster_kernel<T, ARITH, VPT>, 128 * 1024, h->device, configured);  \
+        if (e != cudaSuccess) return e;                                                                                      \
+        step2d_cluster_kernel<T, ARITH, VPT><<<CLUSTER_CTAS, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N,    \
+                                                                                                 nsteps, ks, dg);           \
+    } while (0)
+    if (vpt == 1) PRS_CLUSTER_LAUNCH(1);
+    else if (vpt == 2) PRS_CLUSTER_LAUNCH(2);
+    else PRS_CLUSTER_LAUNCH(4);
+#undef PRS_CLUSTER_LAUNCH
     char name[96];
-    snprintf(name, sizeof(name), "step2d_cluster_kernel<%s,%d>", type_name<T>(), ARITH);
+    snprintf(name, sizeof(name), "step2d_cluster_kernel<%s,%d,%d>", type_name<T>(), ARITH, vpt);
     note_launch(h, name, dim3(CLUSTER_CTAS, 1, 1), dim3(CLUSTER_THREADS, 1, 1), smem, nsteps);
     return cudaGetLastError();
 }
 
 template <typename T>
-int step_cluster(prs_ctx* h, int nsteps) {
+int step_cluster(prs_ctx* h, int nsteps, const ClusterDiag& dg) {
     const T* p = (const T*)h->phi[h->cur];
     const T* v = (const T*)h->pd[h->cur];
     T* pn = (T*)h->phi[h->cur ^ 1];
     T* vn = (T*)h->pd[h->cur ^ 1];
-    const cudaError_t e = (h->opt_arith == PRS_ARITH_LITERAL) ? launch_cluster<T, ARITH_LITERAL>(h, p, v, pn, vn, nsteps)
-                        : (h->opt_arith == PRS_ARITH_COEF)  ? launch_cluster<T, ARITH_COEF>(h, p, v, pn, vn, nsteps)
-                                                            : launch_cluster<T, ARITH_FMA>(h, p, v, pn, vn, nsteps);
+    const cudaError_t e = (h->opt_arith == PRS_ARITH_LITERAL) ? launch_cluster<T, ARITH_LITERAL>(h, p, v, pn, vn, nsteps, dg)
+                        : (h->opt_arith == PRS_ARITH_COEF)  ? launch_cluster<T, ARITH_COEF>(h, p, v, pn, vn, nsteps, dg)
+                                                            : launch_cluster<T, ARITH_FMA>(h, p, v, pn, vn, nsteps, dg);
     if (e != cudaSuccess) return cuda_fail(h, e, "cluster kernel launch");
     h->launches += 1;
     h->cur ^= 1;
@@ -617,7 +626,8 @@ static int step_impl(prs_handle h, int64_t nsteps) {
     if (kernel == PRS_KERNEL_CLUSTER) {
         while (left > 0) {
             const int n = (int)std::min<int64_t>(left, CLUSTER_MAX_STEPS);
-            const int rc = (h->precision == PRS_F32) ? step_cluster<float>(h, n) : step_cluster<double>(h, n);
+            const ClusterDiag none = {0, 0, nullptr, 0.0, 0.0};
+            const int rc = (h->precision == PRS_F32) ? step_cluster<float>(h, n, none) : step_cluster<double>(h, n, none);
             if (rc != PRS_OK) return rc;
             left -= n;
         }
@@ -697,6 +707,30 @@ int prs_run(prs_handle h, int64_t ncycles, int64_t steps_per_cycle, prs_diag* ou
         const int64_t batch = std::min<int64_t>(ncycles - done, RESULTS_CAP);
         host.resize((size_t)batch);
         steps.resize((size_t)batch);
+        if (resolve_step_kernel(h) == PRS_KERNEL_CLUSTER && steps_per_cycle > 0) {
+            // small 2D boxes: the cluster-resident kernel runs the diagnostics passes inside its launches -- up to 64
+            // steps and all their passes per launch, the state never leaving the chip in between
+            const double pi = 3.14159265358979323846;
+            const double V0 = (pi * pi * h->phi0 * h->phi0) / (2.0 * h->W0 * h->W0), I = 1.0 / (h->phi0 * h->phi0);
+            h->main_launch.open = true;
+            int64_t left = batch * steps_per_cycle, until = steps_per_cycle, rec = 0;
+            const int64_t step0 = h->step;
+            while (left > 0) {
+                const int n = (int)std::min<int64_t>(left, CLUSTER_MAX_STEPS);
+                const int64_t passes = (until <= n) ? 1 + (n - until) / steps_per_cycle : 0;
+                const ClusterDiag dg = {passes ? (int)std::min<int64_t>(steps_per_cycle, 1 << 30) : 0, (int)std::min<int64_t>(until, 1 << 30),
+                                        h->d_results + rec, V0, I};
+                const int rc = (h->precision == PRS_F32) ? step_cluster<float>(h, n, dg) : step_cluster<double>(h, n, dg);
+                if (rc != PRS_OK) return rc;
+                // steps to the first pass of the next launch
+                until = passes ? steps_per_cycle - (n - (until + (passes - 1) * steps_per_cycle)) : until - n;
+                rec += passes;
+                left -= n;
+            }
+            for (int64_t i = 0; i < batch; ++i) steps[(size_t)i] = step0 + (i + 1) * steps_per_cycle;
+            h->last_step_kernel = PRS_KERNEL_CLUSTER;
+            h->last_diag_kernel = PRS_KERNEL_CLUSTER;
+        } else
         for (int64_t i = 0; i < batch; ++i) {                         // queued back to back: no sync, no transfer
             int rc = step_impl(h, steps_per_cycle);
             if (rc != PRS_OK) return rc;

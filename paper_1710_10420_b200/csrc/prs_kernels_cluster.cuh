@@ -1,105 +1,207 @@
 // prs_kernels_cluster.cuh -- the small-box regime (small boxes
 // under-use a GPU and are dominated by per-step overheads).  A 256^2 lattice is 768 KB of state: every
-// kernel launch of the streaming kernels is pure latency.  Here the whole state lives in the shared
-// memory of ONE thread-block cluster for many steps: 8 CTAs, each holding N/8 rows of phi (two
-// buffers, ping-pong) and phidot; the rows just across a CTA boundary are read from the neighbouring
-// CTA's shared memory (distributed shared memory), and one cluster barrier per step replaces a kernel
-// launch.  HBM is touched once on entry and once on exit of a launch of up to CLUSTER_MAX_STEPS steps.
+// kernel launch of the streaming kernels is pure latency.  Here the whole state lives ON CHIP in ONE
+// thread-block cluster for many steps: 8 CTAs, each owning N/8 rows.  A thread keeps the phi and phidot
+// of its own sites in REGISTERS from the first step of a launch to the last; only phi is published, to
+// a ping-pong pair of shared-memory buffers, for the neighbours: rows just across a CTA boundary are read
+// from the neighbouring CTA's shared memory (distributed shared memory), and one cluster barrier per step
+// replaces a kernel launch.  HBM is touched once on entry and once on exit of a launch of up to
+// CLUSTER_MAX_STEPS steps.
 //
-// Per-site arithmetic: the packed update of prs_pack.cuh, so the result is bit-identical to the other
-// kernels in every arithmetic form.  2D only, N in {64, 128, 256}; a thread owns whole 16-byte vectors.
+// The wall diagnostics (Eqs. 7-8) can run INSIDE the launch, at the cadence prs_run asks for:
+// after a step's barrier the state is all on chip -- own sites in registers, neighbours in shared memory --
+// so a pass costs a few hundred nanoseconds instead of a launch: sign masks, popcounts, Eq. 8's ratio at
+// the wall sites in double, block reduction, and rank 0 adds the eight CTAs' partials through distributed
+// shared memory, in rank order (reproducible), into the next record of the device ring.
+//
+// Per-site arithmetic: the packed update of prs_pack.cuh, so the fields are bit-identical to the other
+// kernels in every arithmetic form; the diagnostics' integer counts are exact, its double sum differs from the
+// stand-alone kernels' by the order of the additions only.  2D only, N in {64, 128, 256}.
 #pragma once
 
 #include <cooperative_groups.h>
 
 #include "prs_arith.cuh"
 #include "prs_pack.cuh"
+#include "prs_kernels_tiled.cuh"     // VecOps, sign_mask, mask_links, block_reduce
 
 namespace prs {
 
 constexpr int CLUSTER_CTAS = 8;
 constexpr int CLUSTER_THREADS = 1024;
-constexpr int CLUSTER_MAX_STEPS = 32;
+constexpr int CLUSTER_MAX_STEPS = 64;
+
+// 16-byte vectors a thread owns (template argument VPT): N^2 / (8 CTAs x W x 1024 threads), at least 1 --
+// 1 for N = 64, 128; 2 for 256^2 FP32; 4 for 256^2 FP64
+template <typename T>
+constexpr int cluster_vpt(int N) {
+    return (N / CLUSTER_CTAS) * (N / Pk<T>::W) <= CLUSTER_THREADS ? 1 : (N / CLUSTER_CTAS) * (N / Pk<T>::W) / CLUSTER_THREADS;
+}
+
+// A packed vector (prs_pack.cuh) as the plain vector type of the diagnostics code, register to register.
+__device__ __forceinline__ float4 plain_vec(ulonglong2 v) {
+    float4 f;
+    Pk<float>::unpack(v.x, f.x, f.y);
+    Pk<float>::unpack(v.y, f.z, f.w);
+    return f;
+}
+__device__ __forceinline__ double2 plain_vec(double2 v) { return v; }
 
 template <typename T>
 struct ClusterCoefs {
     StepCoef<T> k[CLUSTER_MAX_STEPS];
 };
 
+// When the diagnostics run inside a launch, and where their records go.
+struct ClusterDiag {
+    int every;                  // PRS steps between passes; 0 = no pass in this launch
+    int until;                  // steps from the launch's first step to its first pass (1 <= until <= every)
+    DiagPartial* records;       // DEVICE: the record of the launch's first pass; the following ones follow it
+    double V0, I;               // Eq. 8's constants
+};
+
 template <typename T>
 constexpr size_t cluster_smem_bytes(int N) {
-    return (size_t)3 * (size_t)(N / CLUSTER_CTAS) * (size_t)N * sizeof(T);
+    return (size_t)2 * (size_t)(N / CLUSTER_CTAS) * (size_t)N * sizeof(T);          // phi, ping and pong
 }
 
-template <typename T, int ARITH>
+template <typename T, int ARITH, int VPT>
 __global__ void __cluster_dims__(CLUSTER_CTAS, 1, 1) __launch_bounds__(CLUSTER_THREADS, 1)
 step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
-                      T* __restrict__ phidot_out, int N, int nsteps, ClusterCoefs<T> coefs) {
+                      T* __restrict__ phidot_out, int N, int nsteps, ClusterCoefs<T> coefs, ClusterDiag dg) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char cluster_smem[];
+    __shared__ DiagPartial cta_part;                                 // this CTA's partial of a diagnostics pass
+    using K = Pk<T>;
+    using V = typename K::V;
+    using O = VecOps<T>;
+    constexpr int W = K::W;
     const int R = N / CLUSTER_CTAS;                                  // rows held by this CTA
     const int RN = R * N;
-    T* const bufA = reinterpret_cast<T*>(cluster_smem);
-    T* const bufB = bufA + RN;
-    T* const pd = bufB + RN;
+    // (scalars picked by selects, not arrays indexed by the step's parity: those would live in local memory)
+    T* const buf0 = reinterpret_cast<T*>(cluster_smem);
+    T* const buf1 = buf0 + RN;
     const unsigned rank = cluster.block_rank();
     const unsigned below = (rank + CLUSTER_CTAS - 1) % CLUSTER_CTAS, above = (rank + 1) % CLUSTER_CTAS;
     // the two phi buffers of the CTAs that hold the rows below / above this CTA's rows
-    const T* const belowA = cluster.map_shared_rank(bufA, below);
-    const T* const belowB = cluster.map_shared_rank(bufB, below);
-    const T* const aboveA = cluster.map_shared_rank(bufA, above);
-    const T* const aboveB = cluster.map_shared_rank(bufB, above);
+    const T* const below0 = cluster.map_shared_rank(buf0, below);
+    const T* const below1 = cluster.map_shared_rank(buf1, below);
+    const T* const above0 = cluster.map_shared_rank(buf0, above);
+    const T* const above1 = cluster.map_shared_rank(buf1, above);
 
-    // A thread owns whole 16-byte vectors (4 floats / 2 doubles): vector v = t, t+1024, ... of this CTA's
-    // R x N/W vectors; the arithmetic is the packed form of prs_pack.cuh.
-    using K = Pk<T>;
-    using V = typename K::V;
-    constexpr int W = K::W;
     const int t = threadIdx.x;
-    const int NQ = N / W, RNQ = R * NQ;
+    const int NQ = N / W, RNQ = R * NQ;                              // NQ is a power of two (N = 64, 128, 256)
     const int lgNQ = 31 - __clz(NQ);
     const size_t base = (size_t)rank * RN;                           // first site of this CTA's rows
 
-    for (int i = t; i < RNQ; i += CLUSTER_THREADS) {
-        reinterpret_cast<V*>(bufA)[i] = K::ldg(phi + base + (size_t)i * W);
-        reinterpret_cast<V*>(pd)[i] = K::ldg(phidot + base + (size_t)i * W);
+    // A thread owns vectors v = t, t + 1024, ... of the CTA's R x NQ: phi and phidot stay in registers.
+    V creg[VPT], pdreg[VPT];
+#pragma unroll
+    for (int k = 0; k < VPT; ++k) {
+        const int v = t + k * CLUSTER_THREADS;
+        creg[k] = V{}; pdreg[k] = V{};
+        if (v < RNQ) {
+            creg[k] = K::ldg(phi + base + (size_t)v * W);
+            pdreg[k] = K::ldg(phidot + base + (size_t)v * W);
+            reinterpret_cast<V*>(buf0)[v] = creg[k];
+        }
     }
     cluster.sync();
 
+    int next_diag = dg.every > 0 ? dg.until : -1;                    // the pass follows local step next_diag - 1
+    int rec = 0;
+    bool tail_sync = false;
     for (int s = 0; s < nsteps; ++s) {
-        PackCoef<T> k;
-        k.template set<2>(coefs.k[s]);
-        const T* const src = (s & 1) ? bufB : bufA;
-        T* const dst = (s & 1) ? bufA : bufB;
-        const T* const src_below = (s & 1) ? belowB : belowA;
-        const T* const src_above = (s & 1) ? aboveB : aboveA;
-        for (int v = t; v < RNQ; v += CLUSTER_THREADS) {
-            const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;          // NQ is a power of two (N = 64, 128, 256)
-            const int o = r * N + x;
-            const V c = *reinterpret_cast<const V*>(src + o);
-            const V ym = (r > 0) ? *reinterpret_cast<const V*>(src + o - N)
-                                 : *reinterpret_cast<const V*>(src_below + (R - 1) * N + x);
-            const V yp = (r < R - 1) ? *reinterpret_cast<const V*>(src + o + N)
-                                     : *reinterpret_cast<const V*>(src_above + x);
-            const T left = src[r * N + (x == 0 ? N - 1 : x - 1)];
-            const T right = src[r * N + (x + W == N ? 0 : x + W)];
-            const V q = *reinterpret_cast<const V*>(pd + o);
-            V pn, vn;
-            packed_vector_update<T, 2, ARITH>(k, c, left, right, ym, yp, V{}, V{}, q, pn, vn);
-            *reinterpret_cast<V*>(dst + o) = pn;
-            *reinterpret_cast<V*>(pd + o) = vn;
+        PackCoef<T> kc;
+        kc.template set<2>(coefs.k[s]);
+        const bool odd = (s & 1) != 0;
+        const T* const src = odd ? buf1 : buf0;
+        T* const dst = odd ? buf0 : buf1;
+        const T* const src_below = odd ? below1 : below0;
+        const T* const src_above = odd ? above1 : above0;
+#pragma unroll
+        for (int k = 0; k < VPT; ++k) {
+            const int v = t + k * CLUSTER_THREADS;
+            if (v < RNQ) {
+                const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
+                const int o = r * N + x;
+                const V ym = (r > 0) ? *reinterpret_cast<const V*>(src + o - N)
+                                     : *reinterpret_cast<const V*>(src_below + (R - 1) * N + x);
+                const V yp = (r < R - 1) ? *reinterpret_cast<const V*>(src + o + N)
+                                         : *reinterpret_cast<const V*>(src_above + x);
+                const T left = src[r * N + (x == 0 ? N - 1 : x - 1)];
+                const T right = src[r * N + (x + W == N ? 0 : x + W)];
+                V pn, vn;
+                packed_vector_update<T, 2, ARITH>(kc, creg[k], left, right, ym, yp, V{}, V{}, pdreg[k], pn, vn);
+                creg[k] = pn; pdreg[k] = vn;
+                *reinterpret_cast<V*>(dst + o) = pn;
+            }
         }
-        // everyone has written phi^{n+1} and is done reading phi^n, which is overwritten next step
+        // everyone has published phi^{n+1} and is done reading phi^n, whose buffer is overwritten next step
         PRS_JITTER(1u + s);
         cluster.sync();
-        PRS_JITTER(40u + s);
+        PRS_JITTER(80u + s);
+        if (s + 1 == next_diag) {
+            // ---- Eqs. 7-8 on the state just reached: own sites in registers, neighbours in dst (and the CTAs beside)
+            const T* const cur = dst;
+            const T* const cur_below = odd ? below0 : below1;
+            const T* const cur_above = odd ? above0 : above1;
+            DiagPartial acc = {0ull, 0ull, 0.0};
+#pragma unroll
+            for (int k = 0; k < VPT; ++k) {
+                const int v = t + k * CLUSTER_THREADS;
+                if (v < RNQ) {
+                    const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
+                    const int o = r * N + x;
+                    const typename O::V c = plain_vec(creg[k]);
+                    const typename O::V q = plain_vec(pdreg[k]);
+                    const typename O::V ym = (r > 0) ? *reinterpret_cast<const typename O::V*>(cur + o - N)
+                                                     : *reinterpret_cast<const typename O::V*>(cur_below + (R - 1) * N + x);
+                    const typename O::V yp = (r < R - 1) ? *reinterpret_cast<const typename O::V*>(cur + o + N)
+                                                         : *reinterpret_cast<const typename O::V*>(cur_above + x);
+                    const unsigned l = Ar<T>::neg(cur[r * N + (x == 0 ? N - 1 : x - 1)]) ? 1u : 0u;
+                    const unsigned rr = Ar<T>::neg(cur[r * N + (x + W == N ? 0 : x + W)]) ? 1u : 0u;
+                    const unsigned mc = sign_mask<T>(c);
+                    unsigned nlinks, wallmask;
+                    mask_links<W, 2>(mc, l, rr, sign_mask<T>(ym), sign_mask<T>(yp), mc, mc, nlinks, wallmask);
+                    acc.links += nlinks;
+                    acc.walls += __popc(wallmask);
+#pragma unroll
+                    for (int i = 0; i < W; ++i)
+                        if ((wallmask >> i) & 1u) acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(O::get(c, i), O::get(q, i), dg.V0, dg.I));
+                }
+            }
+            acc = block_reduce(acc);
+            if (t == 0) cta_part = acc;
+            PRS_JITTER(160u + s);
+            cluster.sync();
+            if (rank == 0 && t == 0) {                               // the eight partials in rank order: reproducible
+                DiagPartial sum = {0ull, 0ull, 0.0};
+                for (unsigned rk = 0; rk < CLUSTER_CTAS; ++rk) {
+                    const DiagPartial* part = cluster.map_shared_rank(&cta_part, rk);
+                    sum.links += part->links;
+                    sum.walls += part->walls;
+                    sum.sum = __dadd_rn(sum.sum, part->sum);
+                }
+                dg.records[rec] = sum;
+            }
+            // cta_part is written again only after a further cluster barrier, which rank 0's thread 0 joins after it has
+            // read the partials; but no CTA may EXIT while rank 0 still reads its shared memory: see tail_sync
+            tail_sync = (s + 1 == nsteps);
+            ++rec;
+            next_diag += dg.every;
+        }
     }
-    const T* const fin = (nsteps & 1) ? bufB : bufA;
-    for (int i = t; i < RNQ; i += CLUSTER_THREADS) {
-        K::stg(phi_out + base + (size_t)i * W, reinterpret_cast<const V*>(fin)[i]);
-        K::stg(phidot_out + base + (size_t)i * W, reinterpret_cast<const V*>(pd)[i]);
+#pragma unroll
+    for (int k = 0; k < VPT; ++k) {
+        const int v = t + k * CLUSTER_THREADS;
+        if (v < RNQ) {
+            K::stg(phi_out + base + (size_t)v * W, creg[k]);
+            K::stg(phidot_out + base + (size_t)v * W, pdreg[k]);
+        }
     }
+    if (tail_sync) cluster.sync();                                   // a pass after the last step: rank 0 is done reading
 }
 
 }  // namespace prs

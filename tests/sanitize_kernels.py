@@ -70,6 +70,24 @@ def main():
         for N in (64, 128):                                       # cluster-resident small-box kernel
             want = run(2, N, prec, prs.KERNEL_GENERIC, 35)
             assert run(2, N, prec, prs.KERNEL_CLUSTER, 35) == want
+            # ... and with the diagnostics passes inside its launches (prs_run): counts against the generic kernels'
+            a, b2 = prs.Simulation(2, N, prec, seed=4), prs.Simulation(2, N, prec, seed=4)
+            a.set_step_kernel(prs.KERNEL_CLUSTER)
+            b2.set_step_kernel(prs.KERNEL_GENERIC)
+            b2.set_option(binding.OPT_DIAG_KERNEL, prs.KERNEL_GENERIC)
+            a.init(1.0)
+            b2.init(1.0)
+            recs = a.run(23, 7)
+            for rcd in recs:
+                b2.step(7)
+                d = b2.diagnostics()
+                assert (rcd["link_count"], rcd["wall_sites"]) == (d["link_count"], d["wall_sites"]), (N, prec, rcd["step"])
+                assert abs(rcd["sum_ratio"] - d["sum_ratio"]) <= 1e-10 * d["sum_ratio"]
+            pa, pb = a.copy_out(), b2.copy_out()
+            assert pa[0].tobytes() == pb[0].tobytes() and pa[1].tobytes() == pb[1].tobytes()
+            launches += a.kernel_launches + b2.kernel_launches
+            a.close()
+            b2.close()
             print("ok step cluster            2D N=%-4d %s" % (N, "f32" if prec == prs.F32 else "f64"), flush=True)
         # diagnostics (tiled and generic) and the weighted area, early and on a forming network
         for dims, N in ((3, 68), (3, 132), (2, 260), (3, 128), (2, 256)):

@@ -239,11 +239,11 @@ def test_two_rows_per_thread_kernel_equals_single_steps_bitwise(prec, N, S):
 @pytest.mark.parametrize("N", [64, 128, 256])
 def test_cluster_resident_kernel_equals_single_steps_bitwise(prec, N):
     """Small-box kernel (state in the shared memory of one 8-CTA cluster, neighbour rows through
-    distributed shared memory, one cluster barrier per step): 1, 2, 31, 32, 33 and 75 steps (launches of
-    at most 32) against the single-step kernel, all arithmetic forms; and against the oracle."""
+    distributed shared memory, one cluster barrier per step): 1, 2, 31, 32, 33, 75 and 130 steps (launches of
+    at most 64) against the single-step kernel, all arithmetic forms; and against the oracle."""
     phi, pd = fg.random_state(2, N, 5, NP[prec])
     for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
-        for nsteps in (1, 2, 31, 32, 33, 75) if arith == prs.ARITH_FMA else (33,):
+        for nsteps in (1, 2, 31, 32, 33, 75, 130) if arith == prs.ARITH_FMA else (33,):
             outs = []
             for kernel in (prs.KERNEL_TILED, prs.KERNEL_CLUSTER):
                 g = prs.Simulation(2, N, prec, era_m=2.0)
@@ -253,7 +253,7 @@ def test_cluster_resident_kernel_equals_single_steps_bitwise(prec, N):
                 g.step(nsteps)
                 outs.append(g.copy_out())
                 if kernel == prs.KERNEL_CLUSTER:
-                    assert g.kernel_launches == (nsteps + 31) // 32
+                    assert g.kernel_launches == (nsteps + 63) // 64
             assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
     g = prs.Simulation(2, N, prec, seed=3)
     g.set_step_kernel(prs.KERNEL_CLUSTER)
@@ -927,19 +927,65 @@ def test_batched_cycles_equal_the_step_and_diagnostics_loop(dims, N, prec, every
     b = prs.Simulation(dims, N, prec, seed=3)
     a.init(1.0)
     b.init(1.0)
+    fused = dims == 2 and N in (64, 128)                         # AUTO = the cluster-resident kernel
     got = a.run(ncyc, every)
     assert len(got) == ncyc
+    assert (a.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_CLUSTER) == fused
     for i in range(ncyc):
         b.step(every)
         want = b.diagnostics()
         if i < 40 or i % 97 == 0 or i >= ncyc - 5:
-            assert got[i] == want, i
+            if fused:                                           # the cluster kernel measures inside its launches: the
+                for k in ("step", "eta", "link_count", "wall_sites", "rho"):     # double sum is added in another order
+                    assert got[i][k] == want[k], (i, k)
+                assert abs(got[i]["sum_ratio"] - want["sum_ratio"]) <= 1e-10 * max(want["sum_ratio"], 1e-300)
+                assert abs(got[i]["gv2"] - want["gv2"]) <= 1e-10 * max(want["gv2"], 1e-300)
+            else:
+                assert got[i] == want, i
     assert got[-1]["step"] == ncyc * every and a.get_info(binding.INFO_STEP) == ncyc * every
     pa, pb = a.copy_out(), b.copy_out()
     assert pa[0].tobytes() == pb[0].tobytes() and pa[1].tobytes() == pb[1].tobytes()
     assert a.run(0, 5) == [] and a.get_info(binding.INFO_STEP) == ncyc * every
     zero = a.run(2, 0)                                          # no steps: the same state measured twice
     assert zero[0] == zero[1] and zero[0]["step"] == ncyc * every
+    a.close()
+    b.close()
+
+
+@pytest.mark.parametrize("prec", [prs.F32, prs.F64])
+@pytest.mark.parametrize("N", [64, 128, 256])
+@pytest.mark.parametrize("every,ncyc", [(10, 40), (1, 130), (64, 3), (65, 3), (7, 19), (200, 2)])
+def test_diagnostics_inside_the_cluster_resident_launches(prec, N, every, ncyc):
+    """prs_run with the cluster-resident kernel: the diagnostics passes run inside the step launches (up to 64 steps per
+    launch, any cadence: several passes per launch, a pass on a launch's last step, launches without a pass).  Counts
+    equal to the oracle's on the GPU path's own snapshots and to prs_diagnostics', the double sum within 1e-10; the fields
+    bit-identical to the single-step kernel's; one launch per 64 steps and none for the diagnostics."""
+    a = prs.Simulation(2, N, prec, seed=8, era_m=2.0)
+    a.set_step_kernel(prs.KERNEL_CLUSTER)
+    b = prs.Simulation(2, N, prec, seed=8, era_m=2.0)
+    b.set_step_kernel(prs.KERNEL_TILED)
+    a.init(1.0)
+    b.init(1.0)
+    l0 = a.kernel_launches
+    got = a.run(ncyc, every)
+    assert a.kernel_launches - l0 == (ncyc * every + 63) // 64
+    for i in range(ncyc):
+        b.step(every)
+        want = b.diagnostics()
+        assert got[i]["step"] == want["step"] == (i + 1) * every and got[i]["eta"] == want["eta"]
+        assert got[i]["link_count"] == want["link_count"] and got[i]["wall_sites"] == want["wall_sites"], i
+        assert abs(got[i]["sum_ratio"] - want["sum_ratio"]) <= 1e-10 * max(want["sum_ratio"], 1e-300), i
+        if i in (0, ncyc - 1):
+            o = ref.diagnostics_of(*b.copy_out())
+            assert got[i]["link_count"] == o["link_count"] and got[i]["wall_sites"] == o["wall_sites"]
+            assert abs(got[i]["sum_ratio"] - o["sum_ratio"]) <= 1e-10 * max(o["sum_ratio"], 1e-300)
+    pa, pb = a.copy_out(), b.copy_out()
+    assert pa[0].tobytes() == pb[0].tobytes() and pa[1].tobytes() == pb[1].tobytes()
+    a.run(2, every)                                             # more cycles after a finished batch continue the count
+    again = a.run(1, every)
+    b.step(3 * every)
+    w = b.diagnostics()
+    assert again[0]["step"] == w["step"] and again[0]["link_count"] == w["link_count"]
     a.close()
     b.close()
 
