@@ -113,12 +113,27 @@ def test_multiply_adds_are_fused_exactly_where_the_arithmetic_form_says():
     assert len(arith_of) == step_kernels >= 120 and sorted(set(arith_of.values())) == [0, 1, 2]
     for a in (0, 1, 2):                                   # every family is built in every arithmetic form
         assert sum(1 for v in arith_of.values() if v == a) == step_kernels // 3
+    # Fused instructions of the kernel's OWN step precision: FFMA / FFMA2 in a float kernel, DFMA in a double one.  (A
+    # float kernel may hold DFMAs -- the cluster-resident kernel measures Eqs. 7-8 inside its launches, in double, and the
+    # correctly rounded FP64 division expands into DFMAs -- but its step arithmetic could only ever fuse into FFMA / FFMA2,
+    # which is where ptxas's packed contraction strikes.)
+    is_double = {m: ("<double," in d) for m, d in zip(names, plain)}
+    is_cluster = {m: ("step2d_cluster_kernel" in d) for m, d in zip(names, plain)}
     cur, fused = None, {k: 0 for k in arith_of}
     for line in sass.splitlines():
         m = re.search(r"Function : (\S+)", line)
         if m:
             cur = m.group(1)
-        elif cur in fused and re.search(r"\b(FFMA2?|DFMA)\b", line):
-            fused[cur] += 1
-    assert [k for k, a in arith_of.items() if a == 1 and fused[k]] == []
+        elif cur in fused and re.search(r"\bDFMA\b" if is_double[cur] else r"\bFFMA2?\b", line):
+            # "FFMA Rd, RZ, Ra, Rb" multiplies by zero: the FP64 division's expansion uses it as an exponent-range probe on
+            # the high word of its operands (it follows the division's DFMA pair); no product is fused there
+            if not re.search(r"\bFFMA\s+R\d+, RZ,", line):
+                fused[cur] += 1
+    # COEF: nothing fused.  One exemption, stated: the DOUBLE cluster-resident kernels, whose in-launch FP64 division
+    # cannot be told from step arithmetic in SASS; they are held by bit-identity with the single-step kernel and the
+    # oracle in all three forms (test_cluster_resident_kernel_equals_single_steps_bitwise), and double arithmetic has no
+    # packed form for ptxas to contract in the first place.
+    exempt = [k for k in arith_of if is_cluster[k] and is_double[k]]
+    assert 0 < len(exempt) <= 9
+    assert [k for k, a in arith_of.items() if a == 1 and fused[k] and k not in exempt] == []
     assert [k for k, a in arith_of.items() if a == 2 and not fused[k]] == []
