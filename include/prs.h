@@ -76,6 +76,8 @@ enum {
                                 * applies (1024^3: 17 % faster), else 1                                */
     PRS_OPT_DIAG_CHUNK  = 10,  /* tuning: planes (3D) / rows (2D) one CTA of the one-pass diagnostics kernel marches;
                                 * 0 = auto                                                               */
+    PRS_OPT_CLUSTER_CTAS = 11, /* tuning, cluster-resident kernel at N = 256: CTAs in the cluster, 16 (opt-in size; what 0 =
+                                * auto takes where the device can co-schedule it) or 8                     */
     PRS_OPT_TBS_LOADER  = 9    /* tuning, 3D multi-step kernel: how the shared-memory rings are filled: 0 (default)
                                 * = TMA bulk copies of whole tile rows completing on mbarriers where a lattice
                                 * row holds >= 32 16-byte vectors, else per-thread cp.async; 1 = always cp.async;

@@ -121,6 +121,31 @@ bool cluster_supported(const prs_ctx* h) {
     return smem <= 227 * 1024;
 }
 
+// Can this device co-schedule ONE cluster of 16 CTAs x 1024 threads (non-portable size)?  Asked once per device.
+bool cluster16_fits(const prs_ctx* h) {
+    static std::atomic<unsigned long long> asked{0}, yes{0};
+    const unsigned long long bit = (h->device >= 0 && h->device < 64) ? (1ull << h->device) : 0ull;
+    if (bit && (asked.load() & bit)) return (yes.load() & bit) != 0;
+    auto kern = step2d_cluster_kernel<float, ARITH_FMA, 1, 16>;
+    DeviceGuard guard(h->device);
+    int n = 0;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e == cudaSuccess) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(16, 1, 1); cfg.blockDim = dim3(CLUSTER_THREADS, 1, 1); cfg.dynamicSmemBytes = cluster_smem_bytes<double>(256, 16);
+        cudaLaunchAttribute at;
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = 16; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+        cfg.attrs = &at; cfg.numAttrs = 1;
+        e = cudaOccupancyMaxActiveClusters(&n, kern, &cfg);
+    }
+    if (e != cudaSuccess) cudaGetLastError();
+    const bool ok = (e == cudaSuccess && n >= 1);
+    if (bit) { if (ok) yes.fetch_or(bit); asked.fetch_or(bit); }
+    return ok;
+}
+
 int resolve_step_kernel(const prs_ctx* h) {
     int want = h->opt_step_kernel;
     if (want == PRS_KERNEL_AUTO) {
@@ -128,7 +153,10 @@ int resolve_step_kernel(const prs_ctx* h) {
         // 128^3 up -- on small lattices because it needs a quarter of the launches, on large ones
         // because it moves a quarter of the bytes; below that the single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        else if ((h->N == 64 || h->N == 128) && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;   // us per step, FP32: 64^2 0.64 vs 1.10, 128^2 0.80 vs 1.14 (256^2: 1.92 vs 1.05)
+        // the cluster-resident kernel against the streaming one, us per step (FP32 | FP64): 64^2 0.58 | 0.58 vs 1.03 | 1.03;
+        // 128^2 0.71 | 0.96 vs 1.03 | 1.34; 256^2 on 16 CTAs 0.96 | 1.44 vs 1.09 | 1.37 (on 8 CTAs 1.50 | 3.0)
+        else if ((h->N == 64 || h->N == 128) && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;
+        else if (h->N == 256 && h->precision == PRS_F32 && h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h)) want = PRS_KERNEL_CLUSTER;
         else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
         else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = PRS_KERNEL_TB2;
         else want = PRS_KERNEL_TILED;
@@ -248,25 +276,59 @@ cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int
     ClusterCoefs<T> ks;
     for (int s = 0; s < nsteps; ++s) ks.k[s] = coef_at<T>(h, h->step + s);
     for (int s = nsteps; s < CLUSTER_MAX_STEPS; ++s) ks.k[s] = ks.k[0];
-    const size_t smem = cluster_smem_bytes<T>((int)h->N);
-    const int vpt = cluster_vpt<T>((int)h->N);                 // vectors per thread: 1, 2 or 4 (cluster_supported)
-#define PRS_CLUSTER_LAUNCH(VPT)                                                                                              \
+    // 256^2 runs as ONE cluster of 16 CTAs (non-portable size, opt-in) where the device can co-schedule one: a thread then
+    // owns half as many vectors (FP32: one, like 128^2 with 8 CTAs).  Everything else, and the fall-back, is 8 CTAs.
+    int ncta = (h->N == 256 && h->opt_cluster_ctas != 8) ? 16 : CLUSTER_CTAS;
+    for (;;) {
+        const size_t smem = cluster_smem_bytes<T>((int)h->N, ncta);
+        const int vpt = cluster_vpt<T>((int)h->N, ncta);
+        cudaError_t e = cudaSuccess;
+        bool fits = true;
+#define PRS_CLUSTER_LAUNCH(VPT, NCTA)                                                                                        \
     do {                                                                                                                     \
+        auto kern = step2d_cluster_kernel<T, ARITH, VPT, NCTA>;                                                              \
         static std::atomic<unsigned long long> configured{0};  /* per instantiation: devices already set up */               \
-        /* the most any supported lattice needs (256^2 FP64: 128 KiB); 227 KB would exceed the limit with the static part */ \
-        const cudaError_t e = ensure_dynamic_smem(step2d_cluster_kernel<T, ARITH, VPT>, 128 * 1024, h->device, configured);  \
-        if (e != cudaSuccess) return e;                                                                                      \
-        step2d_cluster_kernel<T, ARITH, VPT><<<CLUSTER_CTAS, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N,    \
-                                                                                                 nsteps, ks, dg);           \
+        static std::atomic<unsigned long long> unfit{0};       /* devices that cannot hold a cluster of NCTA */              \
+        const unsigned long long bit = (h->device >= 0 && h->device < 64) ? (1ull << h->device) : 0ull;                      \
+        if (bit && (unfit.load() & bit)) { fits = false; break; }                                                            \
+        const bool first = !(bit && (configured.load() & bit));                                                              \
+        /* the most any supported lattice needs (256^2 FP64 on 8 CTAs: 128 KiB); 227 KB would exceed the limit with the     \
+           static part */                                                                                                    \
+        e = ensure_dynamic_smem(kern, 128 * 1024, h->device, configured);                                                    \
+        if (e != cudaSuccess) break;                                                                                         \
+        if (NCTA > 8 && first) {                                                                                             \
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);                               \
+            int nclusters = 0;                                                                                               \
+            if (e == cudaSuccess) {                                                                                          \
+                cudaLaunchConfig_t cfg = {};                                                                                 \
+                cfg.gridDim = dim3(NCTA, 1, 1); cfg.blockDim = dim3(CLUSTER_THREADS, 1, 1); cfg.dynamicSmemBytes = smem;     \
+                cudaLaunchAttribute at;                                                                                      \
+                at.id = cudaLaunchAttributeClusterDimension;                                                                 \
+                at.val.clusterDim.x = NCTA; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;                                \
+                cfg.attrs = &at; cfg.numAttrs = 1;                                                                           \
+                e = cudaOccupancyMaxActiveClusters(&nclusters, kern, &cfg);                                                  \
+            }                                                                                                                \
+            if (e != cudaSuccess || nclusters < 1) {                                                                         \
+                cudaGetLastError();                                                                                          \
+                e = cudaSuccess; fits = false;                                                                               \
+                if (bit) unfit.fetch_or(bit);                                                                                \
+                break;                                                                                                       \
+            }                                                                                                                \
+        }                                                                                                                    \
+        kern<<<NCTA, CLUSTER_THREADS, smem, h->stream>>>(p, v, pn, vn, (int)h->N, nsteps, ks, dg);                           \
     } while (0)
-    if (vpt == 1) PRS_CLUSTER_LAUNCH(1);
-    else if (vpt == 2) PRS_CLUSTER_LAUNCH(2);
-    else PRS_CLUSTER_LAUNCH(4);
+        if (ncta == 16) { if (vpt == 1) PRS_CLUSTER_LAUNCH(1, 16); else PRS_CLUSTER_LAUNCH(2, 16); }
+        else if (vpt == 1) PRS_CLUSTER_LAUNCH(1, 8);
+        else if (vpt == 2) PRS_CLUSTER_LAUNCH(2, 8);
+        else PRS_CLUSTER_LAUNCH(4, 8);
 #undef PRS_CLUSTER_LAUNCH
-    char name[96];
-    snprintf(name, sizeof(name), "step2d_cluster_kernel<%s,%d,%d>", type_name<T>(), ARITH, vpt);
-    note_launch(h, name, dim3(CLUSTER_CTAS, 1, 1), dim3(CLUSTER_THREADS, 1, 1), smem, nsteps);
-    return cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        if (!fits && ncta == 16) { ncta = CLUSTER_CTAS; continue; }       // no room for 16 CTAs in one cluster here
+        char name[96];
+        snprintf(name, sizeof(name), "step2d_cluster_kernel<%s,%d,%d,%d>", type_name<T>(), ARITH, vpt, ncta);
+        note_launch(h, name, dim3(ncta, 1, 1), dim3(CLUSTER_THREADS, 1, 1), smem, nsteps);
+        return cudaGetLastError();
+    }
 }
 
 template <typename T>
@@ -486,6 +548,7 @@ static int create_common(prs_handle* out, int dims, int64_t N, size_t sites, int
     h->opt_tbs_rows = 0;                          // auto (prs_launch_tbs.cuh)
     h->opt_tbs_loader = 0;
     h->opt_diag_chunk = 0;
+    h->opt_cluster_ctas = 0;
     h->seen_valid = false; h->seen_links = 0; h->seen_step = 0; h->seen_cur = 0; h->seen_gen = 0;
     h->bits_valid = false; h->bits_step = 0; h->bits_cur = 0; h->bits_gen = 0; h->state_gen = 0;
     h->last_step_kernel = 0; h->last_diag_kernel = 0; h->launches = 0;
@@ -707,7 +770,12 @@ int prs_run(prs_handle h, int64_t ncycles, int64_t steps_per_cycle, prs_diag* ou
         const int64_t batch = std::min<int64_t>(ncycles - done, RESULTS_CAP);
         host.resize((size_t)batch);
         steps.resize((size_t)batch);
-        if (resolve_step_kernel(h) == PRS_KERNEL_CLUSTER && steps_per_cycle > 0) {
+        // (256^2 FP64: stepping alone the streaming kernel is a little faster, 1.37 against 1.44 us, but a cycle with its
+        // diagnostics inside the cluster launch wins up to a cadence of 50 and beyond: 1.75 against 2.11 at 10, 1.51 against 1.58 at 50)
+        const bool run_on_cluster = resolve_step_kernel(h) == PRS_KERNEL_CLUSTER ||
+                                    (h->opt_step_kernel == PRS_KERNEL_AUTO && h->dims == 2 && h->N == 256 && steps_per_cycle <= 64 &&
+                                     h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h));
+        if (run_on_cluster && steps_per_cycle > 0) {
             // small 2D boxes: the cluster-resident kernel runs the diagnostics passes inside its launches -- up to 64
             // steps and all their passes per launch, the state never leaving the chip in between
             const double pi = 3.14159265358979323846;
@@ -940,6 +1008,10 @@ int prs_set_option(prs_handle h, int option, int64_t value) {
             if (value != 0 && value != 1 && !(value == 2 && h->dims == 3))
                 return fail(h, PRS_ERR_INVALID_ARG, "tbs_rows must be 0 (auto), 1 or, in 3D, 2");
             h->opt_tbs_rows = (int)value;
+            return PRS_OK;
+        case PRS_OPT_CLUSTER_CTAS:
+            if (value != 0 && value != 8 && value != 16) return fail(h, PRS_ERR_INVALID_ARG, "cluster_ctas must be 0 (auto), 8 or 16");
+            h->opt_cluster_ctas = (int)value;
             return PRS_OK;
         case PRS_OPT_DIAG_CHUNK:
             if (value < 0 || value > (1 << 20)) return fail(h, PRS_ERR_INVALID_ARG, "diag_chunk must be >= 0");

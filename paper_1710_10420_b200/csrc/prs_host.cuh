@@ -45,7 +45,7 @@ struct prs_ctx {
     double eta0;
     int64_t step;
     bool inited;
-    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps, opt_tbs_rows, opt_tbs_loader, opt_diag_chunk;
+    int opt_step_kernel, opt_arith, opt_diag_kernel, opt_chunk, opt_tile_y, opt_tb2_tile_y, opt_tbs_steps, opt_tbs_rows, opt_tbs_loader, opt_diag_chunk, opt_cluster_ctas;
     int last_step_kernel, last_diag_kernel;
     int64_t launches;
     int sm_count;

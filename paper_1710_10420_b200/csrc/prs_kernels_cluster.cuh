@@ -11,8 +11,8 @@
 // The wall diagnostics (Eqs. 7-8) can run INSIDE the launch, at the cadence prs_run asks for:
 // after a step's barrier the state is all on chip -- own sites in registers, neighbours in shared memory --
 // so a pass costs a few hundred nanoseconds instead of a launch: sign masks, popcounts, Eq. 8's ratio at
-// the wall sites in double, block reduction, and rank 0 adds the eight CTAs' partials through distributed
-// shared memory, in rank order (reproducible), into the next record of the device ring.
+// the wall sites in double, block reduction, and one warp of rank 0 fetches the CTAs' partials through distributed
+// shared memory and adds them in a fixed order (reproducible) into the next record of the device ring.
 //
 // Per-site arithmetic: the packed update of prs_pack.cuh, so the fields are bit-identical to the other
 // kernels in every arithmetic form; the diagnostics' integer counts are exact, its double sum differs from the
@@ -27,15 +27,15 @@
 
 namespace prs {
 
-constexpr int CLUSTER_CTAS = 8;
+constexpr int CLUSTER_CTAS = 8;                  // portable cluster size; 256^2 takes 16 (opt-in, non-portable) where it fits
 constexpr int CLUSTER_THREADS = 1024;
 constexpr int CLUSTER_MAX_STEPS = 64;
 
 // 16-byte vectors a thread owns (template argument VPT): N^2 / (8 CTAs x W x 1024 threads), at least 1 --
-// 1 for N = 64, 128; 2 for 256^2 FP32; 4 for 256^2 FP64
+// with 8 CTAs 1 for N = 64, 128; 2 for 256^2 FP32; 4 for 256^2 FP64; with 16 CTAs 1 / 2 for 256^2 FP32 / FP64
 template <typename T>
-constexpr int cluster_vpt(int N) {
-    return (N / CLUSTER_CTAS) * (N / Pk<T>::W) <= CLUSTER_THREADS ? 1 : (N / CLUSTER_CTAS) * (N / Pk<T>::W) / CLUSTER_THREADS;
+constexpr int cluster_vpt(int N, int ncta = CLUSTER_CTAS) {
+    return (N / ncta) * (N / Pk<T>::W) <= CLUSTER_THREADS ? 1 : (N / ncta) * (N / Pk<T>::W) / CLUSTER_THREADS;
 }
 
 // A packed vector (prs_pack.cuh) as the plain vector type of the diagnostics code, register to register.
@@ -61,12 +61,12 @@ struct ClusterDiag {
 };
 
 template <typename T>
-constexpr size_t cluster_smem_bytes(int N) {
-    return (size_t)2 * (size_t)(N / CLUSTER_CTAS) * (size_t)N * sizeof(T);          // phi, ping and pong
+constexpr size_t cluster_smem_bytes(int N, int ncta = CLUSTER_CTAS) {
+    return (size_t)2 * (size_t)(N / ncta) * (size_t)N * sizeof(T);                  // phi, ping and pong
 }
 
-template <typename T, int ARITH, int VPT>
-__global__ void __cluster_dims__(CLUSTER_CTAS, 1, 1) __launch_bounds__(CLUSTER_THREADS, 1)
+template <typename T, int ARITH, int VPT, int NCTA>
+__global__ void __cluster_dims__(NCTA, 1, 1) __launch_bounds__(CLUSTER_THREADS, 1)
 step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T* __restrict__ phi_out,
                       T* __restrict__ phidot_out, int N, int nsteps, ClusterCoefs<T> coefs, ClusterDiag dg) {
     namespace cg = cooperative_groups;
@@ -77,13 +77,13 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
     using V = typename K::V;
     using O = VecOps<T>;
     constexpr int W = K::W;
-    const int R = N / CLUSTER_CTAS;                                  // rows held by this CTA
+    const int R = N / NCTA;                                          // rows held by this CTA
     const int RN = R * N;
     // (scalars picked by selects, not arrays indexed by the step's parity: those would live in local memory)
     T* const buf0 = reinterpret_cast<T*>(cluster_smem);
     T* const buf1 = buf0 + RN;
     const unsigned rank = cluster.block_rank();
-    const unsigned below = (rank + CLUSTER_CTAS - 1) % CLUSTER_CTAS, above = (rank + 1) % CLUSTER_CTAS;
+    const unsigned below = (rank + NCTA - 1) % NCTA, above = (rank + 1) % NCTA;
     // the two phi buffers of the CTAs that hold the rows below / above this CTA's rows
     const T* const below0 = cluster.map_shared_rank(buf0, below);
     const T* const below1 = cluster.map_shared_rank(buf1, below);
@@ -176,15 +176,16 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
             if (t == 0) cta_part = acc;
             PRS_JITTER(160u + s);
             cluster.sync();
-            if (rank == 0 && t == 0) {                               // the eight partials in rank order: reproducible
-                DiagPartial sum = {0ull, 0ull, 0.0};
-                for (unsigned rk = 0; rk < CLUSTER_CTAS; ++rk) {
-                    const DiagPartial* part = cluster.map_shared_rank(&cta_part, rk);
-                    sum.links += part->links;
-                    sum.walls += part->walls;
-                    sum.sum = __dadd_rn(sum.sum, part->sum);
+            if (rank == 0 && t < 32) {
+                // warp 0 of rank 0: lane l fetches CTA l's partial (the remote reads overlap instead of queueing up), then
+                // the shuffle tree of warp_reduce adds them -- an order fixed by the lane numbers alone: reproducible
+                DiagPartial part = {0ull, 0ull, 0.0};
+                if (t < NCTA) {
+                    const DiagPartial* rp = cluster.map_shared_rank(&cta_part, (unsigned)t);
+                    part.links = rp->links; part.walls = rp->walls; part.sum = rp->sum;
                 }
-                dg.records[rec] = sum;
+                part = warp_reduce(part);
+                if (t == 0) dg.records[rec] = part;
             }
             // cta_part is written again only after a further cluster barrier, which rank 0's thread 0 joins after it has
             // read the partials; but no CTA may EXIT while rank 0 still reads its shared memory: see tail_sync

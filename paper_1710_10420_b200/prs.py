@@ -15,7 +15,7 @@ from . import build as _build
 F32, F64 = 0, 1
 ARITH_LITERAL, ARITH_COEF, ARITH_FMA = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_TB2, KERNEL_TBS, KERNEL_CLUSTER, KERNEL_BITS = 0, 1, 2, 3, 4, 5, 6
-OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS, OPT_TBS_LOADER, OPT_DIAG_CHUNK = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
+OPT_STEP_KERNEL, OPT_ARITH, OPT_DIAG_KERNEL, OPT_CHUNK, OPT_TILE_Y, OPT_TB2_TILE_Y, OPT_TBS_STEPS, OPT_TBS_ROWS, OPT_TBS_LOADER, OPT_DIAG_CHUNK, OPT_CLUSTER_CTAS = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 INFO_KERNEL_LAUNCHES, INFO_STEP_KERNEL, INFO_STEP, INFO_DIAG_KERNEL = 1, 2, 3, 4
 INFO_HALO_VALID, INFO_HALO_PLANES, INFO_DEVICE = 5, 6, 7
 ERR_NAMES = {1: "PRS_ERR_INVALID_ARG", 2: "PRS_ERR_UNSUPPORTED", 3: "PRS_ERR_WORKSPACE",

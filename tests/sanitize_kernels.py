@@ -67,7 +67,7 @@ def main():
                     got = run(dims, N, prec, kernel, 9, opts, chunk)
                     assert got == want, (name, dims, N, prec)
                     print("ok step %-18s %dD N=%-4d %s" % (name, dims, N, "f32" if prec == prs.F32 else "f64"), flush=True)
-        for N in (64, 128):                                       # cluster-resident small-box kernel
+        for N in (64, 128, 256):                                  # cluster-resident small-box kernel (256: 16 CTAs)
             want = run(2, N, prec, prs.KERNEL_GENERIC, 35)
             assert run(2, N, prec, prs.KERNEL_CLUSTER, 35) == want
             # ... and with the diagnostics passes inside its launches (prs_run): counts against the generic kernels'

@@ -927,7 +927,7 @@ def test_batched_cycles_equal_the_step_and_diagnostics_loop(dims, N, prec, every
     b = prs.Simulation(dims, N, prec, seed=3)
     a.init(1.0)
     b.init(1.0)
-    fused = dims == 2 and N in (64, 128)                         # AUTO = the cluster-resident kernel
+    fused = dims == 2 and N in (64, 128, 256)                    # AUTO runs these cycles inside cluster-resident launches
     got = a.run(ncyc, every)
     assert len(got) == ncyc
     assert (a.get_info(binding.INFO_STEP_KERNEL) == prs.KERNEL_CLUSTER) == fused
@@ -981,6 +981,19 @@ def test_diagnostics_inside_the_cluster_resident_launches(prec, N, every, ncyc):
             assert abs(got[i]["sum_ratio"] - o["sum_ratio"]) <= 1e-10 * max(o["sum_ratio"], 1e-300)
     pa, pb = a.copy_out(), b.copy_out()
     assert pa[0].tobytes() == pb[0].tobytes() and pa[1].tobytes() == pb[1].tobytes()
+    if N == 256:                                                # the fall-back for devices without room for 16 CTAs
+        c = prs.Simulation(2, N, prec, seed=8, era_m=2.0)
+        c.set_step_kernel(prs.KERNEL_CLUSTER)
+        c.set_option(binding.OPT_CLUSTER_CTAS, 8)
+        c.init(1.0)
+        got8 = c.run(ncyc, every)
+        assert c.step_launch_info()["grid"] == [8, 1, 1] and a.step_launch_info()["grid"] == [16, 1, 1]
+        for x, y in zip(got, got8):
+            assert (x["step"], x["link_count"], x["wall_sites"]) == (y["step"], y["link_count"], y["wall_sites"])
+            assert abs(x["sum_ratio"] - y["sum_ratio"]) <= 1e-10 * max(y["sum_ratio"], 1e-300)
+        pc = c.copy_out()
+        assert pa[0].tobytes() == pc[0].tobytes() and pa[1].tobytes() == pc[1].tobytes()
+        c.close()
     a.run(2, every)                                             # more cycles after a finished batch continue the count
     again = a.run(1, every)
     b.step(3 * every)
