@@ -226,13 +226,15 @@ dist.init_process_group("gloo")
 sim = sharded.ShardedSimulation(%d, prs.F32, seed=5, era_m=2.0)
 sim.init(1.0)
 diags = []
+areas = []
 for k in (4, 9, 2, 6):
     sim.step(k)
     diags.append(sim.diagnostics())
+    areas.append(sim.weighted_area()[0])           # the slabs' partial areas, all-reduced over the ranks
 phi, pd = sim.copy_out()
 np.save(os.path.join(%r, "phi%%d.npy" %% rank), phi)
 np.save(os.path.join(%r, "pd%%d.npy" %% rank), pd)
-np.save(os.path.join(%r, "diag%%d.npy" %% rank), np.array([[d["link_count"], d["wall_sites"], d["sum_ratio"]] for d in diags]))
+np.save(os.path.join(%r, "diag%%d.npy" %% rank), np.array([[d["link_count"], d["wall_sites"], d["sum_ratio"], a] for d, a in zip(diags, areas)]))
 dist.barrier()
 sim.close()
 dist.destroy_process_group()
@@ -266,7 +268,7 @@ def test_ranks_of_a_distributed_job_share_the_one_gpu(world, tmp_path):
     for k in (4, 9, 2, 6):
         whole.step(k)
         d = whole.diagnostics()
-        want.append([d["link_count"], d["wall_sites"], d["sum_ratio"]])
+        want.append([d["link_count"], d["wall_sites"], d["sum_ratio"], whole.weighted_area()[0]])
     wp, wv = whole.copy_out()
     whole.close()
     gp = np.concatenate([np.load(os.path.join(out, "phi%d.npy" % r)) for r in range(world)])
@@ -277,6 +279,7 @@ def test_ranks_of_a_distributed_job_share_the_one_gpu(world, tmp_path):
         got = np.load(os.path.join(out, "diag%d.npy" % r))
         assert np.array_equal(got[:, :2], want[:, :2])
         assert np.allclose(got[:, 2], want[:, 2], rtol=1e-12, atol=0)
+        assert np.allclose(got[:, 3], want[:, 3], rtol=1e-12, atol=0)       # Eq. 7's weighted area of the whole lattice
 
 
 @pytest.mark.parametrize("N,world", [(64, 1), (64, 4), (132, 3), (256, 2)])        # 256^3 in two slabs: the sign-bit path
