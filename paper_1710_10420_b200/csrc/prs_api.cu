@@ -379,7 +379,8 @@ bool diag_tiled_supported(const prs_ctx* h) {
 // The packed-sign-bit pass (prs_kernels_bits.cuh): whole groups of 32 vectors per row.
 bool diag_bits_supported(const prs_ctx* h) {
     const int W = vec_width(h->precision);
-    return h->N % (32 * W) == 0 && h->N <= (1 << 30);
+    // whole groups of 32 vectors per row; the kernels index groups and rows with 32 bits
+    return h->N % (32 * W) == 0 && h->N <= (1 << 30) && h->S / (size_t)(32 * W) < ((size_t)1 << 31) && h->S / (size_t)h->N < ((size_t)1 << 31);
 }
 
 int resolve_diag_kernel(const prs_ctx* h) {

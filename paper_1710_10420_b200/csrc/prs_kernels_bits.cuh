@@ -40,36 +40,30 @@ sign_bits_kernel(const T* __restrict__ phi, unsigned* __restrict__ bits, int N, 
     constexpr int W = O::W;
     const int lane = threadIdx.x & 31;
     const int NG = N / (32 * W);
-    const long long ngroups = (r1 - r0) * NG;
+    // A row is a whole number of groups, so group gi of the array (row-major, gi = r NG + g) starts at site 32 W gi and its
+    // words at W gi: no row / group decomposition is needed here at all.  (The first version divided a 64-bit index by NG
+    // per group: ncu showed 85 instructions per group, issue slots 73 % busy, DRAM at 61 % -- bound by that, not by HBM.)
+    const long long gbeg = r0 * NG, gend = r1 * NG;
     const long long wstep = (long long)gridDim.x * (blockDim.x >> 5);
-    // four groups per warp and iteration: four independent 16-byte loads per lane in flight.  (ncu had the one-load
-    // version at 0.89 ms for the 4.3 GB of 1024^3 FP32 against a floor of 0.67; in the warm loop the whole diagnostics
-    // pass measured the same with either, 1.66 ms -- kept because it costs nothing, not because it was shown to help.)
-    constexpr int U = 4;
-    for (long long g0 = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); g0 < ngroups; g0 += U * wstep) {
+    constexpr int U = 4;                                             // four independent 16-byte loads per lane in flight
+    for (long long g0 = gbeg + (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); g0 < gend; g0 += U * wstep) {
         V v[U];
-        long long word0[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const long long gi = g0 + u * wstep;
-            word0[u] = -1;
-            if (gi < ngroups) {                                      // warp-uniform
-                const long long r = r0 + gi / NG;
-                const int g = (int)(gi % NG);
-                v[u] = O::ld(phi + r * N + (long long)W * (32 * g + lane));
-                word0[u] = (r * NG + g) * W;
-            }
+            if (gi < gend) v[u] = O::ld(phi + (gi * 32 + lane) * W);                  // warp-uniform condition
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            if (word0[u] < 0) continue;
+            const long long gi = g0 + u * wstep;
+            if (gi >= gend) break;
             unsigned mine = 0u;
 #pragma unroll
             for (int i = 0; i < W; ++i) {
                 const unsigned w = __ballot_sync(0xffffffffu, Ar<T>::neg(O::get(v[u], i)));
                 if (lane == i) mine = w;
             }
-            if (lane < W) bits[word0[u] + lane] = mine;
+            if (lane < W) bits[gi * W + lane] = mine;
         }
     }
 }
@@ -119,9 +113,13 @@ bit_links_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, const 
 #pragma unroll
         for (int i = 0; i < W; ++i) wall[i] = 0u;
         if (live) {
-            const long long r = R0 + gi / NG;
-            const int g = (int)(gi % NG);
-            const int y = (int)(r % N);
+            // 32-bit arithmetic: an array has fewer than 2^31 groups and rows (the host checks), and 64-bit divisions
+            // were most of this kernel's 360 instructions per thread
+            const unsigned gu = (unsigned)gi, ru = gu / (unsigned)NG;
+            const int g = (int)(gu - ru * (unsigned)NG);
+            const long long r = R0 + (long long)ru;
+            const unsigned rr = (unsigned)r, zu = rr / (unsigned)N;
+            const int y = (int)(rr - zu * (unsigned)N);
             site0 = r * N + (long long)(32 * W) * g;
             const long long ryp = (y == N - 1) ? r - (N - 1) : r + 1, rym = (y == 0) ? r + (N - 1) : r - 1;
             const int gxp = (g == NG - 1) ? 0 : g + 1, gxm = (g == 0) ? NG - 1 : g - 1;
@@ -130,7 +128,7 @@ bit_links_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, const 
             yp.load(bits + (ryp * NG + g) * W);
             ym.load(bits + (rym * NG + g) * W);
             if (DIMS == 3) {
-                const long long z = r / N, plane = (long long)N;
+                const long long z = (long long)zu, plane = (long long)N;
                 const long long rzp = (z == NZ - 1) ? r - (long long)(NZ - 1) * plane : r + plane;
                 const long long rzm = (z == 0) ? r + (long long)(NZ - 1) * plane : r - plane;
                 zp.load(bits + (rzp * NG + g) * W);
@@ -202,6 +200,13 @@ bit_links_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, const 
 // square root and the division in double), every lane busy.  partials[].links counts the crossing links again as a
 // cross-check against Eq. 7's unweighted count.  Rows and planes as in bit_links_kernel.
 // ------------------------------------------------------------------------------------------------------------------
+// One out-of-line copy of Eq. 7's link weight: inlined at the dozen places where the unrolled push loop may pop the stack
+// it made the kernel so large that half its stall samples were instruction fetches (ncu: no_instructions 50 %).
+template <typename T, int DIMS>
+__device__ __noinline__ double link_weight_call(const T* __restrict__ phi, int N, int NM, unsigned long long entry) {
+    return link_weight<T, DIMS>(phi, N, NM, entry);
+}
+
 template <typename T, int DIMS>
 __global__ void __launch_bounds__(BITS_THREADS)
 bit_area_kernel(const T* __restrict__ phi, const unsigned* __restrict__ bits, int N, int NZ, long long R0, long long R1,
@@ -226,17 +231,19 @@ bit_area_kernel(const T* __restrict__ phi, const unsigned* __restrict__ bits, in
             for (int i = 0; i < W; ++i) f[k][i] = 0u;
         int row = 0, grp = 0;                                        // this thread's row (y + N z) and group: < 2^31
         if (live) {
-            const long long r = R0 + gi / NG;
-            const int g = (int)(gi % NG);
+            const unsigned gu = (unsigned)gi, ru = gu / (unsigned)NG;                 // 32-bit: see bit_links_kernel
+            const int g = (int)(gu - ru * (unsigned)NG);
+            const long long r = R0 + (long long)ru;
+            const unsigned rr = (unsigned)r, zu = rr / (unsigned)N;
             row = (int)r; grp = g;
-            const int y = (int)(r % N);
+            const int y = (int)(rr - zu * (unsigned)N);
             const long long ryp = (y == N - 1) ? r - (N - 1) : r + 1;
             const int gxp = (g == NG - 1) ? 0 : g + 1;
             BitWords<W> c, yp, zp;
             c.load(bits + (r * NG + g) * W);
             yp.load(bits + (ryp * NG + g) * W);
             if (DIMS == 3) {
-                const long long z = r / N;
+                const long long z = (long long)zu;
                 const long long rzp = (z == NZ - 1) ? r - (long long)(NZ - 1) * N : r + N;
                 zp.load(bits + (rzp * NG + g) * W);
             }
@@ -263,7 +270,7 @@ bit_area_kernel(const T* __restrict__ phi, const unsigned* __restrict__ bits, in
                 const unsigned long long k = (e >> 7) & 3u;
                 // link_weight's entry: x | y << 20 | z << 40 | axis << 60 (2D: the row is y)
                 const unsigned long long entry = x | (yy << 20) | (zz << 40) | (k << 60);
-                acc.sum = __dadd_rn(acc.sum, link_weight<T, DIMS>(phi, N, NM, entry));
+                acc.sum = __dadd_rn(acc.sum, link_weight_call<T, DIMS>(phi, N, NM, entry));
             }
             held -= n;
             __syncwarp();
