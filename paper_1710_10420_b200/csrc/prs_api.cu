@@ -129,7 +129,7 @@ bool cluster16_fits(const prs_ctx* h) {
     auto kern = step2d_cluster_kernel<float, ARITH_FMA, 1, 16>;
     DeviceGuard guard(h->device);
     int n = 0;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CLUSTER_SMEM_LIMIT);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     if (e == cudaSuccess) {
         cudaLaunchConfig_t cfg = {};
@@ -156,7 +156,7 @@ int resolve_step_kernel(const prs_ctx* h) {
         // the cluster-resident kernel against the streaming one, us per step (FP32 | FP64): 64^2 0.58 | 0.58 vs 1.03 | 1.03;
         // 128^2 0.71 | 0.96 vs 1.03 | 1.34; 256^2 on 16 CTAs 0.96 | 1.44 vs 1.09 | 1.37 (on 8 CTAs 1.50 | 3.0)
         else if ((h->N == 64 || h->N == 128) && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;
-        else if (h->N == 256 && h->precision == PRS_F32 && h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h)) want = PRS_KERNEL_CLUSTER;
+        else if (h->N == 256 && h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h)) want = PRS_KERNEL_CLUSTER;
         else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
         else if (h->S >= ((size_t)1 << 22) && tb2_supported(h)) want = PRS_KERNEL_TB2;
         else want = PRS_KERNEL_TILED;
@@ -292,9 +292,9 @@ cudaError_t launch_cluster(prs_ctx* h, const T* p, const T* v, T* pn, T* vn, int
         const unsigned long long bit = (h->device >= 0 && h->device < 64) ? (1ull << h->device) : 0ull;                      \
         if (bit && (unfit.load() & bit)) { fits = false; break; }                                                            \
         const bool first = !(bit && (configured.load() & bit));                                                              \
-        /* the most any supported lattice needs (256^2 FP64 on 8 CTAs: 128 KiB); 227 KB would exceed the limit with the     \
-           static part */                                                                                                    \
-        e = ensure_dynamic_smem(kern, 128 * 1024, h->device, configured);                                                    \
+        /* above the most any supported lattice needs (256^2 FP64 on 8 CTAs: 136 KiB); 227 KB would exceed the limit with   \
+           the static part */                                                                                                \
+        e = ensure_dynamic_smem(kern, CLUSTER_SMEM_LIMIT, h->device, configured);                                            \
         if (e != cudaSuccess) break;                                                                                         \
         if (NCTA > 8 && first) {                                                                                             \
             e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);                               \

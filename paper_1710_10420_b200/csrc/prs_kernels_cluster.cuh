@@ -4,15 +4,16 @@
 // thread-block cluster for many steps: 8 CTAs, each owning N/8 rows.  A thread keeps the phi and phidot
 // of its own sites in REGISTERS from the first step of a launch to the last; only phi is published, to
 // a ping-pong pair of shared-memory buffers, for the neighbours: rows just across a CTA boundary are read
-// from the neighbouring CTA's shared memory (distributed shared memory), and one cluster barrier per step
-// replaces a kernel launch.  HBM is touched once on entry and once on exit of a launch of up to
-// CLUSTER_MAX_STEPS steps.
+// from a halo row that the neighbouring CTA fills through distributed shared memory (st.async + mbarrier, below): a
+// __syncthreads and a neighbour handshake per step replace a kernel launch.  HBM is touched once on entry and once
+// on exit of a launch of up to CLUSTER_MAX_STEPS steps.
 //
 // The wall diagnostics (Eqs. 7-8) can run INSIDE the launch, at the cadence prs_run asks for:
 // after a step's barrier the state is all on chip -- own sites in registers, neighbours in shared memory --
 // so a pass costs a few hundred nanoseconds instead of a launch: sign masks, popcounts, Eq. 8's ratio at
-// the wall sites in double, block reduction, and one warp of rank 0 fetches the CTAs' partials through distributed
-// shared memory and adds them in a fixed order (reproducible) into the next record of the device ring.
+// the wall sites in double, a warp reduction into a per-pass, per-warp slot of the CTA's shared memory -- no barrier; at
+// the end of the launch each CTA adds up its warps' partials, and the warps of rank 0 fetch the CTAs' partials through
+// distributed shared memory and add them, all in a fixed order (reproducible), into the records of the device ring.
 //
 // Per-site arithmetic: the packed update of prs_pack.cuh, so the fields are bit-identical to the other
 // kernels in every arithmetic form; the diagnostics' integer counts are exact, its double sum differs from the
@@ -45,6 +46,48 @@ __device__ __forceinline__ void cluster_barrier() {
     asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
 }
 
+// Between steps a CTA depends on its TWO NEIGHBOURS only, and only through one row each: the row just below its rows and
+// the row just above.  So the step loop takes no cluster barrier (measured at ~800 cycles a step: its release is a
+// MEMBAR.ALL.GPU in every warp) and reads no remote shared memory (~215 cycles a load).  Instead the threads that own a
+// CTA's first / last row PUSH the vectors they have just computed into a halo row in the neighbour's shared memory with
+// st.async, whose bytes are counted on an mbarrier in that neighbour (complete_tx): data and signal travel together, no
+// fence.  The neighbour's boundary-row threads wait on that mbarrier (acquire, cluster scope) right before they read the
+// halo; everyone else needs the CTA's own __syncthreads only, so the inner rows of step s+1 run while the halo rows
+// of phi^{s+1} are in flight.
+//
+// Two halo slots alternate with the parity of the step.  Slot (s+1)&1 receives phi^{s+1} during the neighbour's step s and is
+// read in step s+1; it is written again in the neighbour's step s+2, which cannot start before this CTA's boundary row of step
+// s+1 has arrived there -- pushed by the very threads that read the slot, after they read it.  Each slot and side has its own
+// mbarrier (one arrival, by the thread that arms it with the row's byte count for the next use, plus the bytes); the arming
+// thread is one of the row's pushers and arms before it pushes, so an arming always precedes the bytes it counts.
+__device__ __forceinline__ unsigned cluster_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned cluster_map(unsigned local, unsigned rank) {
+    unsigned remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(remote) : "r"(local), "r"(rank));
+    return remote;
+}
+__device__ __forceinline__ void halo_bar_init(unsigned bar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void halo_arm(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void halo_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nHALO_WAIT:\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra HALO_DONE;\nbra HALO_WAIT;\nHALO_DONE:\n}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void halo_push(unsigned remote, unsigned remote_bar, unsigned long long a, unsigned long long b) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];\n" ::"r"(remote), "l"(a),
+                 "l"(b), "r"(remote_bar)
+                 : "memory");
+}
+__device__ __forceinline__ void halo_push(unsigned remote, unsigned remote_bar, ulonglong2 v) { halo_push(remote, remote_bar, v.x, v.y); }
+__device__ __forceinline__ void halo_push(unsigned remote, unsigned remote_bar, double2 v) {
+    halo_push(remote, remote_bar, (unsigned long long)__double_as_longlong(v.x), (unsigned long long)__double_as_longlong(v.y));
+}
+
 // A packed vector (prs_pack.cuh) as the plain vector type of the diagnostics code, register to register.
 __device__ __forceinline__ float4 plain_vec(ulonglong2 v) {
     float4 f;
@@ -67,9 +110,19 @@ struct ClusterDiag {
     double V0, I;               // Eq. 8's constants
 };
 
+constexpr size_t CLUSTER_SMEM_LIMIT = 176 * 1024;      // dynamic shared memory the kernels are configured for (most used: 168 KiB)
+
+// What a warp keeps of a diagnostics pass until the end of the launch (its 32 vectors x VPT: the counts fit 16 bits).
+struct ClusterWarpPart {
+    unsigned links, walls;
+    double sum;
+};
+
 template <typename T>
 constexpr size_t cluster_smem_bytes(int N, int ncta = CLUSTER_CTAS) {
-    return (size_t)2 * (size_t)(N / ncta) * (size_t)N * sizeof(T);                  // phi, ping and pong
+    return (size_t)2 * (size_t)(N / ncta) * (size_t)N * sizeof(T)                   // phi, ping and pong
+           + (size_t)4 * (size_t)N * sizeof(T)                                      // halo rows: 2 slots x (below, above)
+           + (size_t)CLUSTER_MAX_STEPS * (CLUSTER_THREADS / 32) * sizeof(ClusterWarpPart);      // the warps' partials, per pass
 }
 
 template <typename T, int ARITH, int VPT, int NCTA>
@@ -79,7 +132,8 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char cluster_smem[];
-    __shared__ DiagPartial cta_part;                                 // this CTA's partial of a diagnostics pass
+    __shared__ DiagPartial cta_part[CLUSTER_MAX_STEPS];              // this CTA's partials of the launch's diagnostics passes
+    __shared__ __align__(8) unsigned long long halo_bar[2][2];       // [slot][0: the row below arrives here, 1: the row above]
     using K = Pk<T>;
     using V = typename K::V;
     using O = VecOps<T>;
@@ -89,18 +143,27 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
     // (scalars picked by selects, not arrays indexed by the step's parity: those would live in local memory)
     T* const buf0 = reinterpret_cast<T*>(cluster_smem);
     T* const buf1 = buf0 + RN;
+    T* const halo = buf1 + RN;                                       // halo[(slot * 2 + side) * N + x]
+    ClusterWarpPart* const warp_part = reinterpret_cast<ClusterWarpPart*>(halo + 4 * N);      // [pass][warp]
     const unsigned rank = cluster.block_rank();
     const unsigned below = (rank + NCTA - 1) % NCTA, above = (rank + 1) % NCTA;
-    // the two phi buffers of the CTAs that hold the rows below / above this CTA's rows
-    const T* const below0 = cluster.map_shared_rank(buf0, below);
-    const T* const below1 = cluster.map_shared_rank(buf1, below);
-    const T* const above0 = cluster.map_shared_rank(buf0, above);
-    const T* const above1 = cluster.map_shared_rank(buf1, above);
+    const unsigned row_bytes = (unsigned)N * (unsigned)sizeof(T);
 
     const int t = threadIdx.x;
     const int NQ = N / W, RNQ = R * NQ;                              // NQ is a power of two (N = 64, 128, 256)
     const int lgNQ = 31 - __clz(NQ);
     const size_t base = (size_t)rank * RN;                           // first site of this CTA's rows
+    const unsigned bars = cluster_smem_u32(&halo_bar[0][0]);
+    if (t == 0) {
+        for (unsigned i = 0; i < 4; ++i) halo_bar_init(bars + 8u * i);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        for (unsigned i = 0; i < 4; ++i) halo_arm(bars + 8u * i, row_bytes);       // slot 1: the pushes of step 0, slot 0: of step 1
+    }
+    // where this CTA's first row goes: the "above" halo of the CTA below it; its last row: the "below" halo of the CTA above
+    const unsigned push_down_halo = cluster_map(cluster_smem_u32(halo + N), below);
+    const unsigned push_down_bar = cluster_map(bars + 8u, below);
+    const unsigned push_up_halo = cluster_map(cluster_smem_u32(halo), above);
+    const unsigned push_up_bar = cluster_map(bars, above);
 
     // A thread owns vectors v = t, t + 1024, ... of the CTA's R x NQ: phi and phidot stay in registers.
     V creg[VPT], pdreg[VPT];
@@ -114,57 +177,77 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
             reinterpret_cast<V*>(buf0)[v] = creg[k];
         }
     }
-    cluster_barrier();
+    if (t < 2 * NQ) {
+        // slot 0 of the halo for step 0: the rows around this CTA's rows straight from global memory (periodic in y)
+        const int side = t >> lgNQ, q = t & (NQ - 1);
+        const int grow = side == 0 ? ((int)rank * R + N - 1) % N : ((int)rank * R + R) % N;
+        reinterpret_cast<V*>(halo + side * N)[q] = K::ldg(phi + (size_t)grow * N + (size_t)q * W);
+    }
+    cluster_barrier();                                               // the state is on chip; every CTA's mbarriers are armed
 
     int next_diag = dg.every > 0 ? dg.until : -1;                    // the pass follows local step next_diag - 1
     int rec = 0;
-    bool tail_sync = false;
     for (int s = 0; s < nsteps; ++s) {
         PackCoef<T> kc;
         kc.template set<2>(coefs.k[s]);
         const bool odd = (s & 1) != 0;
         const T* const src = odd ? buf1 : buf0;
         T* const dst = odd ? buf0 : buf1;
-        const T* const src_below = odd ? below1 : below0;
-        const T* const src_above = odd ? above1 : above0;
+        const unsigned slot = odd ? 1u : 0u, nslot = slot ^ 1u;      // the halo slot read in this step / filled for the next
+        const T* const src_below = halo + (slot * 2u) * N;
+        const T* const src_above = halo + (slot * 2u + 1u) * N;
+        const unsigned par = (unsigned)((s - 1) >> 1) & 1u;          // the slot's use that holds phi^s (s >= 1)
 #pragma unroll
         for (int k = 0; k < VPT; ++k) {
             const int v = t + k * CLUSTER_THREADS;
             if (v < RNQ) {
                 const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
                 const int o = r * N + x;
-                const V ym = (r > 0) ? *reinterpret_cast<const V*>(src + o - N)
-                                     : *reinterpret_cast<const V*>(src_below + (R - 1) * N + x);
-                const V yp = (r < R - 1) ? *reinterpret_cast<const V*>(src + o + N)
-                                         : *reinterpret_cast<const V*>(src_above + x);
+                if (s > 0 && r == 0) {                               // the neighbours' rows of phi^s have landed?
+                    halo_wait(bars + 16u * slot, par);
+                    if (x == 0) halo_arm(bars + 16u * slot, row_bytes);               // for the slot's next use, two steps on
+                }
+                if (s > 0 && r == R - 1) {
+                    halo_wait(bars + 16u * slot + 8u, par);
+                    if (x == 0) halo_arm(bars + 16u * slot + 8u, row_bytes);
+                }
+                const V ym = (r > 0) ? *reinterpret_cast<const V*>(src + o - N) : *reinterpret_cast<const V*>(src_below + x);
+                const V yp = (r < R - 1) ? *reinterpret_cast<const V*>(src + o + N) : *reinterpret_cast<const V*>(src_above + x);
                 const T left = src[r * N + (x == 0 ? N - 1 : x - 1)];
                 const T right = src[r * N + (x + W == N ? 0 : x + W)];
                 V pn, vn;
                 packed_vector_update<T, 2, ARITH>(kc, creg[k], left, right, ym, yp, V{}, V{}, pdreg[k], pn, vn);
                 creg[k] = pn; pdreg[k] = vn;
                 *reinterpret_cast<V*>(dst + o) = pn;
+                const unsigned off = ((nslot * 2u) * (unsigned)N + (unsigned)x) * (unsigned)sizeof(T);
+                if (r == 0) halo_push(push_down_halo + off, push_down_bar + 16u * nslot, pn);
+                if (r == R - 1) halo_push(push_up_halo + off, push_up_bar + 16u * nslot, pn);
             }
         }
-        // everyone has published phi^{n+1} and is done reading phi^n, whose buffer is overwritten next step
+        // this CTA has published phi^{s+1} to itself and is done reading phi^s, whose buffer is overwritten next step
         PRS_JITTER(1u + s);
-        cluster_barrier();
+        __syncthreads();
         PRS_JITTER(80u + s);
         if (s + 1 == next_diag) {
-            // ---- Eqs. 7-8 on the state just reached: own sites in registers, neighbours in dst (and the CTAs beside)
+            // ---- Eqs. 7-8 on the state just reached: own sites in registers, neighbours in dst and in the halo slot just filled
             const T* const cur = dst;
-            const T* const cur_below = odd ? below0 : below1;
-            const T* const cur_above = odd ? above0 : above1;
-            DiagPartial acc = {0ull, 0ull, 0.0};
+            const T* const cur_below = halo + (nslot * 2u) * N;
+            const T* const cur_above = halo + (nslot * 2u + 1u) * N;
+            const unsigned dpar = (unsigned)(s >> 1) & 1u;
+            unsigned acc_links = 0u, acc_walls = 0u;
+            double acc_sum = 0.0;
 #pragma unroll
             for (int k = 0; k < VPT; ++k) {
                 const int v = t + k * CLUSTER_THREADS;
                 if (v < RNQ) {
                     const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
                     const int o = r * N + x;
+                    if (r == 0) halo_wait(bars + 16u * nslot, dpar);              // (armed again by the next step, not here)
+                    if (r == R - 1) halo_wait(bars + 16u * nslot + 8u, dpar);
                     const typename O::V c = plain_vec(creg[k]);
                     const typename O::V q = plain_vec(pdreg[k]);
                     const typename O::V ym = (r > 0) ? *reinterpret_cast<const typename O::V*>(cur + o - N)
-                                                     : *reinterpret_cast<const typename O::V*>(cur_below + (R - 1) * N + x);
+                                                     : *reinterpret_cast<const typename O::V*>(cur_below + x);
                     const typename O::V yp = (r < R - 1) ? *reinterpret_cast<const typename O::V*>(cur + o + N)
                                                          : *reinterpret_cast<const typename O::V*>(cur_above + x);
                     const unsigned l = Ar<T>::neg(cur[r * N + (x == 0 ? N - 1 : x - 1)]) ? 1u : 0u;
@@ -172,31 +255,26 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
                     const unsigned mc = sign_mask<T>(c);
                     unsigned nlinks, wallmask;
                     mask_links<W, 2>(mc, l, rr, sign_mask<T>(ym), sign_mask<T>(yp), mc, mc, nlinks, wallmask);
-                    acc.links += nlinks;
-                    acc.walls += __popc(wallmask);
+                    acc_links += nlinks;
+                    acc_walls += (unsigned)__popc(wallmask);
 #pragma unroll
                     for (int i = 0; i < W; ++i)
-                        if ((wallmask >> i) & 1u) acc.sum = __dadd_rn(acc.sum, wall_ratio<T>(O::get(c, i), O::get(q, i), dg.V0, dg.I));
+                        if ((wallmask >> i) & 1u) acc_sum = __dadd_rn(acc_sum, wall_ratio<T>(O::get(c, i), O::get(q, i), dg.V0, dg.I));
                 }
             }
-            acc = block_reduce(acc);
-            if (t == 0) cta_part = acc;
+            // The pass ends inside the WARP, without a barrier: one redux for both counts (16 bits each are plenty for a
+            // warp's 32 x VPT vectors), a shuffle tree for the double, and the warp's partial waits in shared memory for
+            // the end of the launch, where all passes are added up behind one __syncthreads and ONE cluster barrier (a block
+            // reduction and a cluster barrier per pass cost 2.5 us a pass, 3.5 steps' worth).
+            const unsigned counts = __reduce_add_sync(0xffffffffu, acc_links | (acc_walls << 16));
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) acc_sum = __dadd_rn(acc_sum, __shfl_down_sync(0xffffffffu, acc_sum, d));
+            if ((t & 31) == 0) {
+                ClusterWarpPart wp;
+                wp.links = counts & 0xffffu; wp.walls = counts >> 16; wp.sum = acc_sum;
+                warp_part[rec * (CLUSTER_THREADS / 32) + (t >> 5)] = wp;
+            }
             PRS_JITTER(160u + s);
-            cluster_barrier();
-            if (rank == 0 && t < 32) {
-                // warp 0 of rank 0: lane l fetches CTA l's partial (the remote reads overlap instead of queueing up), then
-                // the shuffle tree of warp_reduce adds them -- an order fixed by the lane numbers alone: reproducible
-                DiagPartial part = {0ull, 0ull, 0.0};
-                if (t < NCTA) {
-                    const DiagPartial* rp = cluster.map_shared_rank(&cta_part, (unsigned)t);
-                    part.links = rp->links; part.walls = rp->walls; part.sum = rp->sum;
-                }
-                part = warp_reduce(part);
-                if (t == 0) dg.records[rec] = part;
-            }
-            // cta_part is written again only after a further cluster barrier, which rank 0's thread 0 joins after it has
-            // read the partials; but no CTA may EXIT while rank 0 still reads its shared memory: see tail_sync
-            tail_sync = (s + 1 == nsteps);
             ++rec;
             next_diag += dg.every;
         }
@@ -207,9 +285,43 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
         if (v < RNQ) {
             K::stg(phi_out + base + (size_t)v * W, creg[k]);
             K::stg(phidot_out + base + (size_t)v * W, pdreg[k]);
+            // the neighbours' pushes of the last step land in this CTA's shared memory: it must outlive them
+            if (nsteps > 0) {
+                const unsigned fslot = (unsigned)nsteps & 1u, fpar = (unsigned)((nsteps - 1) >> 1) & 1u;
+                const int r = v >> lgNQ;
+                if (r == 0) halo_wait(bars + 16u * fslot, fpar);
+                if (r == R - 1) halo_wait(bars + 16u * fslot + 8u, fpar);
+            }
         }
     }
-    if (tail_sync) cluster_barrier();                                   // a pass after the last step: rank 0 is done reading
+    if (rec > 0) {
+        const int lane = t & 31;
+        __syncthreads();                                             // the warps' partials of every pass are written
+        // warp w adds up passes w, w + 32: lane l takes warp l's partial, then the shuffle tree -- a fixed order
+        for (int w = t >> 5; w < rec; w += CLUSTER_THREADS / 32) {
+            const ClusterWarpPart wp = warp_part[w * (CLUSTER_THREADS / 32) + lane];
+            DiagPartial part = {(unsigned long long)wp.links, (unsigned long long)wp.walls, wp.sum};
+            part = warp_reduce(part);
+            if (lane == 0) cta_part[w] = part;
+        }
+        PRS_JITTER(200u);
+        cluster_barrier();                                           // every CTA's partials are written
+        if (rank == 0) {
+            // warp w of rank 0 takes passes w, w + 32: lane l fetches CTA l's partial (the remote reads overlap instead of
+            // queueing up), then the shuffle tree of warp_reduce adds them -- an order fixed by the lane numbers alone
+            for (int w = t >> 5; w < rec; w += CLUSTER_THREADS / 32) {
+                DiagPartial part = {0ull, 0ull, 0.0};
+                if (lane < NCTA) {
+                    const DiagPartial* rp = cluster.map_shared_rank(&cta_part[w], (unsigned)lane);
+                    part.links = rp->links; part.walls = rp->walls; part.sum = rp->sum;
+                }
+                part = warp_reduce(part);
+                if (lane == 0) dg.records[w] = part;
+            }
+        }
+        PRS_JITTER(240u);
+        cluster_barrier();                                           // no CTA exits while rank 0 reads its shared memory
+    }
 }
 
 }  // namespace prs
