@@ -330,6 +330,15 @@ def run_gpu(args):
                                                                 "roofline", "gpu_launches", "last_diag")}}
         except Exception as exc:
             also = {"3d_1024_f64_rad": {"error": str(exc)[:200]}}
+        # ---- and BASELINE.json's configs[0] (2D 256^2 FP32, diagnostics every 10 steps): launch- and latency-bound, so what
+        # counts is microseconds per PRS step of the whole cycle (small_lattice), not an HBM fraction
+        try:
+            tiny = time_leg(args, "2d_256_f32_rad", 3, 3, world, rank, local, barrier, with_e2e=False, sample_clocks=False)
+            also["2d_256_f32_rad"] = {k: tiny[k] for k in ("value", "unit", "dtype", "steps", "warmup", "ms_per_step",
+                                                            "gpu_launches", "last_diag", "small_lattice")}
+            also["2d_256_f32_rad"]["step_kernel"] = tiny["roofline"]["kernel"]
+        except Exception as exc:
+            also["2d_256_f32_rad"] = {"error": str(exc)[:200]}
 
     # ---- oracle on the host cores, rank 0, N=1 only: the workload's own lattice, the cycle's cadence
     cpu = None

@@ -3,6 +3,7 @@
     python -m tests.profile_small_kernels diag      # 1024^3 FP32 on a formed network: sign_bits_kernel + bit_links_kernel,
                                                     # then prs_weighted_area on the same bits (bit_area_kernel)
     python -m tests.profile_small_kernels cluster   # 256^2 FP32, prs_run at cadence 10: step2d_cluster_kernel on 16 CTAs
+    python -m tests.profile_small_kernels cluster1  # the same at cadence 1: a launch is 64 steps and 64 diagnostics passes
 """
 import sys
 
@@ -23,7 +24,11 @@ def main():
     else:
         sim = prs.Simulation(2, 256, prs.F32, seed=1)
         sim.init(1.0)
-        recs = sim.run(127, 10)                             # BASELINE.json configs[0]: eta 1 -> 128, diagnostics every 10 steps
+        if what == "cluster1":
+            sim.step(300)
+            recs = sim.run(128, 1)
+        else:
+            recs = sim.run(127, 10)                         # BASELINE.json configs[0]: eta 1 -> 128, diagnostics every 10 steps
         print("cluster ok: %s, %d records, last link_count %d" % (sim.step_launch_info()["kernel"], len(recs), recs[-1]["link_count"]))
     sim.close()
     return 0
