@@ -89,9 +89,9 @@ enum {
     PRS_KERNEL_TILED   = 2,    /* shared-memory tiled, one step per pass over HBM                  */
     PRS_KERNEL_TB2     = 3,    /* temporally blocked: two steps per pass over HBM (same per-site   *
                                 * arithmetic, bit-identical to two single steps)                   */
-    PRS_KERNEL_CLUSTER = 5,    /* small 2D boxes (N = 64, 128, 256): the state stays in the shared   *
-                                * memory and registers of one 8-CTA thread-block cluster for up to 64 steps per    *
-                                * launch; bit-identical to single steps                              */
+    PRS_KERNEL_CLUSTER = 5,    /* small 2D boxes (N = 64, 128, 256): the state stays in the registers and shared *
+                                * memory of one thread-block cluster of 8 (N = 256: 16) CTAs for up to 64 steps per  *
+                                * launch; bit-identical to single steps; what AUTO takes at these sizes          */
     PRS_KERNEL_BITS    = 6,    /* PRS_OPT_DIAG_KERNEL only: diagnostics on packed sign bits -- one pass reads phi   *
                                 * and packs a bit per site, a second counts links and wall sites on the bit words *
                                 * and fetches phidot at wall sites only; N a multiple of 32 16-byte vectors; what *
@@ -153,7 +153,7 @@ int prs_diagnostics(prs_handle h, prs_diag* out);
  * partial sums is what hurts small boxes).  out: HOST array of ncycles records, out[i] = what prs_diagnostics would
  * have returned after (i + 1) * steps_per_cycle further steps: the fields and the integer counts identical, and
  * sum_ratio identical too (the same kernels in the same launch configuration) except where the cluster-resident
- * small-box kernel is the step kernel (2D, N = 64 or 128 by default): there the diagnostics passes run INSIDE the step
+ * small-box kernel is the step kernel (2D, N = 64, 128 or 256 by default): there the diagnostics passes run INSIDE the step
  * launches, up to 64 steps and all their passes per launch with the state on chip throughout, and sum_ratio differs
  * from prs_diagnostics' by the order of its double additions (about 1e-15 relative).  Synchronises the stream before
  * it returns.  Not on a slab (PRS_ERR_UNSUPPORTED). */

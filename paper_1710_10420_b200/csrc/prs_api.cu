@@ -114,7 +114,8 @@ bool tbs_supported(const prs_ctx* h) {
     return h->dims == 3 ? nv <= ((size_t)1 << 31) : nv < ((size_t)1 << 30);     // the 2D kernel's cursors are signed
 }
 
-// The cluster-resident small-box kernel: 2D, whole rows per 1024-thread sweep, state in 8 CTAs' shared memory.
+// The cluster-resident small-box kernel: 2D, whole rows per 1024-thread sweep, state in the registers and shared memory
+// of 8 or 16 CTAs.
 bool cluster_supported(const prs_ctx* h) {
     if (h->dims != 2 || (h->N != 64 && h->N != 128 && h->N != 256)) return false;
     const size_t smem = (h->precision == PRS_F32) ? cluster_smem_bytes<float>((int)h->N) : cluster_smem_bytes<double>((int)h->N);
@@ -153,8 +154,8 @@ int resolve_step_kernel(const prs_ctx* h) {
         // 128^3 up -- on small lattices because it needs a quarter of the launches, on large ones
         // because it moves a quarter of the bytes; below that the single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        // the cluster-resident kernel against the streaming one, us per step (FP32 | FP64): 64^2 0.58 | 0.58 vs 1.03 | 1.03;
-        // 128^2 0.71 | 0.96 vs 1.03 | 1.34; 256^2 on 16 CTAs 0.96 | 1.44 vs 1.09 | 1.37 (on 8 CTAs 1.50 | 3.0)
+        // the cluster-resident kernel against the streaming one, us per step (FP32 | FP64): 64^2 0.39 | 0.40 vs 1.03 | 1.03;
+        // 128^2 0.48 | 0.68 vs 1.03 | 1.28; 256^2 on 16 CTAs 0.72 | 1.25 vs 1.05 | 1.37 (on 8 CTAs 1.35 | 2.4)
         else if ((h->N == 64 || h->N == 128) && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;
         else if (h->N == 256 && h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h)) want = PRS_KERNEL_CLUSTER;
         else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
@@ -771,11 +772,7 @@ int prs_run(prs_handle h, int64_t ncycles, int64_t steps_per_cycle, prs_diag* ou
         const int64_t batch = std::min<int64_t>(ncycles - done, RESULTS_CAP);
         host.resize((size_t)batch);
         steps.resize((size_t)batch);
-        // (256^2 FP64: stepping alone the streaming kernel is a little faster, 1.37 against 1.44 us, but a cycle with its
-        // diagnostics inside the cluster launch wins up to a cadence of 50 and beyond: 1.75 against 2.11 at 10, 1.51 against 1.58 at 50)
-        const bool run_on_cluster = resolve_step_kernel(h) == PRS_KERNEL_CLUSTER ||
-                                    (h->opt_step_kernel == PRS_KERNEL_AUTO && h->dims == 2 && h->N == 256 && steps_per_cycle <= 64 &&
-                                     h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h));
+        const bool run_on_cluster = resolve_step_kernel(h) == PRS_KERNEL_CLUSTER;
         if (run_on_cluster && steps_per_cycle > 0) {
             // small 2D boxes: the cluster-resident kernel runs the diagnostics passes inside its launches -- up to 64
             // steps and all their passes per launch, the state never leaving the chip in between

@@ -238,12 +238,13 @@ def test_two_rows_per_thread_kernel_equals_single_steps_bitwise(prec, N, S):
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("N", [64, 128, 256])
 def test_cluster_resident_kernel_equals_single_steps_bitwise(prec, N):
-    """Small-box kernel (state in the shared memory of one 8-CTA cluster, neighbour rows through
-    distributed shared memory, one cluster barrier per step): 1, 2, 31, 32, 33, 75 and 130 steps (launches of
-    at most 64) against the single-step kernel, all arithmetic forms; and against the oracle."""
+    """Small-box kernel (state in the registers and shared memory of one cluster of 8 or 16 CTAs, the rows across a CTA
+    boundary pushed into the neighbour's shared memory with st.async on mbarriers whose phase flips every second step):
+    1 to 9, 31, 32, 33, 75 and 130 steps (launches of at most 64) against the single-step kernel, all arithmetic forms;
+    and against the oracle."""
     phi, pd = fg.random_state(2, N, 5, NP[prec])
     for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
-        for nsteps in (1, 2, 31, 32, 33, 75, 130) if arith == prs.ARITH_FMA else (33,):
+        for nsteps in (1, 2, 3, 4, 5, 6, 7, 8, 9, 31, 32, 33, 75, 130) if arith == prs.ARITH_FMA else (33,):
             outs = []
             for kernel in (prs.KERNEL_TILED, prs.KERNEL_CLUSTER):
                 g = prs.Simulation(2, N, prec, era_m=2.0)
