@@ -120,8 +120,7 @@ struct ClusterWarpPart {
 
 template <typename T>
 constexpr size_t cluster_smem_bytes(int N, int ncta = CLUSTER_CTAS) {
-    return (size_t)2 * (size_t)(N / ncta) * (size_t)N * sizeof(T)                   // phi, ping and pong
-           + (size_t)4 * (size_t)N * sizeof(T)                                      // halo rows: 2 slots x (below, above)
+    return (size_t)2 * (size_t)(N / ncta + 2) * (size_t)N * sizeof(T)               // phi, ping and pong, each with its two halo rows
            + (size_t)CLUSTER_MAX_STEPS * (CLUSTER_THREADS / 32) * sizeof(ClusterWarpPart);      // the warps' partials, per pass
 }
 
@@ -133,21 +132,22 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char cluster_smem[];
     __shared__ DiagPartial cta_part[CLUSTER_MAX_STEPS];              // this CTA's partials of the launch's diagnostics passes
-    __shared__ __align__(8) unsigned long long halo_bar[2][2];       // [slot][0: the row below arrives here, 1: the row above]
+    __shared__ __align__(8) unsigned long long halo_bar[2][2];       // [buffer][0: the row below arrives here, 1: the row above]
     using K = Pk<T>;
     using V = typename K::V;
     using O = VecOps<T>;
     constexpr int W = K::W;
     const int R = N / NCTA;                                          // rows held by this CTA
     const int RN = R * N;
-    // (scalars picked by selects, not arrays indexed by the step's parity: those would live in local memory)
+    // Two phi buffers of R + 2 rows: row 0 is the halo row below the CTA's rows (the last row of the CTA below, pushed by
+    // that CTA), rows 1 .. R its own, row R + 1 the halo row above.  A site's y neighbours are at -N and +N whatever the row.
+    const int BUF = (R + 2) * N;
     T* const buf0 = reinterpret_cast<T*>(cluster_smem);
-    T* const buf1 = buf0 + RN;
-    T* const halo = buf1 + RN;                                       // halo[(slot * 2 + side) * N + x]
-    ClusterWarpPart* const warp_part = reinterpret_cast<ClusterWarpPart*>(halo + 4 * N);      // [pass][warp]
+    T* const buf1 = buf0 + BUF;
+    ClusterWarpPart* const warp_part = reinterpret_cast<ClusterWarpPart*>(buf1 + BUF);           // [pass][warp]
     const unsigned rank = cluster.block_rank();
     const unsigned below = (rank + NCTA - 1) % NCTA, above = (rank + 1) % NCTA;
-    const unsigned row_bytes = (unsigned)N * (unsigned)sizeof(T);
+    const unsigned row_bytes = (unsigned)N * (unsigned)sizeof(T), buf_bytes = (unsigned)BUF * (unsigned)sizeof(T);
 
     const int t = threadIdx.x;
     const int NQ = N / W, RNQ = R * NQ;                              // NQ is a power of two (N = 64, 128, 256)
@@ -157,31 +157,42 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
     if (t == 0) {
         for (unsigned i = 0; i < 4; ++i) halo_bar_init(bars + 8u * i);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-        for (unsigned i = 0; i < 4; ++i) halo_arm(bars + 8u * i, row_bytes);       // slot 1: the pushes of step 0, slot 0: of step 1
+        for (unsigned i = 0; i < 4; ++i) halo_arm(bars + 8u * i, row_bytes);       // buffer 1: the pushes of step 0, buffer 0: of step 1
     }
-    // where this CTA's first row goes: the "above" halo of the CTA below it; its last row: the "below" halo of the CTA above
-    const unsigned push_down_halo = cluster_map(cluster_smem_u32(halo + N), below);
+    // where this CTA's first row goes: the halo row above the rows of the CTA below it (row R + 1 there); its last row: the
+    // halo row below the rows of the CTA above (row 0 there) -- addresses in buffer 0, buffer 1 is buf_bytes further
+    const unsigned push_down = cluster_map(cluster_smem_u32(buf0 + (R + 1) * N), below);
     const unsigned push_down_bar = cluster_map(bars + 8u, below);
-    const unsigned push_up_halo = cluster_map(cluster_smem_u32(halo), above);
+    const unsigned push_up = cluster_map(cluster_smem_u32(buf0), above);
     const unsigned push_up_bar = cluster_map(bars, above);
 
-    // A thread owns vectors v = t, t + 1024, ... of the CTA's R x NQ: phi and phidot stay in registers.
+    // A thread owns vectors v = t, t + 1024, ... of the CTA's R x NQ: phi and phidot stay in registers; what does not change
+    // from step to step -- where the vector and its x neighbours sit in a buffer, whether it is in a boundary row -- is
+    // worked out once.
     V creg[VPT], pdreg[VPT];
+    int oc[VPT], ol[VPT], orr[VPT];
+    bool first[VPT], last[VPT];
 #pragma unroll
     for (int k = 0; k < VPT; ++k) {
         const int v = t + k * CLUSTER_THREADS;
+        const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
+        oc[k] = (r + 1) * N + x;
+        ol[k] = (r + 1) * N + (x == 0 ? N - 1 : x - 1);
+        orr[k] = (r + 1) * N + (x + W == N ? 0 : x + W);
+        first[k] = (v < RNQ) && r == 0;
+        last[k] = (v < RNQ) && r == R - 1;
         creg[k] = V{}; pdreg[k] = V{};
         if (v < RNQ) {
             creg[k] = K::ldg(phi + base + (size_t)v * W);
             pdreg[k] = K::ldg(phidot + base + (size_t)v * W);
-            reinterpret_cast<V*>(buf0)[v] = creg[k];
+            *reinterpret_cast<V*>(buf0 + oc[k]) = creg[k];
         }
     }
     if (t < 2 * NQ) {
-        // slot 0 of the halo for step 0: the rows around this CTA's rows straight from global memory (periodic in y)
+        // the halo rows of buffer 0 for step 0: the rows around this CTA's rows straight from global memory (periodic in y)
         const int side = t >> lgNQ, q = t & (NQ - 1);
         const int grow = side == 0 ? ((int)rank * R + N - 1) % N : ((int)rank * R + R) % N;
-        reinterpret_cast<V*>(halo + side * N)[q] = K::ldg(phi + (size_t)grow * N + (size_t)q * W);
+        reinterpret_cast<V*>(buf0 + side * (R + 1) * N)[q] = K::ldg(phi + (size_t)grow * N + (size_t)q * W);
     }
     cluster_barrier();                                               // the state is on chip; every CTA's mbarriers are armed
 
@@ -193,35 +204,31 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
         const bool odd = (s & 1) != 0;
         const T* const src = odd ? buf1 : buf0;
         T* const dst = odd ? buf0 : buf1;
-        const unsigned slot = odd ? 1u : 0u, nslot = slot ^ 1u;      // the halo slot read in this step / filled for the next
-        const T* const src_below = halo + (slot * 2u) * N;
-        const T* const src_above = halo + (slot * 2u + 1u) * N;
-        const unsigned par = (unsigned)((s - 1) >> 1) & 1u;          // the slot's use that holds phi^s (s >= 1)
+        const unsigned sbar = bars + (odd ? 16u : 0u);               // the barriers of the buffer read in this step
+        const unsigned par = (unsigned)((s - 1) >> 1) & 1u;          // the buffer's use that holds phi^s (s >= 1)
+        const unsigned dpush = odd ? 0u : buf_bytes, dbar = odd ? 0u : 16u;          // the buffer filled for the next step
 #pragma unroll
         for (int k = 0; k < VPT; ++k) {
-            const int v = t + k * CLUSTER_THREADS;
-            if (v < RNQ) {
-                const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
-                const int o = r * N + x;
-                if (s > 0 && r == 0) {                               // the neighbours' rows of phi^s have landed?
-                    halo_wait(bars + 16u * slot, par);
-                    if (x == 0) halo_arm(bars + 16u * slot, row_bytes);               // for the slot's next use, two steps on
+            if (t + k * CLUSTER_THREADS < RNQ) {
+                if (s > 0 && first[k]) {                             // the neighbour's row of phi^s has landed?
+                    halo_wait(sbar, par);
+                    if (ol[k] != oc[k] - 1) halo_arm(sbar, row_bytes);               // (the thread at x = 0) for the next use, two steps on
                 }
-                if (s > 0 && r == R - 1) {
-                    halo_wait(bars + 16u * slot + 8u, par);
-                    if (x == 0) halo_arm(bars + 16u * slot + 8u, row_bytes);
+                if (s > 0 && last[k]) {
+                    halo_wait(sbar + 8u, par);
+                    if (ol[k] != oc[k] - 1) halo_arm(sbar + 8u, row_bytes);
                 }
-                const V ym = (r > 0) ? *reinterpret_cast<const V*>(src + o - N) : *reinterpret_cast<const V*>(src_below + x);
-                const V yp = (r < R - 1) ? *reinterpret_cast<const V*>(src + o + N) : *reinterpret_cast<const V*>(src_above + x);
-                const T left = src[r * N + (x == 0 ? N - 1 : x - 1)];
-                const T right = src[r * N + (x + W == N ? 0 : x + W)];
+                const V ym = *reinterpret_cast<const V*>(src + oc[k] - N);
+                const V yp = *reinterpret_cast<const V*>(src + oc[k] + N);
+                const T left = src[ol[k]];
+                const T right = src[orr[k]];
                 V pn, vn;
                 packed_vector_update<T, 2, ARITH>(kc, creg[k], left, right, ym, yp, V{}, V{}, pdreg[k], pn, vn);
                 creg[k] = pn; pdreg[k] = vn;
-                *reinterpret_cast<V*>(dst + o) = pn;
-                const unsigned off = ((nslot * 2u) * (unsigned)N + (unsigned)x) * (unsigned)sizeof(T);
-                if (r == 0) halo_push(push_down_halo + off, push_down_bar + 16u * nslot, pn);
-                if (r == R - 1) halo_push(push_up_halo + off, push_up_bar + 16u * nslot, pn);
+                *reinterpret_cast<V*>(dst + oc[k]) = pn;
+                // (x * sizeof(T): the vector's offset within its row = its offset in the buffer minus the row's)
+                if (first[k]) halo_push(push_down + dpush + (unsigned)(oc[k] - N) * (unsigned)sizeof(T), push_down_bar + dbar, pn);
+                if (last[k]) halo_push(push_up + dpush + (unsigned)(oc[k] - RN) * (unsigned)sizeof(T), push_up_bar + dbar, pn);
             }
         }
         // this CTA has published phi^{s+1} to itself and is done reading phi^s, whose buffer is overwritten next step
@@ -229,29 +236,24 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
         __syncthreads();
         PRS_JITTER(80u + s);
         if (s + 1 == next_diag) {
-            // ---- Eqs. 7-8 on the state just reached: own sites in registers, neighbours in dst and in the halo slot just filled
+            // ---- Eqs. 7-8 on the state just reached: own sites in registers, neighbours in dst, whose halo rows the
+            // neighbours have just filled (or are filling)
             const T* const cur = dst;
-            const T* const cur_below = halo + (nslot * 2u) * N;
-            const T* const cur_above = halo + (nslot * 2u + 1u) * N;
+            const unsigned cbar = bars + (odd ? 0u : 16u);
             const unsigned dpar = (unsigned)(s >> 1) & 1u;
             unsigned acc_links = 0u, acc_walls = 0u;
             double acc_sum = 0.0;
 #pragma unroll
             for (int k = 0; k < VPT; ++k) {
-                const int v = t + k * CLUSTER_THREADS;
-                if (v < RNQ) {
-                    const int r = v >> lgNQ, x = (v & (NQ - 1)) * W;
-                    const int o = r * N + x;
-                    if (r == 0) halo_wait(bars + 16u * nslot, dpar);              // (armed again by the next step, not here)
-                    if (r == R - 1) halo_wait(bars + 16u * nslot + 8u, dpar);
+                if (t + k * CLUSTER_THREADS < RNQ) {
+                    if (first[k]) halo_wait(cbar, dpar);             // (armed again by the next step, not here)
+                    if (last[k]) halo_wait(cbar + 8u, dpar);
                     const typename O::V c = plain_vec(creg[k]);
                     const typename O::V q = plain_vec(pdreg[k]);
-                    const typename O::V ym = (r > 0) ? *reinterpret_cast<const typename O::V*>(cur + o - N)
-                                                     : *reinterpret_cast<const typename O::V*>(cur_below + x);
-                    const typename O::V yp = (r < R - 1) ? *reinterpret_cast<const typename O::V*>(cur + o + N)
-                                                         : *reinterpret_cast<const typename O::V*>(cur_above + x);
-                    const unsigned l = Ar<T>::neg(cur[r * N + (x == 0 ? N - 1 : x - 1)]) ? 1u : 0u;
-                    const unsigned rr = Ar<T>::neg(cur[r * N + (x + W == N ? 0 : x + W)]) ? 1u : 0u;
+                    const typename O::V ym = *reinterpret_cast<const typename O::V*>(cur + oc[k] - N);
+                    const typename O::V yp = *reinterpret_cast<const typename O::V*>(cur + oc[k] + N);
+                    const unsigned l = Ar<T>::neg(cur[ol[k]]) ? 1u : 0u;
+                    const unsigned rr = Ar<T>::neg(cur[orr[k]]) ? 1u : 0u;
                     const unsigned mc = sign_mask<T>(c);
                     unsigned nlinks, wallmask;
                     mask_links<W, 2>(mc, l, rr, sign_mask<T>(ym), sign_mask<T>(yp), mc, mc, nlinks, wallmask);
@@ -279,6 +281,7 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
             next_diag += dg.every;
         }
     }
+    const unsigned fbar = bars + ((nsteps & 1) ? 16u : 0u), fpar = (unsigned)((nsteps - 1) >> 1) & 1u;
 #pragma unroll
     for (int k = 0; k < VPT; ++k) {
         const int v = t + k * CLUSTER_THREADS;
@@ -286,12 +289,8 @@ step2d_cluster_kernel(const T* __restrict__ phi, const T* __restrict__ phidot, T
             K::stg(phi_out + base + (size_t)v * W, creg[k]);
             K::stg(phidot_out + base + (size_t)v * W, pdreg[k]);
             // the neighbours' pushes of the last step land in this CTA's shared memory: it must outlive them
-            if (nsteps > 0) {
-                const unsigned fslot = (unsigned)nsteps & 1u, fpar = (unsigned)((nsteps - 1) >> 1) & 1u;
-                const int r = v >> lgNQ;
-                if (r == 0) halo_wait(bars + 16u * fslot, fpar);
-                if (r == R - 1) halo_wait(bars + 16u * fslot + 8u, fpar);
-            }
+            if (nsteps > 0 && first[k]) halo_wait(fbar, fpar);
+            if (nsteps > 0 && last[k]) halo_wait(fbar + 8u, fpar);
         }
     }
     if (rec > 0) {
