@@ -154,8 +154,8 @@ int resolve_step_kernel(const prs_ctx* h) {
         // 128^3 up -- on small lattices because it needs a quarter of the launches, on large ones
         // because it moves a quarter of the bytes; below that the single-step march is quicker.
         if (!tiled_supported(h)) want = PRS_KERNEL_GENERIC;
-        // the cluster-resident kernel against the streaming one, us per step (FP32 | FP64): 64^2 0.39 | 0.40 vs 1.03 | 1.03;
-        // 128^2 0.48 | 0.68 vs 1.03 | 1.28; 256^2 on 16 CTAs 0.72 | 1.25 vs 1.05 | 1.37 (on 8 CTAs 1.35 | 2.4)
+        // the cluster-resident kernel against the streaming one, us per step (FP32 | FP64): 64^2 0.36 | 0.39 vs 1.03 | 1.03;
+        // 128^2 0.43 | 0.61 vs 1.03 | 1.28; 256^2 on 16 CTAs 0.71 | 1.09 vs 1.05 | 1.37 (on 8 CTAs 1.09 | 2.2)
         else if ((h->N == 64 || h->N == 128) && cluster_supported(h)) want = PRS_KERNEL_CLUSTER;
         else if (h->N == 256 && h->opt_cluster_ctas != 8 && cluster_supported(h) && cluster16_fits(h)) want = PRS_KERNEL_CLUSTER;
         else if (tbs_supported(h) && ((h->dims == 2 && h->N >= 64) || (h->dims == 3 && h->N >= 128))) want = PRS_KERNEL_TBS;
