@@ -953,6 +953,49 @@ def test_batched_cycles_equal_the_step_and_diagnostics_loop(dims, N, prec, every
     b.close()
 
 
+@pytest.mark.parametrize("dims,N,prec", [(2, 256, prs.F32), (2, 128, prs.F64), (2, 1024, prs.F32), (3, 64, prs.F32)])
+def test_handles_on_streams_and_threads_of_their_own_run_side_by_side(dims, N, prec):
+    """An ensemble of independent boxes on one GPU (PAPER.md:119: five seeds per configuration; :97, :111: a small box
+    under-uses the GPU): six handles, each on a stream of its own, each driven by its own host thread through prs_run,
+    all at once -- records and fields equal to the same seeds run one after the other on the default stream.  (Exercises
+    the library's process-wide state -- per-device kernel attributes, the 16-CTA cluster probe -- under concurrent calls,
+    and clusters of different handles resident on the GPU together.)"""
+    import threading
+
+    import torch
+
+    boxes, ncyc, every = 6, 12, 10
+    want = []
+    for i in range(boxes):
+        g = prs.Simulation(dims, N, prec, seed=40 + i)
+        g.init(1.0)
+        want.append((g.run(ncyc, every), g.copy_out()))
+        g.close()
+    streams = [torch.cuda.Stream() for _ in range(boxes)]
+    sims = [prs.Simulation(dims, N, prec, seed=40 + i, stream=streams[i]) for i in range(boxes)]
+    got, errors = [None] * boxes, []
+
+    def drive(i):
+        try:
+            sims[i].init(1.0)
+            got[i] = sims[i].run(ncyc, every)
+        except Exception as exc:                                 # pragma: no cover - reported below
+            errors.append(exc)
+
+    threads = [threading.Thread(target=drive, args=(i,)) for i in range(boxes)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for i in range(boxes):
+        assert got[i] == want[i][0], i
+        a = sims[i].copy_out()
+        assert a[0].tobytes() == want[i][1][0].tobytes() and a[1].tobytes() == want[i][1][1].tobytes(), i
+        sims[i].close()
+    assert len({r[-1]["link_count"] for r, _ in want}) > 1      # different seeds, different networks
+
+
 @pytest.mark.parametrize("prec", [prs.F32, prs.F64])
 @pytest.mark.parametrize("N", [64, 128, 256])
 @pytest.mark.parametrize("every,ncyc", [(10, 40), (1, 130), (64, 3), (65, 3), (7, 19), (200, 2)])
