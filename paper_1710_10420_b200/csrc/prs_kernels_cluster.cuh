@@ -1,7 +1,7 @@
 // prs_kernels_cluster.cuh -- the small-box regime (small boxes
 // under-use a GPU and are dominated by per-step overheads).  A 256^2 lattice is 768 KB of state: every
 // kernel launch of the streaming kernels is pure latency.  Here the whole state lives ON CHIP in ONE
-// thread-block cluster for many steps: 8 CTAs, each owning N/8 rows.  A thread keeps the phi and phidot
+// thread-block cluster for many steps: 8 CTAs (256^2: 16), each owning N/8 (N/16) rows.  A thread keeps the phi and phidot
 // of its own sites in REGISTERS from the first step of a launch to the last; only phi is published, to
 // a ping-pong pair of shared-memory buffers, for the neighbours: rows just across a CTA boundary are read
 // from a halo row that the neighbouring CTA fills through distributed shared memory (st.async + mbarrier, below): a
@@ -39,9 +39,9 @@ constexpr int cluster_vpt(int N, int ncta = CLUSTER_CTAS) {
     return (N / ncta) * (N / Pk<T>::W) <= CLUSTER_THREADS ? 1 : (N / ncta) * (N / Pk<T>::W) / CLUSTER_THREADS;
 }
 
-// The cluster barrier as its two halves with exactly the ordering the kernel needs: shared-memory writes before the arrive
-// are visible to every CTA of the cluster after the wait.  (cooperative_groups' cluster.sync() showed a `membar` stall of
-// 13 % in ncu: it fences more than that.)
+// The cluster barrier as its two halves: shared-memory writes before the arrive are visible to every CTA of the cluster
+// after the wait.  Used at the start and the end of a launch only: its release compiles to a MEMBAR.ALL.GPU in every warp
+// (as cooperative_groups' cluster.sync() does), 13 % `membar` stall in ncu when every step ended in one.
 __device__ __forceinline__ void cluster_barrier() {
     asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
 }
@@ -55,11 +55,12 @@ __device__ __forceinline__ void cluster_barrier() {
 // halo; everyone else needs the CTA's own __syncthreads only, so the inner rows of step s+1 run while the halo rows
 // of phi^{s+1} are in flight.
 //
-// Two halo slots alternate with the parity of the step.  Slot (s+1)&1 receives phi^{s+1} during the neighbour's step s and is
-// read in step s+1; it is written again in the neighbour's step s+2, which cannot start before this CTA's boundary row of step
-// s+1 has arrived there -- pushed by the very threads that read the slot, after they read it.  Each slot and side has its own
-// mbarrier (one arrival, by the thread that arms it with the row's byte count for the next use, plus the bytes); the arming
-// thread is one of the row's pushers and arms before it pushes, so an arming always precedes the bytes it counts.
+// The halo rows are rows 0 and R + 1 of the two phi buffers, which alternate with the parity of the step.  Those of buffer
+// (s+1)&1 receive phi^{s+1} during the neighbours' step s and are read in step s+1; they are written again in the
+// neighbours' step s+2, which cannot start before this CTA's boundary rows of step s+1 have arrived there -- pushed by the
+// very threads that read the halo rows, after they read them.  Each buffer and side has its own mbarrier (one arrival, by
+// the thread that arms it with the row's byte count for the next use, plus the bytes); the arming thread is one of the
+// row's pushers and arms before it pushes, so an arming always precedes the bytes it counts.
 __device__ __forceinline__ unsigned cluster_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ unsigned cluster_map(unsigned local, unsigned rank) {
     unsigned remote;
