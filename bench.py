@@ -118,7 +118,8 @@ def ncu_traffic_for(launch):
         return None, "no capture record (%s)" % exc
     for c in captures:
         if c["kernel"] == launch["kernel"] and c["grid"] == launch["grid"] and c["block"] == launch["block"]:
-            return int(c["dram_bytes_read"]) + int(c["dram_bytes_write"]), "ncu capture %s" % c["profile"]
+            return (int(c["dram_bytes_read"]) + int(c["dram_bytes_write"]),
+                    "ncu capture %s" % c["profile"] + ("; " + c["note"] if c.get("note") else ""))
     return None, "no committed ncu capture of %s grid %s block %s" % (launch["kernel"], launch["grid"], launch["block"])
 
 
