@@ -152,7 +152,35 @@ cudaError_t launch_tbs_2d(prs_ctx* h, const T* p, const T* v, T* pn, T* vn) {
     // 2048^2: 6.15 us per step.)
     int YC;
     if (h->opt_chunk > 0) YC = (int)std::min<int64_t>(h->opt_chunk, N);
-    else YC = std::min<int>(N, std::max(8, std::min(128, N / 64)));
+    else {
+        YC = std::min<int>(N, std::max(8, std::min(128, N / 64)));
+        // Grids of a few waves: the last wave costs a full march however few CTAs it holds, so pick the rows per march
+        // that minimise waves x (rows marched per CTA) for the CTAs the device really holds at once (the FP32 eight-step
+        // kernel: 214 registers, two blocks per SM).  Measured on B200, FP32, us per step, N/64 rule -> this rule:
+        // 2048^2 5.25 -> 3.33 (320 CTAs on 296 slots -> 295), 4096^2 12.85 -> 10.99 (640 -> 290).
+        static std::atomic<int> occupancy[64];                     // blocks per SM of this instantiation, per device
+        const int dev = (h->device >= 0 && h->device < 64) ? h->device : 0;
+        int per_sm = occupancy[dev].load();
+        if (per_sm == 0) {
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, step2d_tbs_kernel<T, ARITH, S>, BX, 0) != cudaSuccess || per_sm < 1) {
+                cudaGetLastError();
+                per_sm = 1;
+            }
+            occupancy[dev].store(per_sm);
+        }
+        const long long slots = (long long)std::max(1, h->sm_count) * per_sm;
+        if ((long long)gx * ((N + YC - 1) / YC) <= 6 * slots) {
+            long long best_cost = -1;
+            for (long long w = 1; w <= 8; ++w) {
+                const long long gy_max = w * slots / gx;
+                if (gy_max < 1) continue;
+                const int yc = (int)std::max<long long>(8, (N + gy_max - 1) / gy_max);
+                const long long gy = (N + yc - 1) / yc;
+                const long long cost = (((long long)gx * gy + slots - 1) / slots) * (yc + 2 * S - 2);
+                if (best_cost < 0 || cost < best_cost) { best_cost = cost; YC = yc; }
+            }
+        }
+    }
     const dim3 grid(gx, (unsigned)((N + YC - 1) / YC), 1);
     // rows of L2 prefetch ahead of the load cursor: measured 16384^2 FP32 S = 6, ms per step:
     // none 0.180, 4 rows 0.154, 8 rows 0.153, 16 rows 0.163, 32 rows 0.215
