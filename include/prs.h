@@ -97,8 +97,8 @@ enum {
                                 * and fetches phidot at wall sites only; N a multiple of 32 16-byte vectors; what *
                                 * AUTO takes from 2^26 sites up                                                   */
     PRS_KERNEL_TBS     = 4     /* PRS_OPT_TBS_STEPS steps per pass over HBM (2D and 3D), bit-identical *
-                                * to single steps; leftovers of a prs_step call go through TB2 and  *
-                                * TILED                                                             */
+                                * to single steps; leftovers of a prs_step call go through the      *
+                                * shorter pipelines (6, 4, 3 steps), TB2 and TILED                  */
 };
 /* Arithmetic form of Eqs. 3-5 (R13).  LITERAL: Eq. 4 (:49) as printed, one division per
  * site, ((1-d)*v + deta*f)/(1+d).  COEF: A = (1-d)/(1+d) and B = deta/(1+d) formed in double on the

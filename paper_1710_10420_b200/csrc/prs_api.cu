@@ -698,15 +698,32 @@ static int step_impl(prs_handle h, int64_t nsteps) {
         }
     }
     if (kernel == PRS_KERNEL_TBS) {
+        // S-step launches, then the remainder in as few launches as the instances allow (a launch costs a march whatever
+        // its depth: measured at 4096^2 FP32, us per launch: 8 steps 89, 6: 71, 4: 58, 3: 61, two-step kernel 62, single
+        // step 47; at 1024^3 FP32 4 steps 4.4 ms, two-step kernel 3.1, single 2.8): 3 -> one three-step launch (was 2 + 1),
+        // 6 -> one six-step launch (was 4 + 2), 7 -> 4 + 3 (was 4 + 2 + 1); 2D FP32 only: a remainder of 2 after eight-step
+        // launches trades the last 8 + 2 for 6 + 4 (150 -> 130 us at 4096^2; the 50-step cycle of BASELINE.json's 2D configs
+        // ends that way).  What is left after this block is 0, 1 or 2 steps for the kernels below.
         const int S = h->opt_tbs_steps;
-        for (; left >= S; left -= S) {
+        int64_t mains = left / S;
+        int rem = (int)(left % S);
+        const bool trade = h->dims == 2 && h->precision == PRS_F32 && S == 8 && rem == 2 && mains >= 1;
+        if (trade) mains -= 1;
+        for (int64_t i = 0; i < mains; ++i) {
             const int rc = (h->precision == PRS_F32) ? step_many<float>(h, S) : step_many<double>(h, S);
             if (rc != PRS_OK) return rc;
         }
-        if (S > 4 && left >= 4) {                 // leftover of a long pipeline: one four-step launch first
-            const int rc = (h->precision == PRS_F32) ? step_many<float>(h, 4) : step_many<double>(h, 4);
+        left -= mains * S;
+        int parts[2] = {0, 0};
+        if (trade) { parts[0] = 6; parts[1] = 4; }
+        else if (rem == 7) { parts[0] = 4; parts[1] = 3; }
+        else if (rem == 6 && h->dims == 2) parts[0] = 6;
+        else if (rem >= 4) parts[0] = 4;                           // 4, 5 (-> 4 + 1), 6 in 3D never happens (S <= 4 there)
+        else if (rem == 3) parts[0] = 3;
+        for (int i = 0; i < 2 && parts[i] > 0; ++i) {
+            const int rc = (h->precision == PRS_F32) ? step_many<float>(h, parts[i]) : step_many<double>(h, parts[i]);
             if (rc != PRS_OK) return rc;
-            left -= 4;
+            left -= parts[i];
         }
     }
     if ((kernel == PRS_KERNEL_TB2 || kernel == PRS_KERNEL_TBS) && tb2_supported(h)) {

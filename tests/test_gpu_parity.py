@@ -197,11 +197,13 @@ def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
                 g.step(nsteps)
                 outs.append(g.copy_out())
                 assert g.get_info(binding.INFO_STEP) == 3 + nsteps
-                if kernel == prs.KERNEL_TBS:     # S-step launches, (a four-step one,) two-step ones, a single step
-                    want, rest = nsteps // S, nsteps % S
-                    if S > 4 and rest >= 4:
-                        want, rest = want + 1, rest - 4
-                    assert g.kernel_launches == want + rest // 2 + rest % 2
+                if kernel == prs.KERNEL_TBS:     # S-step launches, then the remainder in as few launches as there are instances for
+                    mains, rest = nsteps // S, nsteps % S
+                    if dims == 2 and prec == prs.F32 and S == 8 and rest == 2 and mains >= 1:
+                        extra = 1                                 # the last 8 + 2 become 6 + 4: the same number of launches
+                    else:
+                        extra = {0: 0, 1: 1, 2: 1, 3: 1, 4: 1, 5: 2, 6: 1 if dims == 2 else 2, 7: 2}[rest]
+                    assert g.kernel_launches == mains + extra, (nsteps, S)
             assert outs[0][0].tobytes() == outs[1][0].tobytes() and outs[0][1].tobytes() == outs[1][1].tobytes()
             if arith != prs.ARITH_FMA:
                 break                             # the other forms: one length is enough
