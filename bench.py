@@ -441,9 +441,10 @@ def time_leg(args, config, steps, warmup, world, rank, local, barrier, with_e2e,
     info = sim.step_launch_info()
     spl = info["steps_per_launch"]
     main_steps = (SUBSTEPS // spl) * spl
-    if dims == 2 and prec == 0 and spl == 8 and SUBSTEPS - main_steps == 2 and main_steps >= 16:
-        # prs_step(50) in 2D FP32 is 5 x 8 + 6 + 4 steps (prs_api.cu: a remainder of 2 trades the last 8 + 2 for 6 + 4):
-        # the second call must see that last eight-step launch to schedule the cycle the way one call would
+    if dims == 2 and SUBSTEPS - main_steps == 2 and main_steps >= 2 * spl and ((prec == 0 and spl == 8) or (prec == 1 and spl == 6)):
+        # prs_step(50) in 2D is 5 x 8 + 6 + 4 steps in FP32 and 7 x 6 + 8 in FP64 (prs_api.cu: a remainder of 2 trades the
+        # last 8 + 2 for 6 + 4, the last 6 + 2 for one 8): the second call must see that last main launch to schedule the
+        # cycle the way one call would
         main_steps -= spl
     main_launches = main_steps // spl
 

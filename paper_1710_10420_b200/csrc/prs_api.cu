@@ -708,7 +708,10 @@ static int step_impl(prs_handle h, int64_t nsteps) {
         int64_t mains = left / S;
         int rem = (int)(left % S);
         const bool trade = h->dims == 2 && h->precision == PRS_F32 && S == 8 && rem == 2 && mains >= 1;
-        if (trade) mains -= 1;
+        // ... and 2D FP64, whose pipeline is six deep: the last 6 + 2 become ONE eight-step launch (4096^2: 125 + 99 -> 184 us,
+        // 16384^2: 1810 + 1505 -> 2769)
+        const bool trade64 = h->dims == 2 && h->precision == PRS_F64 && S == 6 && rem == 2 && mains >= 1;
+        if (trade || trade64) mains -= 1;
         for (int64_t i = 0; i < mains; ++i) {
             const int rc = (h->precision == PRS_F32) ? step_many<float>(h, S) : step_many<double>(h, S);
             if (rc != PRS_OK) return rc;
@@ -716,6 +719,7 @@ static int step_impl(prs_handle h, int64_t nsteps) {
         left -= mains * S;
         int parts[2] = {0, 0};
         if (trade) { parts[0] = 6; parts[1] = 4; }
+        else if (trade64) parts[0] = 8;
         else if (rem == 7) { parts[0] = 4; parts[1] = 3; }
         else if (rem == 6 && h->dims == 2) parts[0] = 6;
         else if (rem >= 4) parts[0] = 4;                           // 4, 5 (-> 4 + 1), 6 in 3D never happens (S <= 4 there)

@@ -201,6 +201,8 @@ def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
                     mains, rest = nsteps // S, nsteps % S
                     if dims == 2 and prec == prs.F32 and S == 8 and rest == 2 and mains >= 1:
                         extra = 1                                 # the last 8 + 2 become 6 + 4: the same number of launches
+                    elif dims == 2 and prec == prs.F64 and S == 6 and rest == 2 and mains >= 1:
+                        extra = 0                                 # the last 6 + 2 become one eight-step launch
                     else:
                         extra = {0: 0, 1: 1, 2: 1, 3: 1, 4: 1, 5: 2, 6: 1 if dims == 2 else 2, 7: 2}[rest]
                     assert g.kernel_launches == mains + extra, (nsteps, S)
