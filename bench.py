@@ -441,10 +441,11 @@ def time_leg(args, config, steps, warmup, world, rank, local, barrier, with_e2e,
     info = sim.step_launch_info()
     spl = info["steps_per_launch"]
     main_steps = (SUBSTEPS // spl) * spl
-    if dims == 2 and SUBSTEPS - main_steps == 2 and main_steps >= 2 * spl and ((prec == 0 and spl == 8) or (prec == 1 and spl == 6)):
-        # prs_step(50) in 2D is 5 x 8 + 6 + 4 steps in FP32 and 7 x 6 + 8 in FP64 (prs_api.cu: a remainder of 2 trades the
-        # last 8 + 2 for 6 + 4, the last 6 + 2 for one 8): the second call must see that last main launch to schedule the
-        # cycle the way one call would
+    if SUBSTEPS - main_steps == 2 and main_steps >= 2 * spl and (
+            (dims == 2 and ((prec == 0 and spl == 8) or (prec == 1 and spl == 6))) or (dims == 3 and spl == 4)):
+        # prs_step(50) is 5 x 8 + 6 + 4 steps in 2D FP32, 7 x 6 + 8 in 2D FP64 and 11 x 4 + 3 + 3 in 3D (prs_api.cu: a
+        # remainder of 2 trades the last 8 + 2 for 6 + 4, the last 6 + 2 for one 8, the last 4 + 2 for 3 + 3): the second
+        # call must see that last main launch to schedule the cycle the way one call would
         main_steps -= spl
     main_launches = main_steps // spl
 

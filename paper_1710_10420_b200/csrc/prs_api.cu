@@ -711,7 +711,10 @@ static int step_impl(prs_handle h, int64_t nsteps) {
         // ... and 2D FP64, whose pipeline is six deep: the last 6 + 2 become ONE eight-step launch (4096^2: 125 + 99 -> 184 us,
         // 16384^2: 1810 + 1505 -> 2769)
         const bool trade64 = h->dims == 2 && h->precision == PRS_F64 && S == 6 && rem == 2 && mains >= 1;
-        if (trade || trade64) mains -= 1;
+        // ... and 3D (four deep): the last 4 + 2 become 3 + 3 (1024^3 FP32, ms per launch: four steps 4.48, three 3.46, the
+        // two-step kernel 3.38: 7.85 -> 6.91; the 50-step cycle of BASELINE.json's 3D configs ends that way)
+        const bool trade3d = h->dims == 3 && S == 4 && rem == 2 && mains >= 1;
+        if (trade || trade64 || trade3d) mains -= 1;
         for (int64_t i = 0; i < mains; ++i) {
             const int rc = (h->precision == PRS_F32) ? step_many<float>(h, S) : step_many<double>(h, S);
             if (rc != PRS_OK) return rc;
@@ -720,6 +723,7 @@ static int step_impl(prs_handle h, int64_t nsteps) {
         int parts[2] = {0, 0};
         if (trade) { parts[0] = 6; parts[1] = 4; }
         else if (trade64) parts[0] = 8;
+        else if (trade3d) { parts[0] = 3; parts[1] = 3; }
         else if (rem == 7) { parts[0] = 4; parts[1] = 3; }
         else if (rem == 6 && h->dims == 2) parts[0] = 6;
         else if (rem >= 4) parts[0] = 4;                           // 4, 5 (-> 4 + 1), 6 in 3D never happens (S <= 4 there)

@@ -186,7 +186,7 @@ def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
         pytest.skip("pipelines of 6 and 8 stages exist in 2D only")
     phi, pd = fg.random_state(dims, N, 5, NP[prec])
     for arith in (prs.ARITH_FMA, prs.ARITH_COEF, prs.ARITH_LITERAL):
-        for nsteps in (S, 2 * S + 1, 11, 2 * S + 7):
+        for nsteps in (S, 2 * S + 1, 2 * S + 2, 11, 2 * S + 7):
             outs = []
             for kernel in (prs.KERNEL_TILED, prs.KERNEL_TBS):
                 g = prs.Simulation(dims, N, prec, era_m=2.0)
@@ -203,6 +203,8 @@ def test_multi_step_kernel_equals_single_steps_bitwise(prec, dims, N, S):
                         extra = 1                                 # the last 8 + 2 become 6 + 4: the same number of launches
                     elif dims == 2 and prec == prs.F64 and S == 6 and rest == 2 and mains >= 1:
                         extra = 0                                 # the last 6 + 2 become one eight-step launch
+                    elif dims == 3 and S == 4 and rest == 2 and mains >= 1:
+                        extra = 1                                 # the last 4 + 2 become 3 + 3
                     else:
                         extra = {0: 0, 1: 1, 2: 1, 3: 1, 4: 1, 5: 2, 6: 1 if dims == 2 else 2, 7: 2}[rest]
                     assert g.kernel_launches == mains + extra, (nsteps, S)
